@@ -1,0 +1,590 @@
+"""Pins of the CPU oracle against things other than itself.
+
+All `-m "not gpu"`.  Each test states what fixes the expected value: a published known answer, a closed
+form, an exact integer identity, brute force in numpy from the raw state dump, or a float64 recomputation.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from helpers import decode_state, forced_single_blob, planner_bias_blob, tiny_spec, ST_RUN, ST_WAIT
+from im_workload import blob_views, lognormal_table, make_policy_blob, make_pool_spec, poisson_cdf_row
+from im_workload.workload import exponential_table_q16
+
+CN = {n: i for i, n in enumerate(
+    ["arrivals", "dropped", "finished", "solved", "missed", "calls_issued", "calls_done", "preemptions", "sum_sojourn",
+     "sum_live_mid", "plans", "exec_decisions", "sum_running", "sum_waiting", "near_boundary", "abandoned"])}
+
+
+# ---------------------------------------------------------------------------------------------- P1
+def test_p1_philox_known_answers(orc):
+    """Random123 kat_vectors for philox4x32-10 (Salmon et al., SC'11), stored in tests/golden/philox4x32_10_kat.txt."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")
+    n = 0
+    for line in open(path):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        v = [int(x, 16) for x in line.split()]
+        assert orc.philox(*v[:6]) == v[6:], line
+        n += 1
+    assert n == 3
+
+
+def test_p1_philox_counter_sensitivity(orc):
+    """Bijection sanity: flipping any single counter/key bit changes the output block."""
+    base = orc.philox(1, 2, 3, 4, 5, 6)
+    seen = {tuple(base)}
+    for pos in range(6):
+        for bit in (0, 13, 31):
+            a = [1, 2, 3, 4, 5, 6]
+            a[pos] ^= 1 << bit
+            out = tuple(orc.philox(*a))
+            assert out not in seen
+            seen.add(out)
+
+
+# ---------------------------------------------------------------------------------------- R23 / P11
+def test_r23_im_exp_accuracy(orc):
+    xs = np.concatenate([-np.random.default_rng(0).random(20000) * 80.0, [0.0, -1e-8, -79.99, -80.0]])
+    worst = 0.0
+    for x in xs:
+        got, ref = orc.im_exp(float(np.float32(x))), math.exp(float(np.float32(x)))
+        worst = max(worst, abs(got - ref) / ref)
+    assert worst < 4 * 2.0 ** -23           # <= 4 ulp (relative) against the float64 exp
+    assert orc.im_exp(-80.5) == 0.0 and orc.im_exp(0.0) == 1.0
+
+
+def test_r23_im_tanh_accuracy(orc):
+    xs = np.random.default_rng(1).normal(size=20000) * 3.0
+    worst = max(abs(orc.im_tanh(float(np.float32(x))) - math.tanh(float(np.float32(x)))) for x in xs)
+    assert worst < 3e-7                      # absolute; (1-e)/(1+e) has cancellation near 0 by construction
+    assert orc.im_tanh(0.0) == 0.0 and orc.im_tanh(50.0) == 1.0 and orc.im_tanh(-50.0) == -1.0
+    assert orc.im_tanh(-0.7) == -orc.im_tanh(0.7)
+
+
+def test_p11_sampler_closed_forms(orc):
+    rng = np.random.default_rng(2)
+    # one-hot logits => that action for every u
+    for n in (4, 15, 24, 48):
+        for a in (0, n // 2, n - 1):
+            l = np.full(n, -200.0, dtype=np.float32)
+            l[a] = 3.0
+            for u in (0.0, 0.3, 0.999999):
+                got, lp, _ = orc.sample(l, u)
+                assert got == a and abs(lp) < 1e-6
+    # equal logits => a = floor(u*n) away from the grid edges
+    for n in (4, 15, 48):
+        l = np.full(n, 0.7, dtype=np.float32)
+        for u in rng.random(500):
+            u = float(np.float32(np.floor(u * 2 ** 24) / 2 ** 24))
+            if abs(u * n - round(u * n)) < 1e-4:
+                continue
+            got, lp, _ = orc.sample(l, u)
+            assert got == int(u * n)
+            assert abs(lp + math.log(n)) < 1e-5
+
+
+def test_p11_sampler_matches_softmax_inverse_cdf(orc):
+    """Against the textbook definition in float64: a = #{j : cdf_j <= u}; chi^2 over 2e5 draws."""
+    rng = np.random.default_rng(3)
+    l = rng.normal(size=15).astype(np.float32) * 2.0
+    p = np.exp(l.astype(np.float64) - l.max())
+    p /= p.sum()
+    cdf = np.cumsum(p)
+    counts = np.zeros(15)
+    n_draw = 200000
+    us = np.floor(rng.random(n_draw) * 2 ** 24) / 2 ** 24
+    for u in us[:5000]:
+        a, lp, _ = orc.sample(l, float(u))
+        ref = int(np.searchsorted(cdf, u, side="right"))
+        if min(abs(cdf - u)) > 1e-5:
+            assert a == min(ref, 14)
+            assert abs(lp - math.log(p[a])) < 1e-5
+    # chi^2 using the oracle's own cdf output for bulk speed (one call gives the cdf)
+    _, _, c = orc.sample(l, 0.0)
+    c = c.astype(np.float64) / float(c[-1])
+    a_all = np.minimum(np.searchsorted(c, us, side="right"), 14)
+    counts = np.bincount(a_all, minlength=15)
+    chi2 = float(np.sum((counts - n_draw * p) ** 2 / (n_draw * p)))
+    assert chi2 < 45.0                       # 14 dof, p ~ 1e-5
+
+
+# ------------------------------------------------------------------------------------------ P2-P5
+def test_p2_poisson_table_and_moments(orc):
+    for m in (0.02, 0.1, 1.6, 2.8):
+        row = poisson_cdf_row(m).astype(np.int64)
+        assert np.all(np.diff(row) >= 0)
+        assert row[30] >= 2 ** 32 * (1 - 1e-9) - 1
+        # pmf recovered from the table equals the Poisson pmf
+        pmf = np.diff(np.concatenate([[0], row[:31]])) / 2.0 ** 32
+        ref = np.array([math.exp(-m) * m ** j / math.factorial(j) for j in range(31)])
+        assert np.max(np.abs(pmf - ref)) < 1e-9
+    # sample mean / variance of the oracle's arrival counts
+    spec = tiny_spec(n_envs=64, N=1, n_ticks=500, qcap=64, rcap=192, rate_tick=0.8, slots=16)
+    o = orc.Oracle(spec, seed=5)
+    o.rollout(forced_single_blob(spec), 500)
+    arr = o.counters()[:, CN["arrivals"]].astype(np.float64)
+    n = 64 * 500
+    mean = arr.sum() / n
+    assert abs(mean - 0.8) < 4 * math.sqrt(0.8 / n)
+    # per-env totals are Poisson(400): variance of totals ~ 400
+    assert abs(arr.var() / 400.0 - 1.0) < 4 * math.sqrt(2.0 / 63)
+
+
+def test_p3_budget_range_and_mean(orc):
+    spec = tiny_spec(n_envs=32, N=1, n_ticks=400, qcap=64, rcap=192, rate_tick=0.5, slots=16, budget=(40, 200), medians=(4, 4, 4))
+    o = orc.Oracle(spec, seed=7)
+    o.rollout(forced_single_blob(spec), 400)
+    b = (o.queries()["info"] & 0xFFFF).astype(np.float64)
+    assert b.size > 4000
+    assert b.min() >= 40 and b.max() <= 200 and b.min() == 40 and b.max() == 200
+    sd = math.sqrt(((200 - 40 + 1) ** 2 - 1) / 12.0)
+    assert abs(b.mean() - 120.0) < 4 * sd / math.sqrt(b.size)
+
+
+def test_p3_budget_mixture_cfg5(orc):
+    spec = make_pool_spec(5, n_envs=64, n_ticks=64)
+    o = orc.Oracle(spec, seed=0)
+    o.rollout(make_policy_blob(spec), 64)
+    st = decode_state(o.state(), spec.n_models, spec.qcap, spec.rcap)
+    b = st["q_budget"][st["q_live"] == 1].astype(np.int64)
+    tight = (b >= 100) & (b <= 300)
+    relaxed = (b >= 800) & (b <= 2400)
+    assert np.all(tight | relaxed) and b.size > 500
+    assert abs(tight.mean() - 0.5) < 4 * 0.5 / math.sqrt(b.size) + 0.08   # survivors skew relaxed; loose bound
+
+
+def test_p4_lognormal_tables():
+    m = lognormal_table(1.0, 0.4, scale=65536.0).astype(np.float64) / 65536.0
+    assert abs(m.mean() / math.exp(0.08) - 1.0) < 3e-4        # -0.013 %
+    t = lognormal_table(800.0, 0.6).astype(np.float64)
+    assert abs(t.mean() / (800 * math.exp(0.18)) - 1.0) < 8e-4
+    assert t.max() == 5784 or abs(t.max() - 5784) <= 2          # SURVEY R8 quotes max 5 784
+    assert np.all(np.diff(m) >= 0) and np.all(np.diff(t) >= 0)
+
+
+def test_p5_beta22_success_table():
+    ps = np.concatenate([make_pool_spec(4, seed=s).succ_prob.ravel() for s in range(400)])
+    assert abs(ps.mean() - 0.5) < 4 * math.sqrt(0.05 / ps.size)
+    assert abs(ps.var() - 0.05) < 0.004
+
+
+# --------------------------------------------------------------------------------------------- P6
+@pytest.mark.parametrize("lam_s", [0.3, 0.5, 0.7])
+def test_p6_mm1_mean_sojourn(orc, lam_s):
+    """Single FCFS server, Poisson arrivals, exponential job sizes: E[sojourn] = 1/(mu - lambda) (M/M/1).
+
+    rate 80 tok/s = exactly 4 tok/tick (frac = 0), mean job 80 tok => mu = 1/s = 1/20 per tick."""
+    T, E = 8000, 256
+    spec = tiny_spec(n_envs=E, N=1, n_ticks=T, qcap=64, rcap=192, rate_tick=lam_s / 20.0, slots=1, rates=[80],
+                     sched_mode=0, budget=(60000, 60000), medians=(80, 80, 80), f_in=16, hidden=8)
+    spec = spec.with_(out_tok_mult_q16=exponential_table_q16(), budget_norm_ticks=60000)
+    o = orc.Oracle(spec, seed=11)
+    o.rollout(forced_single_blob(spec), T, n_threads=8)
+    q = o.queries()
+    keep = q["arrive"] > 1000                      # discard the warm-up from empty
+    soj = q["sojourn"][keep].astype(np.float64)
+    assert soj.size > 20000
+    mean_ticks = soj.mean()
+    exact = 20.0 / (1.0 - lam_s)                   # 1/(mu-lambda) in ticks
+    assert abs(mean_ticks / exact - 1.0) < 0.05, (mean_ticks, exact)
+    # Pollaczek-Khinchine with the realised service moments (ticks of service = ceil(tokens/4), quantile table)
+    tab = np.maximum(1, (80 * exponential_table_q16().astype(np.int64)) >> 16)
+    svc = np.ceil(tab / 4.0)
+    lam_t = lam_s / 20.0
+    rho = lam_t * svc.mean()
+    pk = svc.mean() + lam_t * (svc ** 2).mean() / (2 * (1 - rho))
+    assert abs(mean_ticks / pk - 1.0) < 0.04, (mean_ticks, pk)
+    c = o.counters()
+    assert c[:, CN["dropped"]].sum() == 0
+
+
+# ------------------------------------------------------------------------------------------ P7, P8
+def _check_conservation(spec, st, c, tick_end):
+    N = spec.n_models
+    live = st["q_live"].sum(axis=1)
+    assert np.array_equal(c[:, CN["arrivals"]], c[:, CN["finished"]] + c[:, CN["dropped"]] + live + c[:, CN["abandoned"]])
+    inflight = st["n_wait"].sum(axis=1) + st["n_run"].sum(axis=1)
+    if spec.episode_ticks == 0:
+        assert np.array_equal(c[:, CN["calls_issued"]], c[:, CN["calls_done"]] + inflight)
+    for k in range(N):
+        run_k = ((st["r_state"] == ST_RUN) & (st["r_model"] == k))
+        wait_k = ((st["r_state"] == ST_WAIT) & (st["r_model"] == k))
+        assert np.array_equal(run_k.sum(axis=1), st["n_run"][:, k])
+        assert np.array_equal(wait_k.sum(axis=1), st["n_wait"][:, k])
+        assert np.all(st["n_run"][:, k] <= spec.slots[k])
+        kv = (run_k * (st["r_in_tok"] + st["r_out_total"] - st["r_remaining"])).sum(axis=1)
+        assert np.array_equal(kv, st["kv_used"][:, k])
+        if spec.kv_preempt:
+            assert np.all(st["kv_used"][:, k] <= spec.kv_cap[k])
+    # pending of each live query == its in-flight requests
+    for e in range(st["q_live"].shape[0]):
+        act = st["r_state"][e] != 0
+        cnt = np.bincount(st["r_query"][e][act], minlength=spec.qcap)
+        assert np.array_equal(cnt * st["q_live"][e], st["q_pending"][e] * st["q_live"][e])
+        assert np.all(cnt[st["q_live"][e] == 0] == 0)
+
+
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_p8_conservation_every_tick(orc, cfg):
+    spec = make_pool_spec(cfg, n_envs=6, n_ticks=240)
+    blob = make_policy_blob(spec)
+    o = orc.Oracle(spec, seed=0)
+    for step in range(80):
+        o.rollout(blob, 3)
+        st = decode_state(o.state(), spec.n_models, spec.qcap, spec.rcap)
+        _check_conservation(spec, st, o.counters(), o.tick)
+
+
+def test_p7_little_identity(orc):
+    spec = make_pool_spec(3, n_envs=8, n_ticks=400)     # overload: drops happen and contribute 0
+    o = orc.Oracle(spec, seed=3)
+    o.rollout(make_policy_blob(spec), 400)
+    c = o.counters()
+    st = decode_state(o.state(), spec.n_models, spec.qcap, spec.rcap)
+    still = ((400 - st["q_arrive"]) * st["q_live"]).sum(axis=1)
+    assert np.array_equal(c[:, CN["sum_live_mid"]], c[:, CN["sum_sojourn"]] + still.astype(np.uint64))
+    assert c[:, CN["dropped"]].sum() > 0
+    # query log agrees with the counters
+    q = o.queries()
+    assert q["sojourn"].sum() == c[:, CN["sum_sojourn"]].sum()
+    assert ((q["info"] >> 16) & 1).sum() == c[:, CN["solved"]].sum()
+    # trajectory arrays agree with the counters (R27, R9)
+    assert o.rew().sum() == c[:, CN["solved"]].sum()
+    assert o.miss().astype(np.int64).sum() == (c[:, CN["missed"]] + c[:, CN["dropped"]]).sum()
+
+
+# --------------------------------------------------------------------------------------- P9, P10
+@pytest.mark.parametrize("sched_mode", [0, 1])
+def test_p9_queue_order_and_admission_brute_force(orc, sched_mode):
+    spec = tiny_spec(n_envs=8, N=2, n_ticks=300, qcap=5, rcap=16, rate_tick=0.25, slots=1, sched_mode=sched_mode,
+                     budget=(30, 300), medians=(20, 60, 120), seed=4)
+    blob = make_policy_blob(spec, seed=1)
+    o = orc.Oracle(spec, seed=9)
+    checked = 0
+    prev = None
+    for t in range(300):
+        o.rollout(blob, 1)
+        st = decode_state(o.state(), 2, spec.qcap, spec.rcap)
+        tnow = t + 1                               # keys for the NEXT tick's admission
+        for e in range(8):
+            for k in range(2):
+                w = np.nonzero((st["r_state"][e] == ST_WAIT) & (st["r_model"][e] == k))[0]
+                base = st["r_deadline"][e][w] if sched_mode else st["r_issue"][e][w]
+                ref = w[np.lexsort((w, base))]     # repeated arg-min over (base, ridx)
+                got = o.queue_order(e, k, tnow)
+                assert np.array_equal(got, ref)
+                checked += len(w)
+                # prefix property of the admission that just happened at tick t: every request of model k
+                # that is RUNNING now and was issued/waiting has a smaller key than every one still WAITING
+                if prev is not None and len(w):
+                    newly = np.nonzero((st["r_state"][e] == ST_RUN) & (st["r_model"][e] == k) &
+                                       ~((prev["r_state"][e] == ST_RUN) & (prev["r_issue"][e] == st["r_issue"][e])))[0]
+                    if len(newly):
+                        kb = (st["r_deadline"][e] if sched_mode else st["r_issue"][e]).astype(np.int64)
+                        key_adm = max(kb[i] * 4096 + i for i in newly)
+                        key_wait = min(kb[i] * 4096 + i for i in w)
+                        assert key_adm < key_wait
+        prev = st
+    assert checked > 500
+
+
+def test_p9_equal_budgets_edf_equals_fcfs(orc):
+    """Equal budgets: deadline order == arrival order, so EDF and FCFS produce the same trajectory."""
+    kw = dict(n_envs=6, N=2, n_ticks=300, qcap=8, rcap=24, rate_tick=0.2, slots=1, budget=(100, 100), seed=2)
+    s0, s1 = tiny_spec(sched_mode=0, **kw), tiny_spec(sched_mode=1, **kw)
+    blob = forced_single_blob(s0)                  # one call per query => issue order == deadline order
+    a, b = orc.Oracle(s0, seed=1), orc.Oracle(s1, seed=1)
+    a.rollout(blob, 300), b.rollout(blob, 300)
+    assert np.array_equal(a.state(), b.state()) and np.array_equal(a.counters(), b.counters())
+    assert a.counters()[:, CN["sum_waiting"]].sum() > 0
+
+
+def test_p10_action_decode(orc):
+    """model = a div 3, strategy = a mod 3, a in [0, 3N)."""
+    spec = make_pool_spec(1, n_envs=4, n_ticks=1)
+    spec = spec.with_(max_ticks=200)
+    blob = make_policy_blob(spec, scale=3.0)
+    o = orc.Oracle(spec, seed=2)
+    seen = set()
+    prev = decode_state(o.state(), 5, spec.qcap, spec.rcap)
+    for t in range(200):
+        o.rollout(blob, 1)
+        st = decode_state(o.state(), 5, spec.qcap, spec.rcap)
+        d = o.decisions(1)
+        assert np.all(d["payload"] < 15)
+        for j in range(d["t"].size):
+            e, q, ag, a = int(d["env_local"][j]), int(d["q"][j]), int(d["agent"][j]), int(d["payload"][j])
+            hit = np.nonzero((st["r_state"][e] != 0) & (st["r_query"][e] == q) & (st["r_agent"][e] == ag) & (st["r_issue"][e] == t))[0]
+            if len(hit) == 0:
+                continue                            # completed within its first tick
+            assert st["r_model"][e][hit[0]] == a // 3 and st["r_depth"][e][hit[0]] == a % 3
+            seen.add(a)
+        prev = st
+    assert len(seen) >= 12
+
+
+# ------------------------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("cfg,tol", [(1, 1e-5), (3, 2e-2), (4, 2e-2)])
+def test_p12_mlp_vs_float64(orc, cfg, tol):
+    spec = make_pool_spec(cfg, n_envs=1, n_ticks=1)
+    blob = make_policy_blob(spec, seed=3)
+    o = orc.Oracle(spec, seed=0)
+    o.rollout(blob, 1)
+    w = blob_views(blob)
+    rng = np.random.default_rng(0)
+    for which, net in ((0, "plan"), (1, "exec")):
+        for _ in range(20):
+            x = rng.random(spec.f_in).astype(np.float32)
+            got = o.mlp_forward(which, x).astype(np.float64)
+            h = np.tanh(w[f"{net}_W1"].astype(np.float64) @ x.astype(np.float64) + w[f"{net}_b1"])
+            h = np.tanh(w[f"{net}_W2"].astype(np.float64) @ h + w[f"{net}_b2"])
+            ref = w[f"{net}_W3"].astype(np.float64) @ h + w[f"{net}_b3"]
+            assert np.max(np.abs(got - ref)) < tol
+    # zero weights => logits = bias, V = b_val
+    zb = forced_single_blob(spec, exec_bias=np.arange(3 * spec.n_models) * 0.1)
+    o.reset(); o.rollout(zb, 1)
+    out = o.mlp_forward(1, rng.random(spec.f_in).astype(np.float32))
+    assert np.allclose(out[:-1], np.arange(3 * spec.n_models, dtype=np.float32) * np.float32(0.1)) and out[-1] == 0.0
+    assert o.mlp_forward(0, np.zeros(spec.f_in, np.float32))[0] == 40.0
+
+
+# -------------------------------------------------------------------------------------- P13, P14
+def test_p13_gae_closed_forms(orc):
+    rng = np.random.default_rng(0)
+    T, n = 12, 5
+    rew = rng.random((T, n)).astype(np.float32)
+    cost = rng.random((T, n)).astype(np.float32)
+    val = rng.normal(size=(T + 1, n)).astype(np.float32)
+    done = np.zeros((T, n), np.uint8)
+    g, mu = 0.9, 0.5
+    rt = rew.astype(np.float64) - mu * cost.astype(np.float64)
+    V = val.astype(np.float64)
+    # lambda = 1: A[t] = sum_l g^l r~[t+l] + g^(T-t) V[T] - V[t]   (direct discounted sum)
+    adv, ret = orc.gae(rew, cost, val, done, g, 1.0, mu)
+    for t in range(T):
+        direct = sum(g ** l * rt[t + l] for l in range(T - t)) + g ** (T - t) * V[T] - V[t]
+        assert np.allclose(adv[t], direct, rtol=0, atol=1e-12)
+        assert np.allclose(ret[t], direct + V[t], rtol=0, atol=1e-12)
+    # lambda = 0: A = delta
+    adv, _ = orc.gae(rew, cost, val, done, g, 0.0, mu)
+    assert np.allclose(adv, rt + g * V[1:] - V[:-1], atol=1e-12)
+    # gamma = 0: A = r~ - V
+    adv, _ = orc.gae(rew, cost, val, done, 0.0, 0.95, mu)
+    assert np.allclose(adv, rt - V[:-1], atol=1e-12)
+    # general lambda: direct double sum of discounted deltas
+    lam = 0.8
+    adv, _ = orc.gae(rew, cost, val, done, g, lam, mu)
+    delta = rt + g * V[1:] - V[:-1]
+    for t in range(T):
+        direct = sum((g * lam) ** l * delta[t + l] for l in range(T - t))
+        assert np.allclose(adv[t], direct, atol=1e-12)
+    # done cuts the chain: two episodes of 6 equal two independent computations without bootstrap across
+    done2 = done.copy(); done2[5] = 1
+    adv2, _ = orc.gae(rew, cost, val, done2, g, lam, mu)
+    v_first = np.concatenate([val[:6], np.zeros((1, n), np.float32)])
+    a_first, _ = orc.gae(rew[:6], cost[:6], v_first, done[:6], g, lam, mu)
+    a_second, _ = orc.gae(rew[6:], cost[6:], val[6:], done[6:], g, lam, mu)
+    assert np.allclose(adv2[:6], a_first, atol=1e-12) and np.allclose(adv2[6:], a_second, atol=1e-12)
+    # r~ = 1, V = 0: geometric closed form
+    one = np.ones((T, n), np.float32)
+    adv, _ = orc.gae(one, 0 * one, np.zeros((T + 1, n), np.float32), done, g, lam, 0.0)
+    gl = g * lam
+    for t in range(T):
+        assert np.allclose(adv[t], (1 - gl ** (T - t)) / (1 - gl), atol=1e-12)
+
+
+def test_p14_lagrangian_linearity(orc):
+    rng = np.random.default_rng(1)
+    T, n = 30, 4
+    rew = rng.integers(0, 3, (T, n)).astype(np.float32)
+    cost = rng.random((T, n)).astype(np.float32)
+    val = rng.normal(size=(T + 1, n)).astype(np.float32)
+    done = (rng.random((T, n)) < 0.1).astype(np.uint8)
+    a0, _ = orc.gae(rew, cost, val, done, 0.99, 0.95, 0.0)
+    a1, _ = orc.gae(rew, cost, val, done, 0.99, 0.95, 0.7)
+    # A_cost: GAE of the cost stream alone (reward = cost, V = 0, mu = 0)
+    ac, _ = orc.gae(cost, 0 * cost, np.zeros_like(val), done, 0.99, 0.95, 0.0)
+    assert np.allclose(a1, a0 - 0.7 * ac, atol=1e-9)
+
+
+# ------------------------------------------------------------------------------------------- P15
+def test_p15_determinism_split_and_e_invariance(orc):
+    spec = make_pool_spec(3, n_envs=12, n_ticks=120)
+    blob = make_policy_blob(spec)
+    a = orc.Oracle(spec, seed=4)
+    a.rollout(blob, 120)
+    sa, ca, ra = a.state(), a.counters(), a.rew()
+    a.reset(); a.rollout(blob, 120)
+    assert np.array_equal(sa, a.state()) and np.array_equal(ca, a.counters()) and np.array_equal(ra, a.rew())
+    b = orc.Oracle(spec, seed=4)
+    b.rollout(blob, 50); r1 = b.rew(); v1 = b.val()
+    b.rollout(blob, 70); r2 = b.rew()
+    assert np.array_equal(sa, b.state()) and np.array_equal(ca, b.counters())
+    assert np.array_equal(np.concatenate([r1, r2]), ra)
+    assert np.array_equal(v1[50], a.val()[50])     # bootstrap row == critic row of the next tick
+    # env e of a 12-env run == env e of a run over a subset of ids
+    ids = np.array([3, 7, 11], dtype=np.uint32)
+    c = orc.Oracle(spec, seed=4, env_ids=ids)
+    c.rollout(blob, 120)
+    assert np.array_equal(c.state(), sa[ids]) and np.array_equal(c.rew(), ra[:, ids])
+    d = orc.Oracle(spec, seed=5)
+    d.rollout(blob, 120)
+    assert not np.array_equal(d.counters(), ca)
+
+
+# ------------------------------------------------------------------------------------------- P17
+def test_p17_utility_and_cbar(orc):
+    spec = make_pool_spec(1, n_envs=32, n_ticks=200)
+    o = orc.Oracle(spec, seed=0)
+    o.rollout(make_policy_blob(spec), 200)
+    mu = 0.5
+    o.returns(0.99, 0.95, mu)
+    q = o.queries()
+    U = ((q["info"] >> 16) & 1).astype(np.float64) - mu * q["sojourn"].astype(np.float64) / (q["info"] & 0xFFFF)
+    s = o.scalars()
+    assert s["n_final"] == U.size and abs(s["ubar"] - U.mean()) < 1e-12 and abs(s["usigma"] - U.std()) < 1e-12
+    assert abs(s["cbar"] - o.cost().astype(np.float64).sum() / U.size) < 1e-12
+    z = (U - s["ubar"]) / (s["usigma"] + 1e-8)
+    assert abs(z.mean()) < 1e-9 and abs(z.std() - 1) < 1e-6
+    # for a single sequential call, sum C_k > 1  <=>  SLO miss (up to Q16 truncation)
+    spec1 = tiny_spec(n_envs=8, N=1, n_ticks=400, qcap=32, rcap=96, rate_tick=0.12, slots=1, budget=(5, 60), medians=(30, 60, 90))
+    o1 = orc.Oracle(spec1, seed=3)
+    o1.rollout(forced_single_blob(spec1), 400)
+    q1 = o1.queries()
+    late = q1["sojourn"] > (q1["info"] & 0xFFFF)
+    assert late.sum() > 0 and (~late).sum() > 0
+    assert o1.miss().sum() == late.sum() + o1.counters()[:, CN["dropped"]].sum()   # R9: a drop is a miss
+
+
+# ------------------------------------------------------------------------------------------- P18
+def test_p18_deterministic_stamps_chain(orc):
+    """frac = 0, no contention, chain of K: sojourn = sum_j ceil(out_total_j / tokens_per_tick) exactly (R1, R11, R17)."""
+    for K in (1, 3, 4):
+        spec = tiny_spec(n_envs=16, N=1, n_ticks=600, qcap=64, rcap=192, rate_tick=0.01, slots=64, rates=[100],
+                         budget=(1000, 1000), medians=(30, 70, 150))
+        blob = planner_bias_blob(spec, topo=1, count=K)
+        o = orc.Oracle(spec, seed=K)
+        o.rollout(blob, 600)
+        q, d = o.queries(), o.decisions(1)
+        mult = spec.out_tok_mult_q16
+        assert q["sojourn"].size > 20
+        # recompute out_total of every call from the Philox draw, independently in Python
+        calls = {}
+        for j in range(d["t"].size):
+            env, t, qi, ag, a = int(d["env"][j]), int(d["t"][j]), int(d["q"][j]), int(d["agent"][j]), int(d["payload"][j])
+            x = orc.philox(env, t, qi * 4 + ag, 0, K, 4)   # key = (seed_lo = K, seed_hi ^ STREAM_EXEC = 4), R2
+            out_total = max(1, (int(spec.depth_median_tok[a % 3]) * int(mult[x[1] >> 22])) >> 16)
+            calls.setdefault((env, qi), []).append((t, ag, out_total))
+        done = 0
+        for i in range(q["sojourn"].size):
+            env, arrive = int(q["env"][i]), int(q["arrive"][i])
+            # match the chain whose first call was issued at `arrive`
+            for (e2, qi), lst in calls.items():
+                lst.sort()
+                if e2 == env and lst[0][0] == arrive and len(lst) >= K:
+                    first = [c for c in lst if c[0] >= arrive][:K]
+                    if first[0][0] != arrive:
+                        continue
+                    expect = sum(math.ceil(c[2] / 5.0) for c in first)     # 100 tok/s = 5 tok/tick
+                    if first[-1][0] + math.ceil(first[-1][2] / 5.0) == arrive + expect:
+                        assert int(q["sojourn"][i]) == expect
+                        done += 1
+                        break
+        assert done > 10
+
+
+def test_p18_prefill_reduces_first_tick_tokens(orc):
+    """With prefill p us: first-tick tokens = floor(rate*(50000-p)/1e6) when frac == 0 (R11)."""
+    spec = tiny_spec(n_envs=4, N=1, n_ticks=40, qcap=16, rcap=48, rate_tick=0.3, slots=16, rates=[200],
+                     budget=(500, 500), medians=(400, 400, 400), in_tok=1000, prefill=10000)
+    o = orc.Oracle(spec, seed=1)
+    blob = forced_single_blob(spec)
+    seen = 0
+    for t in range(40):
+        o.rollout(blob, 1)
+        st = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+        new = (st["r_state"] == ST_RUN) & (st["r_issue"] == t)
+        if new.any():
+            # prefill = 10000 us/ktok * 1000 tok / 1000 = 10000 us => usable 40000 us * 200 tok/s = 8 tokens
+            assert np.all((st["r_out_total"] - st["r_remaining"])[new] == 8)
+            assert np.all(st["r_prefill_us"][new] == 0)
+            seen += int(new.sum())
+    assert seen > 5
+
+
+# ------------------------------------------------------------------------------------------- P19
+def test_p19_preemption_victim_and_token_conservation(orc):
+    spec = tiny_spec(n_envs=8, N=1, n_ticks=400, qcap=32, rcap=96, rate_tick=0.4, slots=8, rates=[160],
+                     kv_preempt=1, kv_cap=700, budget=(50, 400), medians=(100, 200, 300), seed=3)
+    blob = make_policy_blob(spec, seed=2)
+    o = orc.Oracle(spec, seed=6)
+    prev, n_pre = None, 0
+    prev_c = np.zeros(8, np.uint64)
+    for t in range(400):
+        o.rollout(blob, 1)
+        st = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+        c = o.counters()[:, CN["preemptions"]]
+        assert np.all(st["kv_used"][:, 0] <= 700)
+        if prev is not None:
+            for e in range(8):
+                k = int(c[e] - prev_c[e])
+                if k == 0:
+                    continue
+                n_pre += k
+                # requests RUNNING before this tick (or admitted during it) that are WAITING now with progress kept
+                evicted = np.nonzero((st["r_state"][e] == ST_WAIT) & (st["r_out_total"][e] > st["r_remaining"][e]) &
+                                     ~((prev["r_state"][e] == ST_WAIT) & (prev["r_remaining"][e] == st["r_remaining"][e])
+                                       & (prev["r_issue"][e] == st["r_issue"][e])))[0]
+                running = np.nonzero(st["r_state"][e] == ST_RUN)[0]
+                if len(evicted) and len(running):
+                    # every victim has a larger (deadline, ridx) than every survivor
+                    vmin = min((int(st["r_deadline"][e][i]), int(i)) for i in evicted)
+                    smax = max((int(st["r_deadline"][e][i]), int(i)) for i in running)
+                    assert vmin > smax
+        prev, prev_c = st, c.copy()
+    assert n_pre > 10
+    cc = o.counters()
+    assert np.array_equal(cc[:, CN["calls_issued"]], cc[:, CN["calls_done"]] + (st["n_wait"] + st["n_run"])[:, 0])
+
+
+# ------------------------------------------------------------------------------------------- P20
+def test_p20_service_rate_stochastic_rounding(orc):
+    """Long-run tokens/tick of a running request = rate*DT (R11): 130 tok/s = 6.5 tok/tick."""
+    spec = tiny_spec(n_envs=32, N=1, n_ticks=260, qcap=8, rcap=24, rate_tick=0.02, slots=8, rates=[130],
+                     budget=(5000, 5000), medians=(60000, 60000, 60000))
+    spec = spec.with_(out_tok_mult_q16=np.full(1024, 65536, dtype=np.uint32), budget_norm_ticks=5000)
+    o = orc.Oracle(spec, seed=8)
+    blob = forced_single_blob(spec)
+    o.rollout(blob, 10)
+    tot, n = 0, 0
+    prev = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+    for _ in range(50):
+        o.rollout(blob, 5)
+        st = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+        both = (prev["r_state"] == ST_RUN) & (st["r_state"] == ST_RUN) & (prev["r_issue"] == st["r_issue"])
+        tot += int((prev["r_remaining"].astype(np.int64) - st["r_remaining"])[both].sum())
+        n += int(both.sum()) * 5
+        prev = st
+    assert n > 1000
+    assert abs(tot / n - 6.5) < 4 * 0.5 / math.sqrt(n)
+
+
+# ------------------------------------------------------------------------------------------- R13
+def test_r13_ewma_converges_to_constant_latency(orc):
+    """Constant call latency L: the integer recursion ewma += (L<<8 - ewma)>>3 reaches within 8 of L<<8."""
+    spec = tiny_spec(n_envs=4, N=1, n_ticks=1500, qcap=16, rcap=48, rate_tick=0.2, slots=16, rates=[100],
+                     budget=(500, 500), medians=(50, 50, 50))
+    spec = spec.with_(out_tok_mult_q16=np.full(1024, 65536, dtype=np.uint32))
+    o = orc.Oracle(spec, seed=2)
+    o.rollout(forced_single_blob(spec), 1500)
+    ew = o.snapshot()[:, 0, 3].astype(np.int64)
+    assert np.all(np.abs(ew - (10 << 8)) <= 8)       # 50 tokens at 5 tok/tick = 10 ticks
+    # closed form of the recursion itself, in Python
+    x = 0
+    for _ in range(200):
+        x += ((10 << 8) - x) >> 3
+    assert abs(x - (10 << 8)) <= 8
