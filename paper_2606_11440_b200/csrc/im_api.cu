@@ -1,0 +1,612 @@
+// im_api.cu — host side of the C ABI declared in include/inframind.h: spec validation, arena carving,
+// per-tick launch sequence, telemetry read-back.  No CPU fallback: every compute call needs an sm_100 device.
+#include "../../include/inframind.h"
+#include "im_device.cuh"
+#include <cuda_bf16.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace im {
+void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st);
+int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm, bool bf16, cudaStream_t st);
+int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st);
+int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st);
+size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP);
+__host__ __device__ size_t sim_warp_smem_bytes(uint32_t RCAP, uint32_t QCAP);
+
+// repack the R26 blob (device copy) into the kernels' layouts
+__global__ void k_repack(const uint8_t *blob, uint32_t dtype, uint32_t F, uint32_t H, uint32_t n_out, uint32_t n_out_pad,
+                         size_t off_W1, size_t off_b1, size_t off_W2, size_t off_b2, size_t off_W3, size_t off_b3,
+                         float *W1t, float *W2t, float *W3t, __nv_bfloat16 *W1, __nv_bfloat16 *W2, __nv_bfloat16 *W3,
+                         float *b1, float *b2, float *b3)
+{
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    if (dtype == 0) {
+        const float *s1 = (const float *)(blob + off_W1), *s2 = (const float *)(blob + off_W2), *s3 = (const float *)(blob + off_W3);
+        for (uint32_t i = tid; i < F * H; i += nth) { const uint32_t o = i / F, k = i % F; W1t[k * H + o] = s1[i]; }
+        for (uint32_t i = tid; i < H * H; i += nth) { const uint32_t o = i / H, k = i % H; W2t[k * H + o] = s2[i]; }
+        for (uint32_t i = tid; i < H * n_out_pad; i += nth) { const uint32_t k = i / n_out_pad, o = i % n_out_pad; W3t[i] = o < n_out ? s3[o * H + k] : 0.0f; }
+    } else {
+        const __nv_bfloat16 *s1 = (const __nv_bfloat16 *)(blob + off_W1), *s2 = (const __nv_bfloat16 *)(blob + off_W2), *s3 = (const __nv_bfloat16 *)(blob + off_W3);
+        for (uint32_t i = tid; i < F * H; i += nth) W1[i] = s1[i];
+        for (uint32_t i = tid; i < H * H; i += nth) W2[i] = s2[i];
+        for (uint32_t i = tid; i < H * n_out_pad; i += nth) W3[i] = (i / H) < n_out ? s3[i] : __float2bfloat16(0.0f);
+    }
+    const float *c1 = (const float *)(blob + off_b1), *c2 = (const float *)(blob + off_b2), *c3 = (const float *)(blob + off_b3);
+    for (uint32_t i = tid; i < H; i += nth) { b1[i] = c1[i]; b2[i] = c2[i]; }
+    for (uint32_t i = tid; i < n_out_pad; i += nth) b3[i] = i < n_out ? c3[i] : 0.0f;
+}
+}  // namespace im
+
+using namespace im;
+
+static thread_local std::string g_last_error;
+
+struct im_ctx {
+    im_pool_spec spec;
+    uint32_t E;
+    uint64_t seed;
+    std::vector<uint32_t> tab_mult, tab_intok, tab_cdf;
+    std::vector<uint8_t> env_level;
+    bool bound = false;
+    uint8_t *arena = nullptr;
+    size_t arena_bytes = 0;
+    cudaStream_t stream = nullptr;
+    Params P;
+    Weights Wp, We;
+    uint8_t *d_blob = nullptr;
+    size_t blob_bytes = 0;
+    float *adv = nullptr, *ret = nullptr;
+    double *sums = nullptr;
+    uint32_t *qorder = nullptr;
+    int32_t tick = 0, last_t0 = 0;
+    uint32_t last_T = 0;
+    bool have_returns = false;
+    uint32_t par_exec = 0, par_plan = 0;
+    int n_sm = 148;
+    uint64_t launches = 0;
+    std::string err;
+    // state region (for reset)
+    size_t state_off = 0, state_bytes = 0;
+};
+
+static int fail(im_ctx *c, int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf;
+    g_last_error = buf;
+    return code;
+}
+
+static size_t blob_size(const im_pool_spec &s)
+{
+    auto pad16 = [](size_t n) { return (n + 15) & ~(size_t)15; };
+    const size_t F = s.f_in, H = s.hidden, ws = s.policy_dtype ? 2 : 4;
+    size_t b = 32;
+    for (int net = 0; net < 2; net++) {
+        const size_t no = net ? 3 * s.n_models + 1 : 24;
+        b += pad16(H * F * ws) + pad16(H * 4) + pad16(H * H * ws) + pad16(H * 4) + pad16(no * H * ws) + pad16(no * 4);
+    }
+    return b;
+}
+
+static int validate(const im_pool_spec *s, uint32_t E)
+{
+    if (!s || E == 0) return fail(nullptr, IM_ERR_INVALID_ARG, "null spec or zero envs");
+    if (s->abi_version != IM_ABI_VERSION) return fail(nullptr, IM_ERR_BAD_SPEC, "abi_version %u != %u", s->abi_version, IM_ABI_VERSION);
+    if (s->n_models == 0 || s->n_models > IM_MAX_MODELS) return fail(nullptr, IM_ERR_BAD_SPEC, "n_models %u out of 1..16", s->n_models);
+    if (s->qcap == 0 || s->qcap % 32 || s->qcap > 1024) return fail(nullptr, IM_ERR_BAD_SPEC, "qcap must be a multiple of 32 <= 1024");
+    if (s->rcap % 128 || s->rcap < 3 * s->qcap || s->rcap > 4096) return fail(nullptr, IM_ERR_BAD_SPEC, "rcap must be a multiple of 128, >= 3*qcap, <= 4096");
+    if (s->max_ticks == 0 || s->max_ticks > 8191) return fail(nullptr, IM_ERR_BAD_SPEC, "max_ticks out of 1..8191");
+    if (s->sched_mode > 1 || s->kv_preempt > 1 || s->cost_mode > 1 || s->policy_dtype > 1) return fail(nullptr, IM_ERR_BAD_SPEC, "mode flag out of range");
+    if (s->n_levels == 0 || s->n_levels > 256 || s->budget_norm_ticks == 0) return fail(nullptr, IM_ERR_BAD_SPEC, "n_levels / budget_norm_ticks");
+    if (s->f_in < 3 * s->n_models + 12) return fail(nullptr, IM_ERR_BAD_SPEC, "f_in %u < 3N+12", s->f_in);
+    if (s->policy_dtype == IM_DTYPE_BF16) {
+        if (!((s->f_in == 64 && s->hidden == 128) || (s->f_in == 128 && s->hidden == 256)))
+            return fail(nullptr, IM_ERR_BAD_SPEC, "bf16 policy supports (f_in,hidden) = (64,128) or (128,256)");
+    } else {
+        if (s->f_in > 128 || s->hidden > 256 || s->hidden < 8) return fail(nullptr, IM_ERR_BAD_SPEC, "fp32 policy: f_in <= 128, 8 <= hidden <= 256");
+        if (f32_smem_bytes(s->f_in, s->hidden, 56) > 200 * 1024) return fail(nullptr, IM_ERR_BAD_SPEC, "fp32 policy too large for shared memory");
+    }
+    if (!s->out_tok_mult_q16 || !s->arr_cdf || !s->env_level) return fail(nullptr, IM_ERR_INVALID_ARG, "null table pointer");
+    for (uint32_t k = 0; k < s->n_models; k++) {
+        const im_model_spec &m = s->model[k];
+        if (m.slots == 0 || m.kv_cap == 0 || m.rate_tok_s == 0 || m.rate_tok_s > 80000) return fail(nullptr, IM_ERR_BAD_SPEC, "model %u: zero slots/kv/rate or rate too large", k);
+    }
+    for (int i = 0; i < 2; i++)
+        if (s->mix_lo[i] == 0 || s->mix_hi[i] < s->mix_lo[i] || s->mix_hi[i] > 65535) return fail(nullptr, IM_ERR_BAD_SPEC, "budget component %d out of range", i);
+    for (uint32_t l = 0; l < s->n_levels; l++)
+        for (int j = 1; j < 31; j++)
+            if (s->arr_cdf[l * 32 + j] < s->arr_cdf[l * 32 + j - 1]) return fail(nullptr, IM_ERR_BAD_SPEC, "arr_cdf row %u not monotone", l);
+    for (uint32_t e = 0; e < E; e++)
+        if (s->env_level[e] >= s->n_levels) return fail(nullptr, IM_ERR_BAD_SPEC, "env_level[%u] out of range", e);
+    for (int i = 0; i < 1024; i++) {
+        const uint64_t v = ((uint64_t)s->depth_median_tok[2] * s->out_tok_mult_q16[i]) >> 16;
+        if (v > 65535) return fail(nullptr, IM_ERR_BAD_SPEC, "output tokens exceed 65535");
+        if (s->in_tok_table && s->in_tok_table[i] > 65535) return fail(nullptr, IM_ERR_BAD_SPEC, "input tokens exceed 65535");
+    }
+    if (s->sched_mode > 1) return fail(nullptr, IM_ERR_BAD_SPEC, "sched_mode");
+    return IM_OK;
+}
+
+// ---- arena carving: the same walk sizes the arena (base == nullptr) and binds the pointers
+struct Carver {
+    uint8_t *base;
+    size_t off = 0;
+    template <typename T> T *take(size_t n)
+    {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+static void default_caps(const im_pool_spec &s, uint32_t E, uint64_t &ce, uint64_t &cp, uint64_t &cq)
+{
+    const bool log = s.debug_flags & IM_FLAG_LOG_DECISIONS;
+    const uint64_t per_tick_e = (uint64_t)E * 16 + 4096, per_tick_p = (uint64_t)E * 8 + 4096;
+    ce = s.log_cap_exec ? s.log_cap_exec : (log ? per_tick_e * s.max_ticks / 4 : per_tick_e);
+    cp = s.log_cap_plan ? s.log_cap_plan : (log ? per_tick_p * s.max_ticks / 4 : per_tick_p);
+    cq = s.log_cap_query ? s.log_cap_query : per_tick_p * s.max_ticks / 4;
+    if (!log) { ce = ce < per_tick_e ? ce : per_tick_e; cp = cp < per_tick_p ? cp : per_tick_p; }
+}
+
+static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
+{
+    Carver cv{base};
+    Params P;
+    memset(&P, 0, sizeof P);
+    const uint32_t N = s.n_models, Q = s.qcap, R = s.rcap;
+    const size_t T1 = (size_t)s.max_ticks + 1;
+    // ---- state (zeroed / re-initialised by im_reset)
+    cv.off = (cv.off + 255) & ~(size_t)255;
+    const size_t state_off = cv.off;
+    P.r_meta = cv.take<uint32_t>((size_t)E * R); P.r_rs = cv.take<uint32_t>((size_t)E * R); P.r_tok = cv.take<uint32_t>((size_t)E * R);
+    P.r_dl = cv.take<int32_t>((size_t)E * R); P.r_issue = cv.take<int32_t>((size_t)E * R);
+    P.q_plan = cv.take<uint32_t>((size_t)E * Q); P.q_bi = cv.take<uint32_t>((size_t)E * Q); P.q_row = cv.take<uint32_t>((size_t)E * Q);
+    P.q_dl = cv.take<int32_t>((size_t)E * Q); P.q_arr = cv.take<int32_t>((size_t)E * Q);
+    P.q_ready = cv.take<uint32_t>((size_t)E * (Q / 32));
+    P.m_cnt = cv.take<uint4>((size_t)E * N);
+    P.e_hdr = cv.take<uint32_t>(E);
+    P.counters = cv.take<unsigned long long>((size_t)E * 16);
+    P.snap = cv.take<float>((size_t)E * 3 * N);
+    P.err_flag = cv.take<uint32_t>(64);
+    P.exec.cnt = cv.take<uint32_t>(kRegions); P.exec.base = cv.take<uint32_t>(2 * kRegions);
+    P.plan.cnt = cv.take<uint32_t>(kRegions); P.plan.base = cv.take<uint32_t>(2 * kRegions);
+    P.qlog.cnt = cv.take<uint32_t>(kRegions);
+    double *sums = cv.take<double>(8);
+    const size_t state_end = cv.off;
+    P.r_free = cv.take<uint32_t>((size_t)E * (R / 32)); P.q_free = cv.take<uint32_t>((size_t)E * (Q / 32));   // reset to all-ones
+    // ---- tables
+    P.tab_mult = cv.take<uint32_t>(1024); P.tab_intok = cv.take<uint32_t>(1024);
+    P.tab_cdf = cv.take<uint32_t>((size_t)s.n_levels * 32); P.env_level = cv.take<uint8_t>(E);
+    // ---- trajectory
+    P.rew = cv.take<float>(T1 * E); P.cost = cv.take<float>(T1 * E); P.val = cv.take<float>(T1 * E);
+    P.done = cv.take<uint8_t>(T1 * E); P.miss = cv.take<uint8_t>(T1 * E);
+    float *adv = cv.take<float>(T1 * E), *ret = cv.take<float>(T1 * E);
+    // ---- row lists / logs
+    uint64_t ce, cp, cq;
+    default_caps(s, E, ce, cp, cq);
+    const uint32_t rce = (uint32_t)((ce + kRegions - 1) / kRegions), rcp = (uint32_t)((cp + kRegions - 1) / kRegions), rcq = (uint32_t)((cq + kRegions - 1) / kRegions);
+    P.exec.regcap = rce; P.plan.regcap = rcp; P.qlog.regcap = rcq;
+    const size_t ne = (size_t)rce * kRegions, np = (size_t)rcp * kRegions, nq = (size_t)rcq * kRegions;
+    P.exec.env = cv.take<uint32_t>(ne); P.exec.a = cv.take<uint32_t>(ne); P.exec.b = cv.take<float>(ne); P.exec.c = cv.take<uint32_t>(ne);
+    P.exec.logp = cv.take<float>(ne); P.exec.val = cv.take<float>(ne);
+    P.plan.env = cv.take<uint32_t>(np); P.plan.a = cv.take<uint32_t>(np); P.plan.b = cv.take<float>(np); P.plan.c = cv.take<uint32_t>(np);
+    P.plan.logp = cv.take<float>(np); P.plan.val = nullptr;
+    P.exec.n_out = 3 * N + 1; P.plan.n_out = 24;
+    if (s.debug_flags & IM_FLAG_LOG_LOGITS) { P.exec.logits = cv.take<float>(ne * (3 * N + 1)); P.plan.logits = cv.take<float>(np * 24); }
+    P.qlog.env = cv.take<uint32_t>(nq); P.qlog.arrive = cv.take<uint32_t>(nq); P.qlog.sojourn = cv.take<uint32_t>(nq); P.qlog.info = cv.take<uint32_t>(nq);
+    P.qlog.unorm = cv.take<float>(nq);
+    // ---- weights
+    const uint32_t F = s.f_in, H = s.hidden;
+    Weights W[2];
+    for (int net = 0; net < 2; net++) {
+        Weights &w = W[net];
+        memset(&w, 0, sizeof w);
+        w.n_out = net ? 3 * N + 1 : 24; w.n_out_pad = (w.n_out + 7) & ~7u;
+        if (s.policy_dtype == IM_DTYPE_F32) {
+            w.W1t = cv.take<float>((size_t)F * H); w.W2t = cv.take<float>((size_t)H * H); w.W3t = cv.take<float>((size_t)H * w.n_out_pad);
+        } else {
+            w.W1 = cv.take<__nv_bfloat16>((size_t)F * H); w.W2 = cv.take<__nv_bfloat16>((size_t)H * H); w.W3 = cv.take<__nv_bfloat16>((size_t)H * w.n_out_pad);
+        }
+        w.b1 = cv.take<float>(H); w.b2 = cv.take<float>(H); w.b3 = cv.take<float>(w.n_out_pad);
+    }
+    uint8_t *d_blob = cv.take<uint8_t>(blob_size(s));
+    uint32_t *qorder = cv.take<uint32_t>((size_t)E * (N + 1 + R));
+    const size_t total = (cv.off + 255) & ~(size_t)255;
+    if (c && base) {
+        P.E = E; P.N = N; P.QCAP = Q; P.RCAP = R; P.QW = Q / 32; P.RW = R / 32;
+        P.sched_mode = s.sched_mode; P.kv_preempt = s.kv_preempt; P.cost_mode = s.cost_mode; P.episode_ticks = s.episode_ticks;
+        P.budget_norm = s.budget_norm_ticks; P.in_tok_const = s.in_tok_const; P.mix_thresh = s.mix_thresh; P.env_id_base = s.env_id_base;
+        for (int i = 0; i < 2; i++) { P.mix_lo[i] = s.mix_lo[i]; P.mix_hi[i] = s.mix_hi[i]; }
+        for (int i = 0; i < 3; i++) P.depth_median[i] = s.depth_median_tok[i];
+        P.flags = s.debug_flags; P.has_intok = c->tab_intok.empty() ? 0 : 1;
+        P.seed_lo = (uint32_t)c->seed; P.seed_hi = (uint32_t)(c->seed >> 32);
+        P.f_in = F; P.hidden = H; P.log_mode = (s.debug_flags & IM_FLAG_LOG_DECISIONS) ? 1 : 0;
+        for (uint32_t k = 0; k < N; k++) {
+            const im_model_spec &m = s.model[k];
+            P.model[k] = ModelTab{m.rate_tok_s, m.slots, m.kv_cap, m.prefill_us_per_ktok, {m.succ_thresh[0], m.succ_thresh[1], m.succ_thresh[2]}, m.kv_inv};
+        }
+        c->P = P; c->Wp = W[0]; c->We = W[1]; c->d_blob = d_blob; c->blob_bytes = blob_size(s);
+        c->adv = adv; c->ret = ret; c->sums = sums; c->qorder = qorder;
+        c->state_off = state_off; c->state_bytes = state_end - state_off;
+    }
+    return total;
+}
+
+#define CUDA_TRY(c, expr)                                                                                  \
+    do {                                                                                                   \
+        cudaError_t _e = (expr);                                                                           \
+        if (_e != cudaSuccess) return fail(c, IM_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(_e));        \
+    } while (0)
+
+static int copy_out(im_ctx *c, const void *src, size_t bytes, void *dst, size_t cap, size_t *written)
+{
+    if (written) *written = bytes;
+    if (!dst) return IM_OK;
+    if (cap < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", cap, bytes);
+    CUDA_TRY(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return IM_OK;
+}
+
+template <typename T>
+static int fetch(im_ctx *c, std::vector<T> &h, const T *d, size_t n)
+{
+    h.resize(n);
+    if (n) CUDA_TRY(c, cudaMemcpyAsync(h.data(), d, n * sizeof(T), cudaMemcpyDeviceToHost, c->stream));
+    return IM_OK;
+}
+
+extern "C" {
+
+size_t im_arena_bytes(const im_pool_spec *spec, uint32_t n_envs)
+{
+    if (validate(spec, n_envs) != IM_OK) return 0;
+    return carve(nullptr, *spec, n_envs, nullptr);
+}
+
+int im_create(const im_pool_spec *spec, uint32_t n_envs, uint64_t seed, im_ctx **out)
+{
+    if (!out) return fail(nullptr, IM_ERR_INVALID_ARG, "out is null");
+    *out = nullptr;
+    const int rc = validate(spec, n_envs);
+    if (rc != IM_OK) return rc;
+    im_ctx *c = new (std::nothrow) im_ctx();
+    if (!c) return fail(nullptr, IM_ERR_NOMEM, "host allocation failed");
+    c->spec = *spec;
+    c->E = n_envs; c->seed = seed;
+    c->tab_mult.assign(spec->out_tok_mult_q16, spec->out_tok_mult_q16 + 1024);
+    if (spec->in_tok_table) c->tab_intok.assign(spec->in_tok_table, spec->in_tok_table + 1024);
+    c->tab_cdf.assign(spec->arr_cdf, spec->arr_cdf + (size_t)spec->n_levels * 32);
+    c->env_level.assign(spec->env_level, spec->env_level + n_envs);
+    c->spec.out_tok_mult_q16 = nullptr; c->spec.in_tok_table = nullptr; c->spec.arr_cdf = nullptr; c->spec.env_level = nullptr;
+    *out = c;
+    return IM_OK;
+}
+
+int im_reset(im_ctx *c)
+{
+    if (!c) return fail(nullptr, IM_ERR_INVALID_ARG, "ctx is null");
+    if (!c->bound) return fail(c, IM_ERR_STATE, "im_reset before im_bind");
+    CUDA_TRY(c, cudaMemsetAsync(c->arena + c->state_off, 0, c->state_bytes, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->P.r_free, 0xFF, (size_t)c->E * c->P.RW * 4, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->P.q_free, 0xFF, (size_t)c->E * c->P.QW * 4, c->stream));
+    c->tick = 0; c->last_T = 0; c->have_returns = false; c->par_exec = 0; c->par_plan = 0;
+    return IM_OK;
+}
+
+int im_bind(im_ctx *c, void *dev_arena, size_t bytes, void *cuda_stream)
+{
+    if (!c || !dev_arena) return fail(c, IM_ERR_INVALID_ARG, "null ctx or arena");
+    if ((uintptr_t)dev_arena & 255) return fail(c, IM_ERR_INVALID_ARG, "arena must be 256-byte aligned");
+    int dev = 0, major = 0;
+    CUDA_TRY(c, cudaGetDevice(&dev));
+    CUDA_TRY(c, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return fail(c, IM_ERR_CUDA, "device compute capability %d.x is not sm_100 (no fallback path)", major);
+    CUDA_TRY(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    const size_t need = carve(nullptr, c->spec, c->E, nullptr);
+    if (bytes < need) return fail(c, IM_ERR_NOMEM, "arena too small: %zu < %zu", bytes, need);
+    c->arena = (uint8_t *)dev_arena; c->arena_bytes = bytes; c->stream = (cudaStream_t)cuda_stream;
+    carve(c, c->spec, c->E, c->arena);
+    CUDA_TRY(c, cudaMemcpyAsync((void *)c->P.tab_mult, c->tab_mult.data(), 4096, cudaMemcpyHostToDevice, c->stream));
+    if (!c->tab_intok.empty()) CUDA_TRY(c, cudaMemcpyAsync((void *)c->P.tab_intok, c->tab_intok.data(), 4096, cudaMemcpyHostToDevice, c->stream));
+    else CUDA_TRY(c, cudaMemsetAsync((void *)c->P.tab_intok, 0, 4096, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync((void *)c->P.tab_cdf, c->tab_cdf.data(), c->tab_cdf.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync((void *)c->P.env_level, c->env_level.data(), c->E, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->bound = true;
+    return im_reset(c);
+}
+
+static int upload_weights(im_ctx *c, const void *blob)
+{
+    cudaPointerAttributes at;
+    bool on_device = false;
+    if (cudaPointerGetAttributes(&at, blob) == cudaSuccess) on_device = (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
+    else cudaGetLastError();
+    if (!on_device) {
+        const uint32_t *h = (const uint32_t *)blob;
+        if (h[0] != 0x494D5042u || h[1] != c->spec.policy_dtype || h[2] != c->spec.f_in || h[3] != c->spec.hidden || h[4] != 24 ||
+            h[5] != 3 * c->spec.n_models + 1)
+            return fail(c, IM_ERR_BAD_SPEC, "policy blob header does not match the spec");
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_blob, blob, c->blob_bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    auto pad16 = [](size_t n) { return (n + 15) & ~(size_t)15; };
+    const size_t F = c->spec.f_in, H = c->spec.hidden, ws = c->spec.policy_dtype ? 2 : 4;
+    size_t off = 32;
+    for (int net = 0; net < 2; net++) {
+        Weights &w = net ? c->We : c->Wp;
+        const size_t oW1 = off; off += pad16(H * F * ws);
+        const size_t ob1 = off; off += pad16(H * 4);
+        const size_t oW2 = off; off += pad16(H * H * ws);
+        const size_t ob2 = off; off += pad16(H * 4);
+        const size_t oW3 = off; off += pad16((size_t)w.n_out * H * ws);
+        const size_t ob3 = off; off += pad16((size_t)w.n_out * 4);
+        k_repack<<<64, 256, 0, c->stream>>>(c->d_blob, c->spec.policy_dtype, (uint32_t)F, (uint32_t)H, w.n_out, w.n_out_pad, oW1, ob1, oW2, ob2, oW3, ob3,
+                                            (float *)w.W1t, (float *)w.W2t, (float *)w.W3t, (__nv_bfloat16 *)w.W1, (__nv_bfloat16 *)w.W2,
+                                            (__nv_bfloat16 *)w.W3, (float *)w.b1, (float *)w.b2, (float *)w.b3);
+        c->launches++;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    return IM_OK;
+}
+
+int im_rollout(im_ctx *c, const void *policy_weights, uint32_t n_ticks)
+{
+    if (!c || !policy_weights) return fail(c, IM_ERR_INVALID_ARG, "null ctx or weights");
+    if (!c->bound) return fail(c, IM_ERR_STATE, "im_rollout before im_bind");
+    if (n_ticks == 0 || n_ticks > c->spec.max_ticks) return fail(c, IM_ERR_CAPACITY, "n_ticks %u out of 1..max_ticks=%u", n_ticks, c->spec.max_ticks);
+    int rc = upload_weights(c, policy_weights);
+    if (rc != IM_OK) return rc;
+    cudaStream_t st = c->stream;
+    const Params &P = c->P;
+    const bool bf16 = c->spec.policy_dtype == IM_DTYPE_BF16;
+    if (P.log_mode) {   // logs restart with every rollout
+        CUDA_TRY(c, cudaMemsetAsync(P.exec.cnt, 0, sizeof(uint32_t) * kRegions, st));
+        CUDA_TRY(c, cudaMemsetAsync(P.exec.base, 0, sizeof(uint32_t) * 2 * kRegions, st));
+        CUDA_TRY(c, cudaMemsetAsync(P.plan.cnt, 0, sizeof(uint32_t) * kRegions, st));
+        CUDA_TRY(c, cudaMemsetAsync(P.plan.base, 0, sizeof(uint32_t) * 2 * kRegions, st));
+    }
+    CUDA_TRY(c, cudaMemsetAsync(P.qlog.cnt, 0, sizeof(uint32_t) * kRegions, st));
+    const int32_t t0 = c->tick;
+    launch_sim(P, -1, 0, t0, 1, t0, st);                                   // A, B of the first tick
+    c->launches++;
+    for (uint32_t i = 0; i < n_ticks; i++) {
+        const int32_t t = t0 + (int32_t)i;
+        if (launch_policy(P, c->Wp, false, c->par_plan, t0, i, c->n_sm, bf16, st)) return fail(c, IM_ERR_BAD_SPEC, "unsupported policy shape");
+        c->par_plan ^= 1;
+        launch_policy(P, c->We, true, c->par_exec, t0, i, c->n_sm, bf16, st);   // C, D: decisions of tick t + critic V[t]
+        c->par_exec ^= 1;
+        const bool last = (i + 1 == n_ticks);
+        launch_sim(P, t, i, t + 1, last ? 2u : 1u, t0, st);                 // D-issue .. I of tick t, A, B of tick t+1
+        c->launches += 3;
+    }
+    launch_policy(P, c->We, true, c->par_exec, t0, n_ticks, c->n_sm, bf16, st);  // bootstrap V[n_ticks] (R30)
+    c->par_exec ^= 1;
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    c->tick = t0 + (int32_t)n_ticks; c->last_t0 = t0; c->last_T = n_ticks; c->have_returns = false;
+    return IM_OK;
+}
+
+int im_returns(im_ctx *c, float gamma, float lambda, float lagrange_mu)
+{
+    if (!c) return fail(nullptr, IM_ERR_INVALID_ARG, "ctx is null");
+    if (!c->bound || c->last_T == 0) return fail(c, IM_ERR_STATE, "im_returns before im_rollout");
+    c->launches += launch_returns(c->P, c->last_T, gamma, lambda, lagrange_mu, c->adv, c->ret, c->sums, c->stream);
+    CUDA_TRY(c, cudaGetLastError());
+    c->have_returns = true;
+    return IM_OK;
+}
+
+int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, size_t *written)
+{
+    if (!c) return fail(nullptr, IM_ERR_INVALID_ARG, "ctx is null");
+    if (!c->bound) return fail(c, IM_ERR_STATE, "im_read_telemetry before im_bind");
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    const Params &P = c->P;
+    uint32_t flag = 0;
+    CUDA_TRY(c, cudaMemcpy(&flag, P.err_flag, 4, cudaMemcpyDeviceToHost));
+    if (flag) return fail(c, IM_ERR_CAPACITY, "log / work-list overflow during rollout (flag %u): raise log_cap_*", flag);
+    const size_t E = c->E, T = c->last_T, N = P.N, Q = P.QCAP, R = P.RCAP;
+    switch (what) {
+    case IM_TEL_REW: return copy_out(c, P.rew, 4 * T * E, dst, dst_bytes, written);
+    case IM_TEL_COST: return copy_out(c, P.cost, 4 * T * E, dst, dst_bytes, written);
+    case IM_TEL_VAL: return copy_out(c, P.val, 4 * (T + 1) * E, dst, dst_bytes, written);
+    case IM_TEL_DONE: return copy_out(c, P.done, T * E, dst, dst_bytes, written);
+    case IM_TEL_MISS: return copy_out(c, P.miss, T * E, dst, dst_bytes, written);
+    case IM_TEL_ADV:
+    case IM_TEL_RET:
+        if (!c->have_returns) return fail(c, IM_ERR_STATE, "ADV/RET read before im_returns");
+        return copy_out(c, what == IM_TEL_ADV ? c->adv : c->ret, 4 * T * E, dst, dst_bytes, written);
+    case IM_TEL_COUNTERS: return copy_out(c, P.counters, 8 * 16 * E, dst, dst_bytes, written);
+    case IM_TEL_SNAPSHOT: return copy_out(c, P.m_cnt, 16 * N * E, dst, dst_bytes, written);
+    case IM_TEL_TABLES: {
+        const size_t bytes = 4096 + 4096 + c->tab_cdf.size() * 4;
+        if (written) *written = bytes;
+        if (!dst) return IM_OK;
+        if (dst_bytes < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small");
+        CUDA_TRY(c, cudaMemcpy(dst, P.tab_mult, 4096, cudaMemcpyDeviceToHost));
+        CUDA_TRY(c, cudaMemcpy((uint8_t *)dst + 4096, P.tab_intok, 4096, cudaMemcpyDeviceToHost));
+        CUDA_TRY(c, cudaMemcpy((uint8_t *)dst + 8192, P.tab_cdf, c->tab_cdf.size() * 4, cudaMemcpyDeviceToHost));
+        return IM_OK;
+    }
+    case IM_TEL_SCALARS: {
+        if (written) *written = 64;
+        if (!dst) return IM_OK;
+        if (dst_bytes < 64) return fail(c, IM_ERR_CAPACITY, "dst too small");
+        double s[8] = {0, 0, 0, 0, 0, 0, 0, 0}, out[8];
+        if (c->have_returns) CUDA_TRY(c, cudaMemcpy(s, c->sums, 32, cudaMemcpyDeviceToHost));
+        uint32_t ce[kRegions], cp[kRegions];
+        CUDA_TRY(c, cudaMemcpy(ce, P.exec.cnt, sizeof ce, cudaMemcpyDeviceToHost));
+        CUDA_TRY(c, cudaMemcpy(cp, P.plan.cnt, sizeof cp, cudaMemcpyDeviceToHost));
+        double ne = 0, np = 0;
+        for (uint32_t r = 0; r < kRegions; r++) { ne += ce[r]; np += cp[r]; }
+        const double cnt = s[3], mean = cnt > 0 ? s[1] / cnt : 0.0;
+        double var = cnt > 0 ? s[2] / cnt - mean * mean : 0.0;
+        var = var > 0 ? var : 0.0;
+        out[0] = cnt > 0 ? s[0] / cnt : 0.0; out[1] = mean; out[2] = std::sqrt(var); out[3] = s[0]; out[4] = cnt;
+        out[5] = P.log_mode ? ne : -1.0; out[6] = P.log_mode ? np : -1.0; out[7] = (double)c->tick;
+        memcpy(dst, out, 64);
+        return IM_OK;
+    }
+    case IM_TEL_DECISIONS_EXEC:
+    case IM_TEL_DECISIONS_PLAN:
+    case IM_TEL_LOGITS_EXEC:
+    case IM_TEL_LOGITS_PLAN: {
+        if (!P.log_mode) return fail(c, IM_ERR_STATE, "decision log needs IM_FLAG_LOG_DECISIONS");
+        const bool ex = what == IM_TEL_DECISIONS_EXEC || what == IM_TEL_LOGITS_EXEC;
+        const bool lg = what == IM_TEL_LOGITS_EXEC || what == IM_TEL_LOGITS_PLAN;
+        const RowBuf &rb = ex ? P.exec : P.plan;
+        if (lg && !rb.logits) return fail(c, IM_ERR_STATE, "logits need IM_FLAG_LOG_LOGITS");
+        uint32_t cnt[kRegions];
+        CUDA_TRY(c, cudaMemcpy(cnt, rb.cnt, sizeof cnt, cudaMemcpyDeviceToHost));
+        size_t n = 0;
+        for (uint32_t r = 0; r < kRegions; r++) n += cnt[r];
+        const size_t rec = lg ? 4 * rb.n_out : 24;
+        if (written) *written = n * rec;
+        if (!dst) return IM_OK;
+        if (dst_bytes < n * rec) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, n * rec);
+        size_t k = 0;
+        for (uint32_t r = 0; r < kRegions; r++) {
+            const size_t m = cnt[r], o = (size_t)r * rb.regcap;
+            if (!m) continue;
+            if (lg) {
+                CUDA_TRY(c, cudaMemcpy((uint8_t *)dst + k * rec, rb.logits + o * rb.n_out, m * rec, cudaMemcpyDeviceToHost));
+            } else {
+                std::vector<uint32_t> env, a, cc, lp, vl;
+                int rc;
+                if ((rc = fetch(c, env, rb.env + o, m)) || (rc = fetch(c, a, rb.a + o, m)) || (rc = fetch(c, cc, rb.c + o, m)) ||
+                    (rc = fetch(c, lp, (const uint32_t *)rb.logp + o, m)))
+                    return rc;
+                if (ex && (rc = fetch(c, vl, (const uint32_t *)rb.val + o, m))) return rc;
+                CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+                uint32_t *out = (uint32_t *)dst + k * 6;
+                for (size_t i = 0; i < m; i++) {
+                    out[i * 6 + 0] = P.env_id_base + env[i];
+                    out[i * 6 + 1] = (uint32_t)(c->last_t0 + (int32_t)(a[i] >> 19));
+                    out[i * 6 + 2] = ex ? ((a[i] & 0x3FFu) | (((a[i] >> 10) & 3u) << 16)) : (a[i] & 0x3FFu);
+                    out[i * 6 + 3] = cc[i] >> 16;
+                    out[i * 6 + 4] = lp[i];
+                    out[i * 6 + 5] = ex ? vl[i] : 0u;
+                }
+            }
+            k += m;
+        }
+        return IM_OK;
+    }
+    case IM_TEL_QUERIES:
+    case IM_TEL_UNORM: {
+        if (what == IM_TEL_UNORM && !c->have_returns) return fail(c, IM_ERR_STATE, "UNORM read before im_returns");
+        uint32_t cnt[kRegions];
+        CUDA_TRY(c, cudaMemcpy(cnt, P.qlog.cnt, sizeof cnt, cudaMemcpyDeviceToHost));
+        size_t n = 0;
+        for (uint32_t r = 0; r < kRegions; r++) n += cnt[r];
+        const size_t rec = what == IM_TEL_QUERIES ? 16 : 4;
+        if (written) *written = n * rec;
+        if (!dst) return IM_OK;
+        if (dst_bytes < n * rec) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, n * rec);
+        size_t k = 0;
+        for (uint32_t r = 0; r < kRegions; r++) {
+            const size_t m = cnt[r], o = (size_t)r * P.qlog.regcap;
+            if (!m) continue;
+            if (what == IM_TEL_UNORM) {
+                CUDA_TRY(c, cudaMemcpy((float *)dst + k, P.qlog.unorm + o, 4 * m, cudaMemcpyDeviceToHost));
+            } else {
+                std::vector<uint32_t> env, ar, so, inf;
+                int rc;
+                if ((rc = fetch(c, env, P.qlog.env + o, m)) || (rc = fetch(c, ar, P.qlog.arrive + o, m)) || (rc = fetch(c, so, P.qlog.sojourn + o, m)) ||
+                    (rc = fetch(c, inf, P.qlog.info + o, m)))
+                    return rc;
+                CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+                uint32_t *out = (uint32_t *)dst + k * 4;
+                for (size_t i = 0; i < m; i++) { out[i * 4] = env[i]; out[i * 4 + 1] = ar[i]; out[i * 4 + 2] = so[i]; out[i * 4 + 3] = inf[i]; }
+            }
+            k += m;
+        }
+        return IM_OK;
+    }
+    case IM_TEL_STATE: {
+        const size_t words = 4 * N + 4 * Q + 5 * R, bytes = 4 * words * E;
+        if (written) *written = bytes;
+        if (!dst) return IM_OK;
+        if (dst_bytes < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, bytes);
+        std::vector<uint32_t> meta, rs, tok, dl, is, qp, qb, qd, qa, mc;
+        int rc;
+        if ((rc = fetch(c, meta, P.r_meta, E * R)) || (rc = fetch(c, rs, P.r_rs, E * R)) || (rc = fetch(c, tok, P.r_tok, E * R)) ||
+            (rc = fetch(c, dl, (const uint32_t *)P.r_dl, E * R)) || (rc = fetch(c, is, (const uint32_t *)P.r_issue, E * R)) ||
+            (rc = fetch(c, qp, P.q_plan, E * Q)) || (rc = fetch(c, qb, P.q_bi, E * Q)) || (rc = fetch(c, qd, (const uint32_t *)P.q_dl, E * Q)) ||
+            (rc = fetch(c, qa, (const uint32_t *)P.q_arr, E * Q)) || (rc = fetch(c, mc, (const uint32_t *)P.m_cnt, E * N * 4)))
+            return rc;
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        uint32_t *w = (uint32_t *)dst;
+        for (size_t e = 0; e < E; e++) {
+            memcpy(w, &mc[e * N * 4], 16 * N); w += 4 * N;
+            for (size_t i = 0; i < Q; i++, w += 4) {
+                const uint32_t p = qp[e * Q + i];
+                if (!(p & QP_LIVE)) { w[0] = w[1] = w[2] = w[3] = 0; continue; }
+                const uint32_t succ = ((p >> QP_SUCC_SHIFT) & 7u) ? 1u : 0u;
+                w[0] = (p & 0x1FFFFu) | (succ << 17) | (((p >> QP_ROLE_SHIFT) & 0xFFu) << 18);
+                w[1] = qd[e * Q + i]; w[2] = qa[e * Q + i]; w[3] = qb[e * Q + i];
+            }
+            for (size_t i = 0; i < R; i++, w += 5) {
+                const uint32_t m = meta[e * R + i];
+                if ((m & 3u) == ST_FREE) { w[0] = w[1] = w[2] = w[3] = w[4] = 0; continue; }
+                w[0] = m; w[1] = dl[e * R + i]; w[2] = is[e * R + i]; w[3] = rs[e * R + i]; w[4] = tok[e * R + i];
+            }
+        }
+        return IM_OK;
+    }
+    case IM_TEL_QUEUE_ORDER: {
+        c->launches += launch_queue_order(P, c->tick, c->qorder, c->stream);
+        CUDA_TRY(c, cudaGetLastError());
+        return copy_out(c, c->qorder, 4 * E * (N + 1 + R), dst, dst_bytes, written);
+    }
+    default: return fail(c, IM_ERR_INVALID_ARG, "unknown telemetry selector %u", what);
+    }
+}
+
+int im_device_ptr(im_ctx *c, uint32_t what, void **dev_ptr, size_t *bytes)
+{
+    if (!c || !dev_ptr || !bytes) return fail(c, IM_ERR_INVALID_ARG, "null argument");
+    if (!c->bound) return fail(c, IM_ERR_STATE, "not bound");
+    const size_t E = c->E, T = c->last_T;
+    switch (what) {
+    case IM_TEL_REW: *dev_ptr = c->P.rew; *bytes = 4 * T * E; break;
+    case IM_TEL_COST: *dev_ptr = c->P.cost; *bytes = 4 * T * E; break;
+    case IM_TEL_VAL: *dev_ptr = c->P.val; *bytes = 4 * (T + 1) * E; break;
+    case IM_TEL_DONE: *dev_ptr = c->P.done; *bytes = T * E; break;
+    case IM_TEL_MISS: *dev_ptr = c->P.miss; *bytes = T * E; break;
+    case IM_TEL_ADV: *dev_ptr = c->adv; *bytes = 4 * T * E; break;
+    case IM_TEL_RET: *dev_ptr = c->ret; *bytes = 4 * T * E; break;
+    default: return fail(c, IM_ERR_INVALID_ARG, "selector %u has no device array", what);
+    }
+    return IM_OK;
+}
+
+uint64_t im_launch_count(const im_ctx *c) { return c ? c->launches : 0; }
+
+void im_destroy(im_ctx *c)
+{
+    if (!c) return;
+    if (c->bound) cudaStreamSynchronize(c->stream);
+    delete c;
+}
+
+const char *im_last_error(const im_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,176 @@
+// im_device.cuh — device-side parameter block and the small defined functions (Philox, im_exp, im_tanh,
+// sampler) of the CUDA path.  Written independently of oracle/ (no shared code); the definitions follow
+// DESIGN.md readings R2, R3, R23, R24.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+namespace im {
+
+constexpr uint32_t kMaxModels = 16;
+constexpr uint32_t kRegions = 64;        // row-list / log regions (one atomic counter each), region = env % 64
+constexpr uint32_t kDtUs = 50000;
+
+// request meta word
+constexpr uint32_t ST_FREE = 0, ST_WAIT = 1, ST_RUN = 2;
+// query plan word (device layout): live0 planned1 topo2-3 cnt4-5 keff6-8 stage9-11 nst12-14 pending15-16 succ17-19 roles20-27
+constexpr uint32_t QP_LIVE = 1u, QP_PLANNED = 2u;
+constexpr uint32_t QP_PEND_SHIFT = 15, QP_SUCC_SHIFT = 17, QP_ROLE_SHIFT = 20;
+
+enum Stream : uint32_t { STREAM_ARR = 1, STREAM_QRY = 2, STREAM_PLAN = 3, STREAM_EXEC = 4, STREAM_SVC = 5 };
+enum Counter : uint32_t { C_ARRIVALS, C_DROPPED, C_FINISHED, C_SOLVED, C_MISSED, C_ISSUED, C_CALLS_DONE, C_PREEMPT,
+                          C_SUM_SOJOURN, C_SUM_LIVE_MID, C_PLANS, C_EXEC_DEC, C_SUM_RUNNING, C_SUM_WAITING, C_NEAR,
+                          C_ABANDONED, C_N };
+
+struct ModelTab {
+    uint32_t rate, slots, kv_cap, prefill;
+    uint32_t succ[3];
+    float kv_inv;
+};
+
+// a work list that doubles as the decision log: 64 regions, each a ring of `regcap` rows
+struct RowBuf {
+    uint32_t *env;       // local env index
+    uint32_t *a;         // exec: q | agent<<10 | topo<<12 | role<<14 | keff<<16 | t_rel<<19 ; plan: q | t_rel<<19
+    float *b;            // budget feature b (R15)
+    uint32_t *c;         // in_tok | result<<16 (exec: action; plan: topo|cnt<<2|roles<<4)
+    float *logp;
+    float *val;          // exec only
+    float *logits;       // optional [rows][n_out]
+    uint32_t *cnt;       // [kRegions] monotonically increasing append counters
+    uint32_t *base;      // [2][kRegions] start of the current tick's rows (parity double buffer)
+    uint32_t regcap;
+    uint32_t n_out;
+};
+
+struct QLog {
+    uint32_t *env, *arrive, *sojourn, *info;
+    float *unorm;
+    uint32_t *cnt;       // [kRegions]
+    uint32_t regcap;
+};
+
+struct Params {
+    uint32_t E, N, QCAP, RCAP, QW, RW;
+    uint32_t sched_mode, kv_preempt, cost_mode, episode_ticks, budget_norm, in_tok_const, mix_thresh, env_id_base;
+    uint32_t mix_lo[2], mix_hi[2], depth_median[3];
+    uint32_t flags, has_intok, seed_lo, seed_hi;
+    uint32_t f_in, hidden, log_mode, pad0;
+    ModelTab model[kMaxModels];
+    // env state, SoA: [E][cap], cap index fastest
+    uint32_t *r_meta, *r_rs, *r_tok;
+    int32_t *r_dl, *r_issue;
+    uint32_t *q_plan, *q_bi, *q_row;
+    int32_t *q_dl, *q_arr;
+    uint32_t *r_free, *q_free, *q_ready;     // bitmaps [E][RW] / [E][QW]
+    uint4 *m_cnt;                            // [E][N] {n_wait, n_run, kv_used, ewma_q8}
+    uint32_t *e_hdr;                         // [E] drops carried from phase A to phase I of the same tick
+    unsigned long long *counters;            // [E][16]
+    float *snap;                             // [E][3N] telemetry features of the current tick (R14)
+    const uint32_t *tab_mult, *tab_intok, *tab_cdf;
+    const uint8_t *env_level;
+    float *rew, *cost, *val;
+    uint8_t *done, *miss;
+    RowBuf exec, plan;
+    QLog qlog;
+    uint32_t *err_flag;
+};
+
+struct Weights {          // device copies of one net, prepared by k_repack (im_api.cu)
+    const float *W1t, *W2t, *W3t;        // fp32 path: transposed [k][o]; W3t has ld = n_out_pad
+    const __nv_bfloat16 *W1, *W2, *W3;   // bf16 path: [o][k] row-major, W3 zero-padded to n_out_pad rows
+    const float *b1, *b2, *b3;           // fp32 biases (b3 padded)
+    uint32_t n_out, n_out_pad;
+};
+
+// ------------------------------------------------------------------------------------------------ R2
+struct Ph4 { uint32_t x, y, z, w; };
+
+__device__ __forceinline__ Ph4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0; c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return Ph4{c0, c1, c2, c3};
+}
+
+__device__ __forceinline__ Ph4 draw(const Params &P, uint32_t stream, uint32_t gid, int32_t t, uint32_t slot, uint32_t sub)
+{
+    return philox4x32_10(gid, (uint32_t)t, slot, sub, P.seed_lo, P.seed_hi ^ stream);
+}
+
+// R3: u = (x >> 8) * 2^-24
+__device__ __forceinline__ float u24(uint32_t x) { return __uint2float_rn(x >> 8) * 0x1p-24f; }
+
+// ----------------------------------------------------------------------------------------------- R23
+__device__ __forceinline__ float im_exp(float x)
+{
+    if (x < -80.0f) return 0.0f;
+    const float n = rintf(__fmul_rn(x, 0x1.715476p+0f));
+    float r = __fmaf_rn(n, -0x1.62e400p-1f, x);
+    r = __fmaf_rn(n, -0x1.7f7d1cp-20f, r);
+    float p = 0x1.6c16c2p-10f;
+    p = __fmaf_rn(p, r, 0x1.111112p-7f);
+    p = __fmaf_rn(p, r, 0x1.555556p-5f);
+    p = __fmaf_rn(p, r, 0x1.555556p-3f);
+    p = __fmaf_rn(p, r, 0.5f);
+    p = __fmaf_rn(p, r, 1.0f);
+    p = __fmaf_rn(p, r, 1.0f);
+    return __fmul_rn(p, __int_as_float(((int)n + 127) << 23));   // exact scaling by 2^n, n in [-116, 0]
+}
+
+__device__ __forceinline__ float im_tanh(float x)
+{
+    const float e = im_exp(__fmul_rn(-2.0f, fabsf(x)));
+    const float q = __fdiv_rn(__fsub_rn(1.0f, e), __fadd_rn(1.0f, e));
+    return copysignf(q, x);
+}
+
+// ----------------------------------------------------------------------------------------------- R24
+// Sequential softmax inverse-CDF over n <= 48 logits read through `get(i)`; returns the action, writes logp.
+template <typename F>
+__device__ __forceinline__ uint32_t sample_head(F get, uint32_t n, float u, float &logp)
+{
+    float m = get(0);
+    for (uint32_t i = 1; i < n; i++) m = fmaxf(m, get(i));
+    float Z = 0.0f;
+    for (uint32_t i = 0; i < n; i++) Z = __fadd_rn(Z, im_exp(__fsub_rn(get(i), m)));
+    const float th = __fmul_rn(u, Z);
+    uint32_t a = n - 1;
+    float c = 0.0f;
+    for (uint32_t i = 0; i < n; i++) {
+        c = __fadd_rn(c, im_exp(__fsub_rn(get(i), m)));
+        if (c > th) { a = i; break; }
+    }
+    logp = __fsub_rn(__fsub_rn(get(a), m), logf(Z));
+    return a;
+}
+
+// ----------------------------------------------------------------------------------------------- R17
+__device__ __forceinline__ uint32_t keff_of(uint32_t topo, uint32_t K) { return topo == 0 ? 1u : (topo == 1 ? K : (K < 2 ? 2u : K)); }
+__device__ __forceinline__ uint32_t nstages_of(uint32_t topo, uint32_t keff) { return topo == 0 ? 1u : (topo == 1 ? keff : 2u); }
+__device__ __forceinline__ void stage_calls(uint32_t topo, uint32_t keff, uint32_t stage, uint32_t &a0, uint32_t &nc)
+{
+    if (topo == 0) { a0 = 0; nc = 1; }
+    else if (topo == 1) { a0 = stage; nc = 1; }
+    else if (topo == 2) { if (stage == 0) { a0 = 0; nc = keff - 1; } else { a0 = keff - 1; nc = 1; } }
+    else { if (stage == 0) { a0 = 0; nc = 1; } else { a0 = 1; nc = keff - 1; } }
+}
+
+__device__ __forceinline__ uint32_t row_gid(const RowBuf &rb, uint32_t region, uint32_t idx) { return region * rb.regcap + (idx % rb.regcap); }
+
+// claim n consecutive rows of region `region`; flags overflow in log mode
+__device__ __forceinline__ uint32_t rows_claim(const Params &P, const RowBuf &rb, uint32_t region, uint32_t n)
+{
+    const uint32_t idx = atomicAdd(&rb.cnt[region], n);
+    if (P.log_mode && idx + n > rb.regcap) atomicOr(P.err_flag, 1u);
+    return idx;
+}
+
+}  // namespace im

@@ -1,0 +1,436 @@
+// im_policy.cu — batched planner / executor / critic MLP forward + inverse-CDF sampling (R15-R26).
+//
+// Work comes as row lists written by k_sim (and, for stage 0 of new queries, by the planner kernel itself);
+// the executor launch also evaluates one critic row per env (R30).  Two numerics contracts:
+//   fp32 (R22): y = b; for k ascending: y = fmaf(W[o][k], x[k], y); tanh = im_tanh  -> bit-exact vs the oracle.
+//   bf16 (R25): bf16 operands, fp32 accumulation on the tensor cores (mma.sync m16n8k16 in this version),
+//               tanh.approx, fp32 logits; sampling by the exact R24 sampler on those logits.
+#include "im_device.cuh"
+#include <cuda_bf16.h>
+
+namespace im {
+
+struct RowInfo { uint32_t env, a, c; float b; uint32_t gidx; bool critic; };
+
+// ------------------------------------------------------------------------------------------------ tiles
+struct TileSched {
+    uint32_t pref[kRegions + 1];
+    uint32_t base[kRegions];
+    uint32_t crit_tiles, total;
+};
+
+__device__ __forceinline__ void sched_init(TileSched &S, const RowBuf &rb, uint32_t parity, uint32_t rows_per_tile, uint32_t n_crit)
+{
+    if (threadIdx.x < kRegions) {
+        const uint32_t b = rb.base[parity * kRegions + threadIdx.x], c = rb.cnt[threadIdx.x];
+        S.base[threadIdx.x] = b;
+        S.pref[threadIdx.x + 1] = (c - b + rows_per_tile - 1) / rows_per_tile;
+        if (blockIdx.x == 0) rb.base[(parity ^ 1u) * kRegions + threadIdx.x] = c;   // next tick starts here
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        S.crit_tiles = (n_crit + rows_per_tile - 1) / rows_per_tile;
+        S.pref[0] = 0;
+        for (uint32_t r = 0; r < kRegions; r++) S.pref[r + 1] += S.pref[r];
+        S.total = S.crit_tiles + S.pref[kRegions];
+    }
+    __syncthreads();
+}
+
+// row `r` of tile `tile`: fills info, returns false if out of range
+__device__ __forceinline__ bool tile_row(const TileSched &S, const RowBuf &rb, uint32_t tile, uint32_t r, uint32_t rows_per_tile,
+                                         uint32_t n_crit, RowInfo &ri)
+{
+    if (tile < S.crit_tiles) {
+        const uint32_t env = tile * rows_per_tile + r;
+        if (env >= n_crit) return false;
+        ri.env = env; ri.a = 0; ri.c = 0; ri.b = 0.0f; ri.gidx = 0; ri.critic = true;
+        return true;
+    }
+    const uint32_t lt = tile - S.crit_tiles;
+    uint32_t lo = 0, hi = kRegions;
+    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
+    const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * rows_per_tile + r;
+    if (idx >= rb.cnt[lo]) return false;
+    const uint32_t g = row_gid(rb, lo, idx);
+    ri.env = rb.env[g]; ri.a = rb.a[g]; ri.c = rb.c[g]; ri.b = rb.b[g]; ri.gidx = g; ri.critic = false;
+    return true;
+}
+
+// feature k of a row (R15)
+__device__ __forceinline__ float feature(const Params &P, bool exec, const RowInfo &ri, uint32_t k)
+{
+    const uint32_t N3 = 3 * P.N;
+    if (k == 0) return ri.b;
+    if (k <= N3) return P.snap[(size_t)ri.env * N3 + (k - 1)];
+    if (ri.critic) return 0.0f;
+    if (k == N3 + 1) return __uint2float_rn(ri.c & 0xFFFFu) * 0x1p-13f;
+    if (!exec) return 0.0f;
+    const uint32_t j = k - (N3 + 2);
+    if (j < 4) return j == ((ri.a >> 12) & 3u) ? 1.0f : 0.0f;
+    if (j < 8) return (j - 4) == ((ri.a >> 14) & 3u) ? 1.0f : 0.0f;
+    if (j == 8) return __uint2float_rn((ri.a >> 10) & 3u) * 0.25f;
+    if (j == 9) return __uint2float_rn((ri.a >> 16) & 7u) * 0.25f;
+    return 0.0f;
+}
+
+// ------------------------------------------------------------------------------------------- epilogues
+// sequential R24 sampler over logits l[0..n) (shared memory); e[] is scratch of n floats
+__device__ __forceinline__ uint32_t sample_seq(const float *l, float *e, uint32_t n, float u, float &logp)
+{
+    float m = l[0];
+    for (uint32_t i = 1; i < n; i++) m = fmaxf(m, l[i]);
+    float Z = 0.0f;
+    for (uint32_t i = 0; i < n; i++) { const float v = im_exp(__fsub_rn(l[i], m)); e[i] = v; Z = __fadd_rn(Z, v); }
+    const float th = __fmul_rn(u, Z);
+    uint32_t a = n - 1;
+    float c = 0.0f;
+    for (uint32_t i = 0; i < n; i++) { c = __fadd_rn(c, e[i]); if (c > th) { a = i; break; } }
+    logp = __fsub_rn(__fsub_rn(l[a], m), logf(Z));
+    return a;
+}
+
+// executor / critic row: logits[0..3N) + value at 3N
+__device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri, const float *logits, float *scratch,
+                                              int32_t t0, uint32_t trow)
+{
+    const uint32_t n = 3 * P.N;
+    const float value = logits[n];
+    if (ri.critic) { P.val[(size_t)trow * P.E + ri.env] = value; return; }
+    const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
+    const int32_t t = t0 + (int32_t)(ri.a >> 19);
+    if (P.exec.logits) for (uint32_t i = 0; i <= n; i++) P.exec.logits[(size_t)ri.gidx * P.exec.n_out + i] = logits[i];
+    const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
+    float logp;
+    const uint32_t act = sample_seq(logits, scratch, n, u24(d.x), logp);
+    P.exec.c[ri.gidx] = (ri.c & 0xFFFFu) | (act << 16);
+    P.exec.logp[ri.gidx] = logp;
+    P.exec.val[ri.gidx] = value;
+}
+
+// planner row: 24 logits = [4 topology | 4 count | 4 agents x 4 roles] (R16); emits the stage-0 executor rows (R17)
+__device__ __forceinline__ void plan_epilogue(const Params &P, const RowInfo &ri, const float *logits, float *scratch, int32_t t0)
+{
+    const uint32_t q = ri.a & 0x3FFu, t_rel = ri.a >> 19;
+    const int32_t t = t0 + (int32_t)t_rel;
+    const uint32_t gid = P.env_id_base + ri.env;
+    if (P.plan.logits) for (uint32_t i = 0; i < 24; i++) P.plan.logits[(size_t)ri.gidx * 24 + i] = logits[i];
+    const Ph4 d0 = draw(P, STREAM_PLAN, gid, t, q, 0), d1 = draw(P, STREAM_PLAN, gid, t, q, 1);
+    float lp_t, lp_c, lp_r[4];
+    const uint32_t topo = sample_seq(logits, scratch, 4, u24(d0.x), lp_t);
+    const uint32_t cnt = sample_seq(logits + 4, scratch, 4, u24(d0.y), lp_c);
+    const uint32_t ur[4] = {d1.x, d1.y, d1.z, d1.w};
+    uint32_t roles = 0;
+#pragma unroll
+    for (uint32_t a = 0; a < 4; a++) roles |= sample_seq(logits + 8 + 4 * a, scratch, 4, u24(ur[a]), lp_r[a]) << (2 * a);
+    const uint32_t keff = keff_of(topo, cnt + 1), nst = nstages_of(topo, keff);
+    float lp = __fadd_rn(lp_t, lp_c);
+#pragma unroll
+    for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
+    P.plan.c[ri.gidx] = (ri.c & 0xFFFFu) | ((topo | (cnt << 2) | (roles << 4)) << 16);
+    P.plan.logp[ri.gidx] = lp;
+    const size_t qi = (size_t)ri.env * P.QCAP + q;
+    P.q_plan[qi] = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
+    // stage 0 executor rows
+    uint32_t a0, nc;
+    stage_calls(topo, keff, 0, a0, nc);
+    const uint32_t region = ri.env % kRegions;
+    const uint32_t idx0 = rows_claim(P, P.exec, region, nc);
+    P.q_row[qi] = idx0;
+    float b = __fdiv_rn(__int2float_rn(P.q_dl[qi] - t), __uint2float_rn(P.budget_norm));
+    b = fminf(fmaxf(b, -1.0f), 1.0f);
+    for (uint32_t j = 0; j < nc; j++) {
+        const uint32_t agent = a0 + j, g = row_gid(P.exec, region, idx0 + j);
+        P.exec.env[g] = ri.env;
+        P.exec.a[g] = q | (agent << 10) | (topo << 12) | (((roles >> (2 * agent)) & 3u) << 14) | (keff << 16) | (t_rel << 19);
+        P.exec.b[g] = b;
+        P.exec.c[g] = ri.c & 0xFFFFu;
+    }
+    atomicOr(&P.q_ready[(size_t)ri.env * P.QW + (q >> 5)], 1u << (q & 31));
+}
+
+// ================================================================================================ fp32 path (R22)
+constexpr int kF32Warps = 8, kF32RowsPerWarp = 4, kF32Rows = kF32Warps * kF32RowsPerWarp;
+
+template <bool EXEC>
+__global__ void __launch_bounds__(kF32Warps * 32)
+k_policy_f32(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32_t trow)
+{
+    extern __shared__ __align__(16) float smem_f[];
+    __shared__ TileSched sched;
+    const uint32_t F = P.f_in, H = P.hidden, NO = W.n_out, NOP = W.n_out_pad;
+    float *sW1 = smem_f, *sW2 = sW1 + F * H, *sW3 = sW2 + H * H, *sb1 = sW3 + H * NOP, *sb2 = sb1 + H, *sb3 = sb2 + H;
+    float *sx = sb3 + NOP;                               // per warp: [4][F] + [4][H] + [4][H] + [4][64] logits + [4][64] scratch
+    for (uint32_t i = threadIdx.x; i < F * H; i += blockDim.x) sW1[i] = W.W1t[i];
+    for (uint32_t i = threadIdx.x; i < H * H; i += blockDim.x) sW2[i] = W.W2t[i];
+    for (uint32_t i = threadIdx.x; i < H * NOP; i += blockDim.x) sW3[i] = W.W3t[i];
+    for (uint32_t i = threadIdx.x; i < H; i += blockDim.x) { sb1[i] = W.b1[i]; sb2[i] = W.b2[i]; }
+    for (uint32_t i = threadIdx.x; i < NOP; i += blockDim.x) sb3[i] = W.b3[i];
+    const RowBuf &rb = EXEC ? P.exec : P.plan;
+    const uint32_t n_crit = EXEC ? P.E : 0u;
+    sched_init(sched, rb, parity, kF32Rows, n_crit);
+
+    const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const uint32_t per_warp = kF32RowsPerWarp * (F + 2 * H + 128);
+    float *x = sx + wib * per_warp, *h1 = x + kF32RowsPerWarp * F, *h2 = h1 + kF32RowsPerWarp * H, *lg = h2 + kF32RowsPerWarp * H;
+    float *scr = lg + kF32RowsPerWarp * 64;
+
+    for (uint32_t tile = blockIdx.x; tile < sched.total; tile += gridDim.x) {
+        RowInfo ri[kF32RowsPerWarp];
+        bool ok[kF32RowsPerWarp];
+#pragma unroll
+        for (int r = 0; r < kF32RowsPerWarp; r++) {
+            ok[r] = tile_row(sched, rb, tile, wib * kF32RowsPerWarp + r, kF32Rows, n_crit, ri[r]);
+            for (uint32_t k = lane; k < F; k += 32) x[r * F + k] = ok[r] ? feature(P, EXEC, ri[r], k) : 0.0f;
+        }
+        __syncwarp();
+        if (!(ok[0] | ok[1] | ok[2] | ok[3])) continue;
+        for (uint32_t o = lane; o < H; o += 32) {
+            float acc[kF32RowsPerWarp];
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) acc[r] = sb1[o];
+            for (uint32_t k = 0; k < F; k++) {
+                const float w = sW1[k * H + o];
+#pragma unroll
+                for (int r = 0; r < kF32RowsPerWarp; r++) acc[r] = __fmaf_rn(w, x[r * F + k], acc[r]);
+            }
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) h1[r * H + o] = im_tanh(acc[r]);
+        }
+        __syncwarp();
+        for (uint32_t o = lane; o < H; o += 32) {
+            float acc[kF32RowsPerWarp];
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) acc[r] = sb2[o];
+            for (uint32_t k = 0; k < H; k++) {
+                const float w = sW2[k * H + o];
+#pragma unroll
+                for (int r = 0; r < kF32RowsPerWarp; r++) acc[r] = __fmaf_rn(w, h1[r * H + k], acc[r]);
+            }
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) h2[r * H + o] = im_tanh(acc[r]);
+        }
+        __syncwarp();
+        for (uint32_t o = lane; o < NO; o += 32) {
+            float acc[kF32RowsPerWarp];
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) acc[r] = sb3[o];
+            for (uint32_t k = 0; k < H; k++) {
+                const float w = sW3[k * NOP + o];
+#pragma unroll
+                for (int r = 0; r < kF32RowsPerWarp; r++) acc[r] = __fmaf_rn(w, h2[r * H + k], acc[r]);
+            }
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) lg[r * 64 + o] = acc[r];
+        }
+        __syncwarp();
+        if (lane < kF32RowsPerWarp) {
+            // lane r finishes row r
+            bool mine = false; RowInfo mi = ri[0];
+#pragma unroll
+            for (int r = 0; r < kF32RowsPerWarp; r++) if (lane == (uint32_t)r) { mine = ok[r]; mi = ri[r]; }
+            if (mine) {
+                if (EXEC) exec_epilogue(P, mi, lg + lane * 64, scr + lane * 64, t0, trow);
+                else plan_epilogue(P, mi, lg + lane * 64, scr + lane * 64, t0);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP)
+{
+    return 4ull * (F * H + H * H + H * NOP + 2 * H + NOP + kF32Warps * kF32RowsPerWarp * (F + 2 * H + 128));
+}
+
+// ================================================================================================ bf16 path (R25)
+// One CTA computes a tile of 128 rows through the three layers with mma.sync.m16n8k16 (bf16 x bf16 -> fp32).
+// Activations live in shared memory (bf16, padded rows), weights stream from L2 as B fragments.
+constexpr int kBfRows = 128, kBfWarps = 16;
+
+__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], const void *p)
+{
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(p);
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ float tanh_fast(float x)
+{
+    float y;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// out[128][NT*8*nwarps...] = act[128][K] * W^T ; each warp owns NT n-tiles starting at n0 and all 8 m-tiles
+template <int K, int NT>
+__device__ __forceinline__ void layer_mma(const __nv_bfloat16 *act, int lda, const __nv_bfloat16 *W, int n0, float (&acc)[8][NT][4], uint32_t lane)
+{
+#pragma unroll
+    for (int mt = 0; mt < 8; mt++)
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++)
+#pragma unroll
+            for (int i = 0; i < 4; i++) acc[mt][nt][i] = 0.0f;
+    const int g = lane >> 2, tq = lane & 3;
+    const int lrow = lane & 15, lcol = (lane >> 4) * 8;
+#pragma unroll 2
+    for (int k0 = 0; k0 < K; k0 += 16) {
+        uint32_t b[NT][2];
+#pragma unroll
+        for (int nt = 0; nt < NT; nt++) {
+            const __nv_bfloat16 *wp = W + (size_t)(n0 + nt * 8 + g) * K + k0 + 2 * tq;
+            b[nt][0] = __ldg(reinterpret_cast<const unsigned int *>(wp));
+            b[nt][1] = __ldg(reinterpret_cast<const unsigned int *>(wp + 8));
+        }
+#pragma unroll
+        for (int mt = 0; mt < 8; mt++) {
+            uint32_t a[4];
+            ldmatrix_x4(a, act + (size_t)(mt * 16 + lrow) * lda + k0 + lcol);
+#pragma unroll
+            for (int nt = 0; nt < NT; nt++) mma_bf16(acc[mt][nt], a, b[nt][0], b[nt][1]);
+        }
+    }
+}
+
+template <int F, int H, bool EXEC>
+__global__ void __launch_bounds__(kBfWarps * 32, 1)
+k_policy_bf16(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32_t trow)
+{
+    constexpr int LDA = H + 8;                     // padded row (bf16 elements): conflict-free ldmatrix
+    constexpr int NT_H = H / 8 / kBfWarps;         // n-tiles per warp in the hidden layers
+    static_assert(NT_H >= 1, "hidden width too small for 16 warps");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ TileSched sched;
+    __shared__ RowInfo s_ri[kBfRows];
+    __shared__ uint8_t s_ok[kBfRows];
+    __nv_bfloat16 *actA = reinterpret_cast<__nv_bfloat16 *>(smem_raw);
+    __nv_bfloat16 *actB = actA + kBfRows * LDA;
+    float *lg = reinterpret_cast<float *>(actA);   // logits [128][64] fp32 reuse actA after layer 2 consumed it
+    const RowBuf &rb = EXEC ? P.exec : P.plan;
+    const uint32_t n_crit = EXEC ? P.E : 0u;
+    sched_init(sched, rb, parity, kBfRows, n_crit);
+    const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int g = lane >> 2, tq = lane & 3;
+    const uint32_t n_tiles3 = W.n_out_pad / 8;
+
+    for (uint32_t tile = blockIdx.x; tile < sched.total; tile += gridDim.x) {
+        __syncthreads();
+        if (threadIdx.x < kBfRows) {
+            RowInfo ri;
+            const bool ok = tile_row(sched, rb, tile, threadIdx.x, kBfRows, n_crit, ri);
+            s_ri[threadIdx.x] = ri; s_ok[threadIdx.x] = ok;
+        }
+        __syncthreads();
+        // features -> actA (bf16, RNE)
+        for (uint32_t i = threadIdx.x; i < kBfRows * F; i += blockDim.x) {
+            const uint32_t r = i / F, k = i % F;
+            const float v = s_ok[r] ? feature(P, EXEC, s_ri[r], k) : 0.0f;
+            actA[r * LDA + k] = __float2bfloat16_rn(v);
+        }
+        __syncthreads();
+        // layer 1: actA[128][F] -> actB[128][H]
+        {
+            float acc[8][NT_H][4];
+            const int n0 = wib * NT_H * 8;
+            layer_mma<F, NT_H>(actA, LDA, W.W1, n0, acc, lane);
+#pragma unroll
+            for (int nt = 0; nt < NT_H; nt++) {
+                const int col = n0 + nt * 8 + 2 * tq;
+                const float bb0 = W.b1[col], bb1 = W.b1[col + 1];
+#pragma unroll
+                for (int mt = 0; mt < 8; mt++) {
+                    const int r0 = mt * 16 + g;
+                    *reinterpret_cast<__nv_bfloat162 *>(actB + r0 * LDA + col) =
+                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][0] + bb0), tanh_fast(acc[mt][nt][1] + bb1));
+                    *reinterpret_cast<__nv_bfloat162 *>(actB + (r0 + 8) * LDA + col) =
+                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][2] + bb0), tanh_fast(acc[mt][nt][3] + bb1));
+                }
+            }
+        }
+        __syncthreads();
+        // layer 2: actB[128][H] -> actA[128][H]
+        {
+            float acc[8][NT_H][4];
+            const int n0 = wib * NT_H * 8;
+            layer_mma<H, NT_H>(actB, LDA, W.W2, n0, acc, lane);
+#pragma unroll
+            for (int nt = 0; nt < NT_H; nt++) {
+                const int col = n0 + nt * 8 + 2 * tq;
+                const float bb0 = W.b2[col], bb1 = W.b2[col + 1];
+#pragma unroll
+                for (int mt = 0; mt < 8; mt++) {
+                    const int r0 = mt * 16 + g;
+                    *reinterpret_cast<__nv_bfloat162 *>(actA + r0 * LDA + col) =
+                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][0] + bb0), tanh_fast(acc[mt][nt][1] + bb1));
+                    *reinterpret_cast<__nv_bfloat162 *>(actA + (r0 + 8) * LDA + col) =
+                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][2] + bb0), tanh_fast(acc[mt][nt][3] + bb1));
+                }
+            }
+        }
+        __syncthreads();
+        // layer 3: actA[128][H] -> logits (registers), then to shared memory after everyone finished reading actA
+        float acc3[8][1][4];
+        const bool has3 = wib < n_tiles3;
+        if (has3) layer_mma<H, 1>(actA, LDA, W.W3, wib * 8, acc3, lane);
+        __syncthreads();
+        if (has3) {
+            const int col = wib * 8 + 2 * tq;
+            const float bb0 = W.b3[col], bb1 = W.b3[col + 1];
+#pragma unroll
+            for (int mt = 0; mt < 8; mt++) {
+                const int r0 = mt * 16 + g;
+                lg[r0 * 64 + col] = acc3[mt][0][0] + bb0; lg[r0 * 64 + col + 1] = acc3[mt][0][1] + bb1;
+                lg[(r0 + 8) * 64 + col] = acc3[mt][0][2] + bb0; lg[(r0 + 8) * 64 + col + 1] = acc3[mt][0][3] + bb1;
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x < kBfRows && s_ok[threadIdx.x]) {
+            float *scratch = reinterpret_cast<float *>(actB) + threadIdx.x * 64;   // actB is free now
+            if (EXEC) exec_epilogue(P, s_ri[threadIdx.x], lg + threadIdx.x * 64, scratch, t0, trow);
+            else plan_epilogue(P, s_ri[threadIdx.x], lg + threadIdx.x * 64, scratch, t0);
+        }
+    }
+}
+
+template <int F, int H>
+static size_t bf16_smem_bytes() { return 2ull * kBfRows * (H + 8) * 2; }
+
+// ------------------------------------------------------------------------------------------------ launchers
+int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm,
+                  bool bf16, cudaStream_t st)
+{
+    if (!bf16) {
+        const size_t smem = f32_smem_bytes(P.f_in, P.hidden, W.n_out_pad);
+        static size_t set_p = 0, set_e = 0;
+        if (exec) { if (set_e < smem) { cudaFuncSetAttribute(k_policy_f32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); set_e = smem; } }
+        else { if (set_p < smem) { cudaFuncSetAttribute(k_policy_f32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); set_p = smem; } }
+        const uint32_t grid = (uint32_t)n_sm * 2;
+        if (exec) k_policy_f32<true><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
+        else k_policy_f32<false><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
+        return 0;
+    }
+    const uint32_t grid = (uint32_t)n_sm;
+#define IM_BF16_CASE(FF, HH)                                                                                          \
+    if (P.f_in == FF && P.hidden == HH) {                                                                             \
+        const size_t smem = bf16_smem_bytes<FF, HH>();                                                                \
+        if (exec) {                                                                                                   \
+            cudaFuncSetAttribute(k_policy_bf16<FF, HH, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            k_policy_bf16<FF, HH, true><<<grid, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);                   \
+        } else {                                                                                                      \
+            cudaFuncSetAttribute(k_policy_bf16<FF, HH, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);\
+            k_policy_bf16<FF, HH, false><<<grid, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);                  \
+        }                                                                                                             \
+        return 0;                                                                                                     \
+    }
+    IM_BF16_CASE(64, 128)
+    IM_BF16_CASE(128, 256)
+#undef IM_BF16_CASE
+    return -1;
+}
+
+}  // namespace im

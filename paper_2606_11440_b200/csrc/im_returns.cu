@@ -1,0 +1,203 @@
+// im_returns.cu — (a) reverse-scan GAE with the Lagrangian reward r - mu*cost (Eq. 3; R29, R31),
+// (b) planner utility U_i = solved - mu*L_total/beta and its batch normalisation (Eq. 6; R32),
+// (c) the sums behind C-bar of the dual update (Eq. 7).
+//
+// GAE is a first-order linear recurrence along t for every env independently: one thread per env walks
+// t = T-1 .. 0 over [T][E] arrays (E fastest => every load/store of a warp is one coalesced 128-byte line).
+// HBM-bound: 13 B read + 8 B written per env-tick.  Loads are issued kBatch ticks ahead of the dependent
+// chain so that the walk is bandwidth- not latency-limited.  The arithmetic is the R31 sequence of separately
+// rounded fp32 operations.
+#include "im_device.cuh"
+
+namespace im {
+
+constexpr int kGaeBatch = 8;
+
+__global__ void __launch_bounds__(128)
+k_gae(const float *__restrict__ rew, const float *__restrict__ cost, const float *__restrict__ val,
+      const uint8_t *__restrict__ done, float *__restrict__ adv, float *__restrict__ ret, uint32_t T, uint32_t E,
+      float gamma, float lam, float mu, double *__restrict__ sums)
+{
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    double csum = 0.0;
+    if (e < E) {
+        const float gl = __fmul_rn(gamma, lam);
+        float A = 0.0f;
+        float vnext = val[(size_t)T * E + e];
+        int64_t t = (int64_t)T - 1;
+        while (t >= 0) {
+            const int nb = (int)(t + 1 < kGaeBatch ? t + 1 : kGaeBatch);
+            float r[kGaeBatch], c[kGaeBatch], v[kGaeBatch];
+            uint8_t d[kGaeBatch];
+#pragma unroll
+            for (int j = 0; j < kGaeBatch; j++)
+                if (j < nb) {
+                    const size_t i = (size_t)(t - j) * E + e;
+                    r[j] = __ldcs(rew + i); c[j] = __ldcs(cost + i); v[j] = __ldcs(val + i); d[j] = __ldcs(done + i);
+                }
+#pragma unroll
+            for (int j = 0; j < kGaeBatch; j++)
+                if (j < nb) {
+                    const size_t i = (size_t)(t - j) * E + e;
+                    const bool nd = d[j] == 0;
+                    const float rt = __fsub_rn(r[j], __fmul_rn(mu, c[j]));
+                    const float delta = __fsub_rn(__fadd_rn(rt, nd ? __fmul_rn(gamma, vnext) : 0.0f), v[j]);
+                    A = __fadd_rn(delta, nd ? __fmul_rn(gl, A) : 0.0f);
+                    __stcs(adv + i, A);
+                    __stcs(ret + i, __fadd_rn(A, v[j]));
+                    vnext = v[j];
+                    csum += (double)c[j];
+                }
+            t -= nb;
+        }
+    }
+    // sum of cost (for C-bar), block reduction then one atomic
+#pragma unroll
+    for (int o = 16; o; o >>= 1) csum += __shfl_xor_sync(0xffffffffu, csum, o);
+    __shared__ double s[4];
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = csum;
+    __syncthreads();
+    if (threadIdx.x == 0) atomicAdd(&sums[0], s[0] + s[1] + s[2] + s[3]);
+}
+
+// U_i per finished query; sums[1] += U, sums[2] += U^2, sums[3] += count
+__global__ void __launch_bounds__(256)
+k_utility(const QLog ql, float mu, double *__restrict__ sums)
+{
+    const uint32_t region = blockIdx.y;
+    const uint32_t n = min(ql.cnt[region], ql.regcap);
+    double su = 0.0, su2 = 0.0, cn = 0.0;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const size_t g = (size_t)region * ql.regcap + i;
+        const uint32_t info = ql.info[g];
+        const float U = __fsub_rn(__uint2float_rn((info >> 16) & 1u),
+                                  __fdiv_rn(__fmul_rn(mu, __uint2float_rn(ql.sojourn[g])), __uint2float_rn(info & 0xFFFFu)));
+        ql.unorm[g] = U;
+        su += (double)U; su2 += (double)U * (double)U; cn += 1.0;
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        su += __shfl_xor_sync(0xffffffffu, su, o); su2 += __shfl_xor_sync(0xffffffffu, su2, o); cn += __shfl_xor_sync(0xffffffffu, cn, o);
+    }
+    __shared__ double s[3][8];
+    if ((threadIdx.x & 31) == 0) { s[0][threadIdx.x >> 5] = su; s[1][threadIdx.x >> 5] = su2; s[2][threadIdx.x >> 5] = cn; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0, b = 0, c = 0;
+        for (int w = 0; w < 8; w++) { a += s[0][w]; b += s[1][w]; c += s[2][w]; }
+        if (c > 0) { atomicAdd(&sums[1], a); atomicAdd(&sums[2], b); atomicAdd(&sums[3], c); }
+    }
+}
+
+// (U - mean) / (sigma + 1e-8), population sigma
+__global__ void __launch_bounds__(256)
+k_unorm(const QLog ql, const double *__restrict__ sums)
+{
+    const uint32_t region = blockIdx.y;
+    const uint32_t n = min(ql.cnt[region], ql.regcap);
+    const double cnt = sums[3];
+    const double mean = cnt > 0 ? sums[1] / cnt : 0.0;
+    double var = cnt > 0 ? sums[2] / cnt - mean * mean : 0.0;
+    var = var > 0 ? var : 0.0;
+    const float fm = (float)mean, fs = (float)(sqrt(var) + 1e-8);
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const size_t g = (size_t)region * ql.regcap + i;
+        ql.unorm[g] = __fdiv_rn(__fsub_rn(ql.unorm[g], fm), fs);
+    }
+}
+
+int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st)
+{
+    cudaMemsetAsync(sums, 0, 4 * sizeof(double), st);
+    k_gae<<<(P.E + 127) / 128, 128, 0, st>>>(P.rew, P.cost, P.val, P.done, adv, ret, T, P.E, gamma, lam, mu, sums);
+    const dim3 grid(32, kRegions);
+    k_utility<<<grid, 256, 0, st>>>(P.qlog, mu, sums);
+    k_unorm<<<grid, 256, 0, st>>>(P.qlog, sums);
+    return 3;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Slack-ordered queue (R20): per env, all WAITING requests sorted by (model, key) with a warp-level segmented bitonic
+// sort — shared-memory staging, strides >= 32 exchanged through shared memory, strides < 32 by warp shuffles.
+// Serves IM_TEL_QUEUE_ORDER; the admission phase of k_sim extracts only the few smallest keys it can admit.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int kQoWarps = 4;
+
+__global__ void __launch_bounds__(kQoWarps * 32)
+k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
+{
+    extern __shared__ __align__(16) unsigned long long s_keys[];
+    const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const uint32_t e = blockIdx.x * kQoWarps + wib;
+    if (e >= P.E) return;
+    uint32_t n2cap = 32;
+    while (n2cap < P.RCAP) n2cap <<= 1;
+    unsigned long long *keys = s_keys + (size_t)wib * n2cap;
+    const uint32_t *r_meta = P.r_meta + (size_t)e * P.RCAP;
+    const int32_t *r_dl = P.r_dl + (size_t)e * P.RCAP, *r_issue = P.r_issue + (size_t)e * P.RCAP;
+    uint32_t n = 0;
+    uint32_t per_model = 0;                       // lane k counts model k
+    for (uint32_t i0 = 0; i0 < P.RCAP; i0 += 32) {
+        const uint32_t i = i0 + lane;
+        const uint32_t m = r_meta[i];
+        const bool w = (m & 3u) == ST_WAIT;
+        const uint32_t bal = __ballot_sync(0xffffffffu, w);
+        if (w) {
+            const int32_t base = P.sched_mode ? r_dl[i] : r_issue[i];
+            const uint32_t key = ((uint32_t)(base - t + (1 << 19)) << 12) | i;
+            keys[n + __popc(bal & ((1u << lane) - 1u))] = ((unsigned long long)((m >> 2) & 15u) << 32) | key;
+        }
+        for (uint32_t k = 0; k < P.N; k++) {
+            const uint32_t c = __popc(__ballot_sync(0xffffffffu, w && ((m >> 2) & 15u) == k));
+            if (lane == k) per_model += c;
+        }
+        n += __popc(bal);
+    }
+    uint32_t n2 = 32;
+    while (n2 < n) n2 <<= 1;
+    for (uint32_t i = n + lane; i < n2; i += 32) keys[i] = ~0ull;
+    __syncwarp();
+    for (uint32_t k = 2; k <= n2; k <<= 1) {
+        uint32_t j = k >> 1;
+        for (; j >= 32; j >>= 1) {                 // shared-memory exchanges
+            for (uint32_t i = lane; i < n2; i += 32) {
+                const uint32_t p = i ^ j;
+                if (p > i) {
+                    const unsigned long long a = keys[i], b = keys[p];
+                    const bool up = (i & k) == 0;
+                    if ((a > b) == up) { keys[i] = b; keys[p] = a; }
+                }
+            }
+            __syncwarp();
+        }
+        for (uint32_t it = 0; it < n2; it += 32) { // warp-shuffle exchanges within 32 consecutive keys
+            const uint32_t i = it + lane;
+            unsigned long long v = keys[i];
+            const bool up = (i & k) == 0;
+            for (uint32_t jj = j; jj > 0; jj >>= 1) {
+                const unsigned long long o = __shfl_xor_sync(0xffffffffu, v, jj);
+                const bool lower = (lane & jj) == 0;
+                v = (lower == up) ? (v < o ? v : o) : (v > o ? v : o);
+            }
+            keys[i] = v;
+        }
+        __syncwarp();
+    }
+    uint32_t *o = out + (size_t)e * (P.N + 1 + P.RCAP);
+    const uint32_t inc = [&] { uint32_t v = per_model; for (int s = 1; s < 32; s <<= 1) { const uint32_t u = __shfl_up_sync(0xffffffffu, v, s); if (lane >= (uint32_t)s) v += u; } return v; }();
+    if (lane < P.N) o[lane + 1] = inc;
+    if (lane == 0) o[0] = 0;
+    for (uint32_t i = lane; i < P.RCAP; i += 32) o[P.N + 1 + i] = i < n ? (uint32_t)(keys[i] & 0xFFFu) : 0xFFFFFFFFu;
+}
+
+int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st)
+{
+    uint32_t n2cap = 32;
+    while (n2cap < P.RCAP) n2cap <<= 1;
+    const size_t smem = (size_t)kQoWarps * n2cap * 8;
+    cudaFuncSetAttribute(k_queue_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    k_queue_order<<<(P.E + kQoWarps - 1) / kQoWarps, kQoWarps * 32, smem, st>>>(P, t, out);
+    return 1;
+}
+
+}  // namespace im
