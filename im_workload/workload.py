@@ -128,14 +128,16 @@ def exponential_table_q16(n: int = 1024) -> np.ndarray:
 CONFIGS: Dict[int, dict] = {
     1: dict(E=64, N=5, T=200, dtype=0, f_in=32, hidden=64, qcap=256, rcap=768),
     2: dict(E=4096, N=5, T=2000, dtype=0, f_in=32, hidden=64, qcap=256, rcap=768),
-    3: dict(E=65536, N=8, T=4000, dtype=1, f_in=64, hidden=128, qcap=256, rcap=768),
-    4: dict(E=131072, N=16, T=4000, dtype=1, f_in=128, hidden=256, qcap=512, rcap=1536),
+    # chunk: ticks per im_rollout call (trajectory / log capacity); the 4000-tick rollouts of configs 3-4 run as
+    # 8 consecutive calls of 500 ticks with persistent env state, so that the logs of one call fit in HBM
+    3: dict(E=65536, N=8, T=4000, dtype=1, f_in=64, hidden=128, qcap=256, rcap=768, chunk=500),
+    4: dict(E=131072, N=16, T=4000, dtype=1, f_in=128, hidden=256, qcap=512, rcap=1536, chunk=500),
     5: dict(E=262144, N=16, T=512, dtype=1, f_in=128, hidden=256, qcap=512, rcap=1536),
 }
 
 
 def make_pool_spec(config_id: int, seed: int = 0, n_envs: Optional[int] = None,
-                   n_ticks: Optional[int] = None, debug_flags: int = 0) -> PoolSpec:
+                   n_ticks: Optional[int] = None, debug_flags: int = 0, max_ticks: Optional[int] = None) -> PoolSpec:
     """Materialise BASELINE.json configs[config_id-1] from `seed`.
 
     n_envs / n_ticks override E / T for parity tests on a slice; pool rows depend only on
@@ -146,6 +148,7 @@ def make_pool_spec(config_id: int, seed: int = 0, n_envs: Optional[int] = None,
     E_full, N, T = cfg["E"], cfg["N"], cfg["T"]
     E = E_full if n_envs is None else int(n_envs)
     T = T if n_ticks is None else int(n_ticks)
+    chunk = min(T, int(max_ticks) if max_ticks is not None else cfg.get("chunk", T))
     rng = np.random.Generator(np.random.PCG64([config_id, seed, 0x1F2A]))
 
     if config_id in (1, 2):
@@ -206,11 +209,11 @@ def make_pool_spec(config_id: int, seed: int = 0, n_envs: Optional[int] = None,
     in_tok_table = lognormal_table(800.0, 0.6) if config_id >= 4 else None
 
     mean_rate = float(np.mean(rates_tick[env_level.astype(np.int64)])) if E > 0 else 0.0
-    exec_nom = E * T * mean_rate * 2.25
-    plan_nom = E * T * mean_rate
+    exec_nom = E * chunk * mean_rate * 2.25
+    plan_nom = E * chunk * mean_rate
     spec = PoolSpec(
         config_id=config_id, n_envs=E, n_ticks=T, n_models=N,
-        qcap=cfg["qcap"], rcap=cfg["rcap"], max_ticks=T,
+        qcap=cfg["qcap"], rcap=cfg["rcap"], max_ticks=chunk,
         sched_mode=1, kv_preempt=kv_preempt, cost_mode=0, episode_ticks=0,
         budget_norm_ticks=budget_norm, n_levels=n_levels,
         policy_dtype=cfg["dtype"], f_in=cfg["f_in"], hidden=cfg["hidden"],
@@ -222,7 +225,7 @@ def make_pool_spec(config_id: int, seed: int = 0, n_envs: Optional[int] = None,
         kv_inv=(1.0 / kv.astype(np.float64)).astype(np.float32),
         out_tok_mult_q16=lognormal_table(1.0, 0.4, scale=65536.0),
         in_tok_table=in_tok_table, arr_cdf=arr_cdf, env_level=env_level,
-        log_cap_exec=int(exec_nom * 1.6) + 64 * E + 4096,
+        log_cap_exec=int(exec_nom * 1.4) + 64 * E + 4096,
         log_cap_plan=int(plan_nom * 1.3) + 32 * E + 4096,
         log_cap_query=int(plan_nom * 1.3) + 32 * E + 4096,
         arr_rate_tick=np.asarray(rates_tick, dtype=np.float64), succ_prob=p,

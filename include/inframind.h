@@ -169,6 +169,17 @@ int im_device_ptr(im_ctx *ctx, uint32_t what, void **dev_ptr, size_t *bytes);
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 uint64_t im_launch_count(const im_ctx *ctx);
 
+/* Per-kernel-class device timing for roofline reports: when enabled, every launch of im_rollout / im_returns is
+ * bracketed by CUDA events on the bound stream. im_kernel_times synchronises, returns the accumulated
+ * milliseconds and launch counts per class since the last call, and clears them. HOST arrays of IM_KERNEL_CLASSES. */
+#define IM_KERNEL_SIM 0       /* k_sim: tick phases A, B, D-issue .. I */
+#define IM_KERNEL_PLAN 1      /* planner MLP + sampling */
+#define IM_KERNEL_EXEC 2      /* executor + critic MLP + sampling */
+#define IM_KERNEL_RETURNS 3   /* GAE + utility kernels of one im_returns */
+#define IM_KERNEL_CLASSES 4
+int im_set_profiling(im_ctx *ctx, int enable);
+int im_kernel_times(im_ctx *ctx, double *ms, uint64_t *launches);
+
 void im_destroy(im_ctx *ctx);
 
 /* Message of the last failing call on this ctx (string owned by ctx, valid until the next call); "" if none.

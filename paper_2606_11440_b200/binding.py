@@ -23,7 +23,7 @@ IM_FLAG_LOG_DECISIONS, IM_FLAG_LOG_LOGITS = 1, 2
  IM_TEL_QUEUE_ORDER, IM_TEL_TABLES, IM_TEL_LOGITS_EXEC, IM_TEL_LOGITS_PLAN) = range(1, 20)
 
 EXPORTS = ["im_arena_bytes", "im_create", "im_bind", "im_reset", "im_rollout", "im_returns", "im_read_telemetry",
-           "im_device_ptr", "im_launch_count", "im_destroy", "im_last_error"]
+           "im_device_ptr", "im_launch_count", "im_set_profiling", "im_kernel_times", "im_destroy", "im_last_error"]
 
 
 class im_model_spec(C.Structure):
@@ -65,6 +65,8 @@ def load_library():
         L.im_device_ptr.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
         L.im_launch_count.restype = C.c_uint64
         L.im_launch_count.argtypes = [C.c_void_p]
+        L.im_set_profiling.argtypes = [C.c_void_p, C.c_int]
+        L.im_kernel_times.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.im_destroy.restype = None
         L.im_destroy.argtypes = [C.c_void_p]
         L.im_last_error.restype = C.c_char_p
@@ -112,7 +114,8 @@ class IMError(RuntimeError):
 class InfraMind:
     """im_create + im_bind on a torch-owned arena; methods mirror the C ABI one to one."""
 
-    def __init__(self, spec, seed: int = 0, device: str = "cuda:0", debug_flags: Optional[int] = None, stream=None):
+    def __init__(self, spec, seed: int = 0, device: str = "cuda:0", debug_flags: Optional[int] = None, stream=None,
+                 arena=None):
         import torch
         self._L = load_library()
         self.spec = spec
@@ -130,7 +133,9 @@ class InfraMind:
             raise RuntimeError("no CUDA device: libinframind has no CPU fallback")
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.arena = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        # `arena` lets several contexts of the SAME spec (e.g. one per seed) share one allocation, used one at a time
+        self.arena = arena if arena is not None else torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        assert self.arena.numel() >= nbytes + 256
         ptr = (self.arena.data_ptr() + 255) & ~255
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._check(self._L.im_bind(self._h, C.c_void_p(ptr), nbytes, C.c_void_p(self.stream.cuda_stream)))
@@ -235,6 +240,16 @@ class InfraMind:
         base = (self.arena.data_ptr() + 255) & ~255
         off = p.value - base + (base - self.arena.data_ptr())
         return self.arena[off: off + b.value].view(dtype)
+
+    def set_profiling(self, on: bool):
+        self._check(self._L.im_set_profiling(self._h, 1 if on else 0))
+
+    def kernel_times(self):
+        """{'sim': (ms, launches), 'plan': ..., 'exec': ..., 'returns': ...} since the last call."""
+        ms = (C.c_double * 4)()
+        n = (C.c_uint64 * 4)()
+        self._check(self._L.im_kernel_times(self._h, ms, n))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("sim", "plan", "exec", "returns"))}
 
     @property
     def launches(self) -> int:

@@ -75,7 +75,42 @@ struct im_ctx {
     std::string err;
     // state region (for reset)
     size_t state_off = 0, state_bytes = 0;
+    // optional per-kernel-class timing with CUDA events on the bound stream (im_set_profiling)
+    bool prof = false;
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> ev_class;
+    size_t ev_used = 0;
+    double prof_ms[IM_KERNEL_CLASSES] = {0, 0, 0, 0};
+    uint64_t prof_n[IM_KERNEL_CLASSES] = {0, 0, 0, 0};
 };
+
+static void prof_begin(im_ctx *c, int cls)
+{
+    if (!c->prof) return;
+    if (c->ev_used + 2 > c->ev.size()) {
+        const size_t old = c->ev.size();
+        c->ev.resize(old + 1024);
+        for (size_t i = old; i < c->ev.size(); i++) cudaEventCreate(&c->ev[i]);
+    }
+    c->ev_class.push_back(cls);
+    cudaEventRecord(c->ev[c->ev_used++], c->stream);
+}
+static void prof_end(im_ctx *c)
+{
+    if (!c->prof) return;
+    cudaEventRecord(c->ev[c->ev_used++], c->stream);
+}
+static void prof_collect(im_ctx *c)
+{
+    for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]) == cudaSuccess) {
+            const int cls = c->ev_class[i / 2];
+            c->prof_ms[cls] += ms; c->prof_n[cls]++;
+        }
+    }
+    c->ev_used = 0; c->ev_class.clear();
+}
 
 static int fail(im_ctx *c, int code, const char *fmt, ...)
 {
@@ -383,19 +418,29 @@ int im_rollout(im_ctx *c, const void *policy_weights, uint32_t n_ticks)
     }
     CUDA_TRY(c, cudaMemsetAsync(P.qlog.cnt, 0, sizeof(uint32_t) * kRegions, st));
     const int32_t t0 = c->tick;
+    prof_begin(c, IM_KERNEL_SIM);
     launch_sim(P, -1, 0, t0, 1, t0, st);                                   // A, B of the first tick
+    prof_end(c);
     c->launches++;
     for (uint32_t i = 0; i < n_ticks; i++) {
         const int32_t t = t0 + (int32_t)i;
+        prof_begin(c, IM_KERNEL_PLAN);
         if (launch_policy(P, c->Wp, false, c->par_plan, t0, i, c->n_sm, bf16, st)) return fail(c, IM_ERR_BAD_SPEC, "unsupported policy shape");
+        prof_end(c);
         c->par_plan ^= 1;
+        prof_begin(c, IM_KERNEL_EXEC);
         launch_policy(P, c->We, true, c->par_exec, t0, i, c->n_sm, bf16, st);   // C, D: decisions of tick t + critic V[t]
+        prof_end(c);
         c->par_exec ^= 1;
         const bool last = (i + 1 == n_ticks);
+        prof_begin(c, IM_KERNEL_SIM);
         launch_sim(P, t, i, t + 1, last ? 2u : 1u, t0, st);                 // D-issue .. I of tick t, A, B of tick t+1
+        prof_end(c);
         c->launches += 3;
     }
+    prof_begin(c, IM_KERNEL_EXEC);
     launch_policy(P, c->We, true, c->par_exec, t0, n_ticks, c->n_sm, bf16, st);  // bootstrap V[n_ticks] (R30)
+    prof_end(c);
     c->par_exec ^= 1;
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
@@ -407,7 +452,9 @@ int im_returns(im_ctx *c, float gamma, float lambda, float lagrange_mu)
 {
     if (!c) return fail(nullptr, IM_ERR_INVALID_ARG, "ctx is null");
     if (!c->bound || c->last_T == 0) return fail(c, IM_ERR_STATE, "im_returns before im_rollout");
+    prof_begin(c, IM_KERNEL_RETURNS);
     c->launches += launch_returns(c->P, c->last_T, gamma, lambda, lagrange_mu, c->adv, c->ret, c->sums, c->stream);
+    prof_end(c);
     CUDA_TRY(c, cudaGetLastError());
     c->have_returns = true;
     return IM_OK;
@@ -600,10 +647,27 @@ int im_device_ptr(im_ctx *c, uint32_t what, void **dev_ptr, size_t *bytes)
 
 uint64_t im_launch_count(const im_ctx *c) { return c ? c->launches : 0; }
 
+int im_set_profiling(im_ctx *c, int enable)
+{
+    if (!c) return fail(nullptr, IM_ERR_INVALID_ARG, "ctx is null");
+    if (c->bound) { cudaStreamSynchronize(c->stream); prof_collect(c); }
+    c->prof = enable != 0;
+    return IM_OK;
+}
+
+int im_kernel_times(im_ctx *c, double *ms, uint64_t *launches)
+{
+    if (!c || !ms || !launches) return fail(c, IM_ERR_INVALID_ARG, "null argument");
+    if (c->bound) { CUDA_TRY(c, cudaStreamSynchronize(c->stream)); prof_collect(c); }
+    for (int i = 0; i < IM_KERNEL_CLASSES; i++) { ms[i] = c->prof_ms[i]; launches[i] = c->prof_n[i]; c->prof_ms[i] = 0; c->prof_n[i] = 0; }
+    return IM_OK;
+}
+
 void im_destroy(im_ctx *c)
 {
     if (!c) return;
     if (c->bound) cudaStreamSynchronize(c->stream);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     delete c;
 }
 
