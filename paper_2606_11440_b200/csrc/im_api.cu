@@ -19,7 +19,18 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
 int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st);
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st);
 size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP);
-__host__ __device__ size_t sim_warp_smem_bytes(uint32_t RCAP, uint32_t QCAP);
+
+// empty pools: zero the header of every env record, free bitmaps all ones (free slots are defined by the bitmaps)
+__global__ void k_reset(const Params P)
+{
+    const size_t n = (size_t)P.E * P.hdr_words;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const uint32_t e = (uint32_t)(i / P.hdr_words), w = (uint32_t)(i % P.hdr_words);
+        uint32_t v = 0;
+        if ((w >= P.hw_rfree && w < P.hw_rfree + P.RW) || (w >= P.hw_qfree && w < P.hw_qfree + P.QW)) v = 0xFFFFFFFFu;
+        reinterpret_cast<uint32_t *>(env_rec(P, e))[w] = v;
+    }
+}
 
 // repack the R26 blob (device copy) into the kernels' layouts
 __global__ void k_repack(const uint8_t *blob, uint32_t dtype, uint32_t F, uint32_t H, uint32_t n_out, uint32_t n_out_pad,
@@ -205,25 +216,31 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     memset(&P, 0, sizeof P);
     const uint32_t N = s.n_models, Q = s.qcap, R = s.rcap;
     const size_t T1 = (size_t)s.max_ticks + 1;
-    // ---- state (zeroed / re-initialised by im_reset)
+    auto up4 = [](uint32_t w) { return (w + 3u) & ~3u; };
+    // ---- per-env record (im_device.cuh): header words, then the arrays
+    P.RW = R / 32; P.QW = Q / 32;
+    P.hw_rfree = 4 * N; P.hw_qfree = P.hw_rfree + up4(P.RW); P.hw_qready = P.hw_qfree + up4(P.QW);
+    P.hw_misc = P.hw_qready + up4(P.QW); P.hw_ctr = P.hw_misc + 4; P.hdr_words = P.hw_ctr + 32;
+    uint32_t off = (P.hdr_words * 4 + 127u) & ~127u;
+    P.off_iss = off; off += kIssueCap * 16;
+    P.off_hot = off; off += R * 4;
+    P.off_dl = off; off += R * 4;
+    P.off_issue = off; off += R * 4;
+    P.off_tok = off; off += R * 4;
+    P.off_aux = off; off += R * 4;
+    P.off_q = off; off += Q * 16;
+    P.env_stride = (off + 127u) & ~127u;
+    P.env_base = cv.take<uint8_t>((size_t)E * P.env_stride);
+    // ---- control block (zeroed by im_reset)
     cv.off = (cv.off + 255) & ~(size_t)255;
-    const size_t state_off = cv.off;
-    P.r_meta = cv.take<uint32_t>((size_t)E * R); P.r_rs = cv.take<uint32_t>((size_t)E * R); P.r_tok = cv.take<uint32_t>((size_t)E * R);
-    P.r_dl = cv.take<int32_t>((size_t)E * R); P.r_issue = cv.take<int32_t>((size_t)E * R);
-    P.q_plan = cv.take<uint32_t>((size_t)E * Q); P.q_bi = cv.take<uint32_t>((size_t)E * Q); P.q_row = cv.take<uint32_t>((size_t)E * Q);
-    P.q_dl = cv.take<int32_t>((size_t)E * Q); P.q_arr = cv.take<int32_t>((size_t)E * Q);
-    P.q_ready = cv.take<uint32_t>((size_t)E * (Q / 32));
-    P.m_cnt = cv.take<uint4>((size_t)E * N);
-    P.e_hdr = cv.take<uint32_t>(E);
-    P.counters = cv.take<unsigned long long>((size_t)E * 16);
+    const size_t ctl_off = cv.off;
     P.snap = cv.take<float>((size_t)E * 3 * N);
     P.err_flag = cv.take<uint32_t>(64);
     P.exec.cnt = cv.take<uint32_t>(kRegions); P.exec.base = cv.take<uint32_t>(2 * kRegions);
     P.plan.cnt = cv.take<uint32_t>(kRegions); P.plan.base = cv.take<uint32_t>(2 * kRegions);
     P.qlog.cnt = cv.take<uint32_t>(kRegions);
     double *sums = cv.take<double>(8);
-    const size_t state_end = cv.off;
-    P.r_free = cv.take<uint32_t>((size_t)E * (R / 32)); P.q_free = cv.take<uint32_t>((size_t)E * (Q / 32));   // reset to all-ones
+    const size_t ctl_end = cv.off;
     // ---- tables
     P.tab_mult = cv.take<uint32_t>(1024); P.tab_intok = cv.take<uint32_t>(1024);
     P.tab_cdf = cv.take<uint32_t>((size_t)s.n_levels * 32); P.env_level = cv.take<uint8_t>(E);
@@ -237,13 +254,12 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     const uint32_t rce = (uint32_t)((ce + kRegions - 1) / kRegions), rcp = (uint32_t)((cp + kRegions - 1) / kRegions), rcq = (uint32_t)((cq + kRegions - 1) / kRegions);
     P.exec.regcap = rce; P.plan.regcap = rcp; P.qlog.regcap = rcq;
     const size_t ne = (size_t)rce * kRegions, np = (size_t)rcp * kRegions, nq = (size_t)rcq * kRegions;
-    P.exec.env = cv.take<uint32_t>(ne); P.exec.a = cv.take<uint32_t>(ne); P.exec.b = cv.take<float>(ne); P.exec.c = cv.take<uint32_t>(ne);
-    P.exec.logp = cv.take<float>(ne); P.exec.val = cv.take<float>(ne);
-    P.plan.env = cv.take<uint32_t>(np); P.plan.a = cv.take<uint32_t>(np); P.plan.b = cv.take<float>(np); P.plan.c = cv.take<uint32_t>(np);
-    P.plan.logp = cv.take<float>(np); P.plan.val = nullptr;
+    const bool log = s.debug_flags & IM_FLAG_LOG_DECISIONS;
+    P.exec.row = cv.take<uint4>(ne); P.plan.row = cv.take<uint4>(np);
+    if (log) { P.exec.logp = cv.take<float>(ne); P.exec.val = cv.take<float>(ne); P.plan.logp = cv.take<float>(np); }
     P.exec.n_out = 3 * N + 1; P.plan.n_out = 24;
     if (s.debug_flags & IM_FLAG_LOG_LOGITS) { P.exec.logits = cv.take<float>(ne * (3 * N + 1)); P.plan.logits = cv.take<float>(np * 24); }
-    P.qlog.env = cv.take<uint32_t>(nq); P.qlog.arrive = cv.take<uint32_t>(nq); P.qlog.sojourn = cv.take<uint32_t>(nq); P.qlog.info = cv.take<uint32_t>(nq);
+    P.qlog.rec = cv.take<uint4>(nq);
     P.qlog.unorm = cv.take<float>(nq);
     // ---- weights
     const uint32_t F = s.f_in, H = s.hidden;
@@ -263,21 +279,21 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     uint32_t *qorder = cv.take<uint32_t>((size_t)E * (N + 1 + R));
     const size_t total = (cv.off + 255) & ~(size_t)255;
     if (c && base) {
-        P.E = E; P.N = N; P.QCAP = Q; P.RCAP = R; P.QW = Q / 32; P.RW = R / 32;
+        P.E = E; P.N = N; P.QCAP = Q; P.RCAP = R;
         P.sched_mode = s.sched_mode; P.kv_preempt = s.kv_preempt; P.cost_mode = s.cost_mode; P.episode_ticks = s.episode_ticks;
         P.budget_norm = s.budget_norm_ticks; P.in_tok_const = s.in_tok_const; P.mix_thresh = s.mix_thresh; P.env_id_base = s.env_id_base;
         for (int i = 0; i < 2; i++) { P.mix_lo[i] = s.mix_lo[i]; P.mix_hi[i] = s.mix_hi[i]; }
         for (int i = 0; i < 3; i++) P.depth_median[i] = s.depth_median_tok[i];
         P.flags = s.debug_flags; P.has_intok = c->tab_intok.empty() ? 0 : 1;
         P.seed_lo = (uint32_t)c->seed; P.seed_hi = (uint32_t)(c->seed >> 32);
-        P.f_in = F; P.hidden = H; P.log_mode = (s.debug_flags & IM_FLAG_LOG_DECISIONS) ? 1 : 0;
+        P.f_in = F; P.hidden = H; P.log_mode = log ? 1 : 0;
         for (uint32_t k = 0; k < N; k++) {
             const im_model_spec &m = s.model[k];
             P.model[k] = ModelTab{m.rate_tok_s, m.slots, m.kv_cap, m.prefill_us_per_ktok, {m.succ_thresh[0], m.succ_thresh[1], m.succ_thresh[2]}, m.kv_inv};
         }
         c->P = P; c->Wp = W[0]; c->We = W[1]; c->d_blob = d_blob; c->blob_bytes = blob_size(s);
         c->adv = adv; c->ret = ret; c->sums = sums; c->qorder = qorder;
-        c->state_off = state_off; c->state_bytes = state_end - state_off;
+        c->state_off = ctl_off; c->state_bytes = ctl_end - ctl_off;
     }
     return total;
 }
@@ -294,6 +310,18 @@ static int copy_out(im_ctx *c, const void *src, size_t bytes, void *dst, size_t 
     if (!dst) return IM_OK;
     if (cap < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", cap, bytes);
     CUDA_TRY(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return IM_OK;
+}
+
+// E rows of `width` bytes, `pitch` apart on the device, packed densely into dst
+static int copy_out_2d(im_ctx *c, const void *src, size_t pitch, size_t width, size_t rows, void *dst, size_t cap, size_t *written)
+{
+    const size_t bytes = width * rows;
+    if (written) *written = bytes;
+    if (!dst) return IM_OK;
+    if (cap < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", cap, bytes);
+    CUDA_TRY(c, cudaMemcpy2DAsync(dst, width, src, pitch, width, rows, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return IM_OK;
 }
@@ -338,8 +366,9 @@ int im_reset(im_ctx *c)
     if (!c) return fail(nullptr, IM_ERR_INVALID_ARG, "ctx is null");
     if (!c->bound) return fail(c, IM_ERR_STATE, "im_reset before im_bind");
     CUDA_TRY(c, cudaMemsetAsync(c->arena + c->state_off, 0, c->state_bytes, c->stream));
-    CUDA_TRY(c, cudaMemsetAsync(c->P.r_free, 0xFF, (size_t)c->E * c->P.RW * 4, c->stream));
-    CUDA_TRY(c, cudaMemsetAsync(c->P.q_free, 0xFF, (size_t)c->E * c->P.QW * 4, c->stream));
+    k_reset<<<c->n_sm * 8, 256, 0, c->stream>>>(c->P);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
     c->tick = 0; c->last_T = 0; c->have_returns = false; c->par_exec = 0; c->par_plan = 0;
     return IM_OK;
 }
@@ -480,8 +509,8 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
     case IM_TEL_RET:
         if (!c->have_returns) return fail(c, IM_ERR_STATE, "ADV/RET read before im_returns");
         return copy_out(c, what == IM_TEL_ADV ? c->adv : c->ret, 4 * T * E, dst, dst_bytes, written);
-    case IM_TEL_COUNTERS: return copy_out(c, P.counters, 8 * 16 * E, dst, dst_bytes, written);
-    case IM_TEL_SNAPSHOT: return copy_out(c, P.m_cnt, 16 * N * E, dst, dst_bytes, written);
+    case IM_TEL_COUNTERS: return copy_out_2d(c, P.env_base + 4 * (size_t)P.hw_ctr, P.env_stride, 128, E, dst, dst_bytes, written);
+    case IM_TEL_SNAPSHOT: return copy_out_2d(c, P.env_base, P.env_stride, 16 * N, E, dst, dst_bytes, written);
     case IM_TEL_TABLES: {
         const size_t bytes = 4096 + 4096 + c->tab_cdf.size() * 4;
         if (written) *written = bytes;
@@ -535,19 +564,19 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
             if (lg) {
                 CUDA_TRY(c, cudaMemcpy((uint8_t *)dst + k * rec, rb.logits + o * rb.n_out, m * rec, cudaMemcpyDeviceToHost));
             } else {
-                std::vector<uint32_t> env, a, cc, lp, vl;
+                std::vector<uint4> row;
+                std::vector<uint32_t> lp, vl;
                 int rc;
-                if ((rc = fetch(c, env, rb.env + o, m)) || (rc = fetch(c, a, rb.a + o, m)) || (rc = fetch(c, cc, rb.c + o, m)) ||
-                    (rc = fetch(c, lp, (const uint32_t *)rb.logp + o, m)))
-                    return rc;
+                if ((rc = fetch(c, row, rb.row + o, m)) || (rc = fetch(c, lp, (const uint32_t *)rb.logp + o, m))) return rc;
                 if (ex && (rc = fetch(c, vl, (const uint32_t *)rb.val + o, m))) return rc;
                 CUDA_TRY(c, cudaStreamSynchronize(c->stream));
                 uint32_t *out = (uint32_t *)dst + k * 6;
                 for (size_t i = 0; i < m; i++) {
-                    out[i * 6 + 0] = P.env_id_base + env[i];
-                    out[i * 6 + 1] = (uint32_t)(c->last_t0 + (int32_t)(a[i] >> 19));
-                    out[i * 6 + 2] = ex ? ((a[i] & 0x3FFu) | (((a[i] >> 10) & 3u) << 16)) : (a[i] & 0x3FFu);
-                    out[i * 6 + 3] = cc[i] >> 16;
+                    const uint32_t a = row[i].y;
+                    out[i * 6 + 0] = P.env_id_base + row[i].x;
+                    out[i * 6 + 1] = (uint32_t)(c->last_t0 + (int32_t)(a >> 19));
+                    out[i * 6 + 2] = ex ? ((a & 0x3FFu) | (((a >> 10) & 3u) << 16)) : (a & 0x3FFu);
+                    out[i * 6 + 3] = row[i].w >> 16;
                     out[i * 6 + 4] = lp[i];
                     out[i * 6 + 5] = ex ? vl[i] : 0u;
                 }
@@ -571,18 +600,8 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         for (uint32_t r = 0; r < kRegions; r++) {
             const size_t m = cnt[r], o = (size_t)r * P.qlog.regcap;
             if (!m) continue;
-            if (what == IM_TEL_UNORM) {
-                CUDA_TRY(c, cudaMemcpy((float *)dst + k, P.qlog.unorm + o, 4 * m, cudaMemcpyDeviceToHost));
-            } else {
-                std::vector<uint32_t> env, ar, so, inf;
-                int rc;
-                if ((rc = fetch(c, env, P.qlog.env + o, m)) || (rc = fetch(c, ar, P.qlog.arrive + o, m)) || (rc = fetch(c, so, P.qlog.sojourn + o, m)) ||
-                    (rc = fetch(c, inf, P.qlog.info + o, m)))
-                    return rc;
-                CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-                uint32_t *out = (uint32_t *)dst + k * 4;
-                for (size_t i = 0; i < m; i++) { out[i * 4] = env[i]; out[i * 4 + 1] = ar[i]; out[i * 4 + 2] = so[i]; out[i * 4 + 3] = inf[i]; }
-            }
+            if (what == IM_TEL_UNORM) CUDA_TRY(c, cudaMemcpy((float *)dst + k, P.qlog.unorm + o, 4 * m, cudaMemcpyDeviceToHost));
+            else CUDA_TRY(c, cudaMemcpy((uint32_t *)dst + k * 4, P.qlog.rec + o, 16 * m, cudaMemcpyDeviceToHost));
             k += m;
         }
         return IM_OK;
@@ -592,28 +611,28 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         if (written) *written = bytes;
         if (!dst) return IM_OK;
         if (dst_bytes < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, bytes);
-        std::vector<uint32_t> meta, rs, tok, dl, is, qp, qb, qd, qa, mc;
-        int rc;
-        if ((rc = fetch(c, meta, P.r_meta, E * R)) || (rc = fetch(c, rs, P.r_rs, E * R)) || (rc = fetch(c, tok, P.r_tok, E * R)) ||
-            (rc = fetch(c, dl, (const uint32_t *)P.r_dl, E * R)) || (rc = fetch(c, is, (const uint32_t *)P.r_issue, E * R)) ||
-            (rc = fetch(c, qp, P.q_plan, E * Q)) || (rc = fetch(c, qb, P.q_bi, E * Q)) || (rc = fetch(c, qd, (const uint32_t *)P.q_dl, E * Q)) ||
-            (rc = fetch(c, qa, (const uint32_t *)P.q_arr, E * Q)) || (rc = fetch(c, mc, (const uint32_t *)P.m_cnt, E * N * 4)))
-            return rc;
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        std::vector<uint8_t> buf;
+        const size_t batch = 256;
         uint32_t *w = (uint32_t *)dst;
-        for (size_t e = 0; e < E; e++) {
-            memcpy(w, &mc[e * N * 4], 16 * N); w += 4 * N;
-            for (size_t i = 0; i < Q; i++, w += 4) {
-                const uint32_t p = qp[e * Q + i];
-                if (!(p & QP_LIVE)) { w[0] = w[1] = w[2] = w[3] = 0; continue; }
-                const uint32_t succ = ((p >> QP_SUCC_SHIFT) & 7u) ? 1u : 0u;
-                w[0] = (p & 0x1FFFFu) | (succ << 17) | (((p >> QP_ROLE_SHIFT) & 0xFFu) << 18);
-                w[1] = qd[e * Q + i]; w[2] = qa[e * Q + i]; w[3] = qb[e * Q + i];
-            }
-            for (size_t i = 0; i < R; i++, w += 5) {
-                const uint32_t m = meta[e * R + i];
-                if ((m & 3u) == ST_FREE) { w[0] = w[1] = w[2] = w[3] = w[4] = 0; continue; }
-                w[0] = m; w[1] = dl[e * R + i]; w[2] = is[e * R + i]; w[3] = rs[e * R + i]; w[4] = tok[e * R + i];
+        for (size_t e0 = 0; e0 < E; e0 += batch) {
+            const size_t ne = E - e0 < batch ? E - e0 : batch;
+            buf.resize(ne * P.env_stride);
+            CUDA_TRY(c, cudaMemcpy(buf.data(), P.env_base + e0 * P.env_stride, ne * P.env_stride, cudaMemcpyDeviceToHost));
+            for (size_t e = 0; e < ne; e++) {
+                const uint8_t *rec = buf.data() + e * P.env_stride;
+                const uint32_t *hdr = (const uint32_t *)rec, *rfree = hdr + P.hw_rfree, *qfree = hdr + P.hw_qfree;
+                const uint32_t *hot = (const uint32_t *)(rec + P.off_hot), *dl = (const uint32_t *)(rec + P.off_dl), *is = (const uint32_t *)(rec + P.off_issue);
+                const uint32_t *tok = (const uint32_t *)(rec + P.off_tok), *aux = (const uint32_t *)(rec + P.off_aux);
+                const uint4 *qt = (const uint4 *)(rec + P.off_q);
+                memcpy(w, hdr, 16 * N); w += 4 * N;
+                for (size_t i = 0; i < Q; i++, w += 4) {
+                    if ((qfree[i >> 5] >> (i & 31)) & 1u) { w[0] = w[1] = w[2] = w[3] = 0; continue; }
+                    w[0] = qt[i].x; w[1] = qt[i].z; w[2] = qt[i].w; w[3] = qt[i].y;
+                }
+                for (size_t i = 0; i < R; i++, w += 5) {
+                    if ((rfree[i >> 5] >> (i & 31)) & 1u) { w[0] = w[1] = w[2] = w[3] = w[4] = 0; continue; }
+                    w[0] = (aux[i] & ~3u) | ((hot[i] >> HOT_STATE_SHIFT) & 3u); w[1] = dl[i]; w[2] = is[i]; w[3] = hot[i] & 0xFFFFu; w[4] = tok[i];
+                }
             }
         }
         return IM_OK;

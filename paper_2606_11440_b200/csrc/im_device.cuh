@@ -1,6 +1,17 @@
-// im_device.cuh — device-side parameter block and the small defined functions (Philox, im_exp, im_tanh,
-// sampler) of the CUDA path.  Written independently of oracle/ (no shared code); the definitions follow
+// im_device.cuh — device-side parameter block, HBM state layout and the small defined functions (Philox, im_exp,
+// im_tanh) of the CUDA path.  Written independently of oracle/ (no shared code); the definitions follow
 // DESIGN.md readings R2, R3, R23, R24.
+//
+// HBM layout of the environment state: one contiguous record per env,
+//   [ header | issue list | hot[RCAP] | r_dl[RCAP] | r_issue[RCAP] | r_tok[RCAP] | r_aux[RCAP] | q[QCAP] (uint4) ]
+// so that the group of lanes that owns an env streams `header` and `hot[0..hwm)` with 128-bit coalesced loads and
+// touches the cold arrays only for the few requests that change state in a tick.
+//   header (u32 words): m[N] as uint4 {n_wait, n_run, kv_used, ewma_q8} | rfree[RW] | qfree[QW] | qready[QW] |
+//                       misc[4] {drops, icnt, -, -} | counters u64[16]
+//   hot[i]   = remaining(16) | state(2)<<16 | model(4)<<18        — the only per-request word the service phase touches
+//   r_tok[i] = out_total | in_tok<<16 ; r_aux[i] = model<<2 | depth<<6 | agent<<8 | succ<<10 | query<<16
+//   q[i]     = {plan word, budget | in_tok<<16, deadline, arrive}
+// Free slots are defined by the bitmaps (a set bit = free); arrays of free slots hold stale data.
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
@@ -11,12 +22,13 @@ namespace im {
 constexpr uint32_t kMaxModels = 16;
 constexpr uint32_t kRegions = 64;        // row-list / log regions (one atomic counter each), region = env % 64
 constexpr uint32_t kDtUs = 50000;
+constexpr uint32_t kIssueCap = 128;      // issue records per env per tick (31 arrivals x 3 calls + continuing stages)
 
-// request meta word
 constexpr uint32_t ST_FREE = 0, ST_WAIT = 1, ST_RUN = 2;
-// query plan word (device layout): live0 planned1 topo2-3 cnt4-5 keff6-8 stage9-11 nst12-14 pending15-16 succ17-19 roles20-27
+constexpr uint32_t HOT_STATE_SHIFT = 16, HOT_MODEL_SHIFT = 18;
+// query plan word: live0 planned1 topo2-3 cnt4-5 keff6-8 stage9-11 nst12-14 pending15-16 solved17 roles18-25
 constexpr uint32_t QP_LIVE = 1u, QP_PLANNED = 2u;
-constexpr uint32_t QP_PEND_SHIFT = 15, QP_SUCC_SHIFT = 17, QP_ROLE_SHIFT = 20;
+constexpr uint32_t QP_PEND_SHIFT = 15, QP_SUCC_SHIFT = 17, QP_ROLE_SHIFT = 18;
 
 enum Stream : uint32_t { STREAM_ARR = 1, STREAM_QRY = 2, STREAM_PLAN = 3, STREAM_EXEC = 4, STREAM_SVC = 5 };
 enum Counter : uint32_t { C_ARRIVALS, C_DROPPED, C_FINISHED, C_SOLVED, C_MISSED, C_ISSUED, C_CALLS_DONE, C_PREEMPT,
@@ -30,11 +42,11 @@ struct ModelTab {
 };
 
 // a work list that doubles as the decision log: 64 regions, each a ring of `regcap` rows
+//   row = { env (local), a, deadline, in_tok | result<<16 }
+//   a (exec) = q | agent<<10 | topo<<12 | role<<14 | keff<<16 | t_rel<<19 ; a (plan) = q | t_rel<<19
+//   result (exec) = action ; result (plan) = topo | cnt<<2 | roles<<4
 struct RowBuf {
-    uint32_t *env;       // local env index
-    uint32_t *a;         // exec: q | agent<<10 | topo<<12 | role<<14 | keff<<16 | t_rel<<19 ; plan: q | t_rel<<19
-    float *b;            // budget feature b (R15)
-    uint32_t *c;         // in_tok | result<<16 (exec: action; plan: topo|cnt<<2|roles<<4)
+    uint4 *row;
     float *logp;
     float *val;          // exec only
     float *logits;       // optional [rows][n_out]
@@ -45,7 +57,7 @@ struct RowBuf {
 };
 
 struct QLog {
-    uint32_t *env, *arrive, *sojourn, *info;
+    uint4 *rec;          // {env (global), arrive, sojourn, budget | solved<<16 | topo<<17 | keff<<19}
     float *unorm;
     uint32_t *cnt;       // [kRegions]
     uint32_t regcap;
@@ -58,15 +70,11 @@ struct Params {
     uint32_t flags, has_intok, seed_lo, seed_hi;
     uint32_t f_in, hidden, log_mode, pad0;
     ModelTab model[kMaxModels];
-    // env state, SoA: [E][cap], cap index fastest
-    uint32_t *r_meta, *r_rs, *r_tok;
-    int32_t *r_dl, *r_issue;
-    uint32_t *q_plan, *q_bi, *q_row;
-    int32_t *q_dl, *q_arr;
-    uint32_t *r_free, *q_free, *q_ready;     // bitmaps [E][RW] / [E][QW]
-    uint4 *m_cnt;                            // [E][N] {n_wait, n_run, kv_used, ewma_q8}
-    uint32_t *e_hdr;                         // [E] drops carried from phase A to phase I of the same tick
-    unsigned long long *counters;            // [E][16]
+    // per-env record
+    uint8_t *env_base;
+    unsigned long long env_stride;           // bytes, multiple of 128
+    uint32_t hw_rfree, hw_qfree, hw_qready, hw_misc, hw_ctr, hdr_words;   // header word offsets (m at word 0)
+    uint32_t off_iss, off_hot, off_dl, off_issue, off_tok, off_aux, off_q; // byte offsets inside the record
     float *snap;                             // [E][3N] telemetry features of the current tick (R14)
     const uint32_t *tab_mult, *tab_intok, *tab_cdf;
     const uint8_t *env_level;
@@ -83,6 +91,9 @@ struct Weights {          // device copies of one net, prepared by k_repack (im_
     const float *b1, *b2, *b3;           // fp32 biases (b3 padded)
     uint32_t n_out, n_out_pad;
 };
+
+__device__ __forceinline__ uint8_t *env_rec(const Params &P, uint32_t e) { return P.env_base + (size_t)e * P.env_stride; }
+__device__ __forceinline__ uint4 *env_q(const Params &P, uint32_t e) { return reinterpret_cast<uint4 *>(env_rec(P, e) + P.off_q); }
 
 // ------------------------------------------------------------------------------------------------ R2
 struct Ph4 { uint32_t x, y, z, w; };
@@ -132,26 +143,6 @@ __device__ __forceinline__ float im_tanh(float x)
     return copysignf(q, x);
 }
 
-// ----------------------------------------------------------------------------------------------- R24
-// Sequential softmax inverse-CDF over n <= 48 logits read through `get(i)`; returns the action, writes logp.
-template <typename F>
-__device__ __forceinline__ uint32_t sample_head(F get, uint32_t n, float u, float &logp)
-{
-    float m = get(0);
-    for (uint32_t i = 1; i < n; i++) m = fmaxf(m, get(i));
-    float Z = 0.0f;
-    for (uint32_t i = 0; i < n; i++) Z = __fadd_rn(Z, im_exp(__fsub_rn(get(i), m)));
-    const float th = __fmul_rn(u, Z);
-    uint32_t a = n - 1;
-    float c = 0.0f;
-    for (uint32_t i = 0; i < n; i++) {
-        c = __fadd_rn(c, im_exp(__fsub_rn(get(i), m)));
-        if (c > th) { a = i; break; }
-    }
-    logp = __fsub_rn(__fsub_rn(get(a), m), logf(Z));
-    return a;
-}
-
 // ----------------------------------------------------------------------------------------------- R17
 __device__ __forceinline__ uint32_t keff_of(uint32_t topo, uint32_t K) { return topo == 0 ? 1u : (topo == 1 ? K : (K < 2 ? 2u : K)); }
 __device__ __forceinline__ uint32_t nstages_of(uint32_t topo, uint32_t keff) { return topo == 0 ? 1u : (topo == 1 ? keff : 2u); }
@@ -171,6 +162,18 @@ __device__ __forceinline__ uint32_t rows_claim(const Params &P, const RowBuf &rb
     const uint32_t idx = atomicAdd(&rb.cnt[region], n);
     if (P.log_mode && idx + n > rb.regcap) atomicOr(P.err_flag, 1u);
     return idx;
+}
+
+// executor rows of one stage of query q (R17); `pw` is the query's plan word with stage = the stage to dispatch
+__device__ __forceinline__ void write_exec_rows(const Params &P, uint32_t region, uint32_t idx0, uint32_t e, uint32_t q, uint32_t pw,
+                                                uint32_t in_tok, int32_t dl, uint32_t t_rel, uint32_t a0, uint32_t nc)
+{
+    const uint32_t topo = (pw >> 2) & 3u, keff = (pw >> 6) & 7u, roles = (pw >> QP_ROLE_SHIFT) & 0xFFu;
+    for (uint32_t j = 0; j < nc; j++) {
+        const uint32_t agent = a0 + j;
+        const uint32_t a = q | (agent << 10) | (topo << 12) | (((roles >> (2 * agent)) & 3u) << 14) | (keff << 16) | (t_rel << 19);
+        P.exec.row[row_gid(P.exec, region, idx0 + j)] = make_uint4(e, a, (uint32_t)dl, in_tok);
+    }
 }
 
 }  // namespace im

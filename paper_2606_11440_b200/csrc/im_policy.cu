@@ -10,7 +10,7 @@
 
 namespace im {
 
-struct RowInfo { uint32_t env, a, c; float b; uint32_t gidx; bool critic; };
+struct RowInfo { uint32_t env, a, c; int32_t dl; float b; uint32_t gidx; bool critic; };
 
 // ------------------------------------------------------------------------------------------------ tiles
 struct TileSched {
@@ -38,13 +38,14 @@ __device__ __forceinline__ void sched_init(TileSched &S, const RowBuf &rb, uint3
 }
 
 // row `r` of tile `tile`: fills info, returns false if out of range
-__device__ __forceinline__ bool tile_row(const TileSched &S, const RowBuf &rb, uint32_t tile, uint32_t r, uint32_t rows_per_tile,
-                                         uint32_t n_crit, RowInfo &ri)
+template <bool EXEC>
+__device__ __forceinline__ bool tile_row(const Params &P, const TileSched &S, const RowBuf &rb, uint32_t tile, uint32_t r, uint32_t rows_per_tile,
+                                         uint32_t n_crit, int32_t t0, RowInfo &ri)
 {
     if (tile < S.crit_tiles) {
         const uint32_t env = tile * rows_per_tile + r;
         if (env >= n_crit) return false;
-        ri.env = env; ri.a = 0; ri.c = 0; ri.b = 0.0f; ri.gidx = 0; ri.critic = true;
+        ri.env = env; ri.a = 0; ri.c = 0; ri.dl = 0; ri.b = 0.0f; ri.gidx = 0; ri.critic = true;
         return true;
     }
     const uint32_t lt = tile - S.crit_tiles;
@@ -53,7 +54,14 @@ __device__ __forceinline__ bool tile_row(const TileSched &S, const RowBuf &rb, u
     const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * rows_per_tile + r;
     if (idx >= rb.cnt[lo]) return false;
     const uint32_t g = row_gid(rb, lo, idx);
-    ri.env = rb.env[g]; ri.a = rb.a[g]; ri.c = rb.c[g]; ri.b = rb.b[g]; ri.gidx = g; ri.critic = false;
+    const uint4 row = rb.row[g];
+    ri.env = row.x; ri.a = row.y; ri.dl = (int32_t)row.z; ri.c = row.w; ri.gidx = g; ri.critic = false;
+    // budget feature (R15): planner b = budget / norm (the row is created at the arrival tick, deadline - t = budget);
+    // executor b = clamp((deadline - t) / norm, -1, 1) ("normalized remaining budget")
+    const int32_t t = t0 + (int32_t)(row.y >> 19);
+    float b = __fdiv_rn(__int2float_rn(ri.dl - t), __uint2float_rn(P.budget_norm));
+    if (EXEC) b = fminf(fmaxf(b, -1.0f), 1.0f);
+    ri.b = b;
     return true;
 }
 
@@ -90,7 +98,8 @@ __device__ __forceinline__ uint32_t sample_seq(const float *l, float *e, uint32_
     return a;
 }
 
-// executor / critic row: logits[0..3N) + value at 3N
+// executor / critic row: logits[0..3N) + value at 3N.  A decision becomes one issue record of its env (R18): the
+// simulation kernel only has to give it the canonical pool index.
 __device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri, const float *logits, float *scratch,
                                               int32_t t0, uint32_t trow)
 {
@@ -103,9 +112,22 @@ __device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri
     const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
     float logp;
     const uint32_t act = sample_seq(logits, scratch, n, u24(d.x), logp);
-    P.exec.c[ri.gidx] = (ri.c & 0xFFFFu) | (act << 16);
-    P.exec.logp[ri.gidx] = logp;
-    P.exec.val[ri.gidx] = value;
+    if (P.log_mode) {
+        P.exec.row[ri.gidx].w = (ri.c & 0xFFFFu) | (act << 16);
+        P.exec.logp[ri.gidx] = logp;
+        P.exec.val[ri.gidx] = value;
+    }
+    const uint32_t model = act / 3u, depth = act - model * 3u;
+    uint32_t out_total = (uint32_t)(((unsigned long long)P.depth_median[depth] * __ldg(&P.tab_mult[d.y >> 22])) >> 16);
+    out_total = out_total < 1u ? 1u : out_total;
+    const uint32_t succ = d.z < P.model[model].succ[depth] ? 1u : 0u;
+    uint8_t *rec = env_rec(P, ri.env);
+    const uint32_t slot = atomicAdd(reinterpret_cast<uint32_t *>(rec) + P.hw_misc + 1, 1u);
+    if (slot < kIssueCap)
+        reinterpret_cast<uint4 *>(rec + P.off_iss)[slot] =
+            make_uint4(out_total | ((ri.c & 0xFFFFu) << 16), (model << 2) | (depth << 6) | (agent << 8) | (succ << 10) | (q << 16), (uint32_t)ri.dl, 0u);
+    else
+        atomicOr(P.err_flag, 4u);
 }
 
 // planner row: 24 logits = [4 topology | 4 count | 4 agents x 4 roles] (R16); emits the stage-0 executor rows (R17)
@@ -127,26 +149,18 @@ __device__ __forceinline__ void plan_epilogue(const Params &P, const RowInfo &ri
     float lp = __fadd_rn(lp_t, lp_c);
 #pragma unroll
     for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
-    P.plan.c[ri.gidx] = (ri.c & 0xFFFFu) | ((topo | (cnt << 2) | (roles << 4)) << 16);
-    P.plan.logp[ri.gidx] = lp;
-    const size_t qi = (size_t)ri.env * P.QCAP + q;
-    P.q_plan[qi] = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
-    // stage 0 executor rows
+    if (P.log_mode) {
+        P.plan.row[ri.gidx].w = (ri.c & 0xFFFFu) | ((topo | (cnt << 2) | (roles << 4)) << 16);
+        P.plan.logp[ri.gidx] = lp;
+    }
+    // stage 0 executor rows; the plan word records stage = 1, pending = calls of stage 0 (issued in phase D of this tick)
     uint32_t a0, nc;
     stage_calls(topo, keff, 0, a0, nc);
+    const uint32_t pw = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
+    env_q(P, ri.env)[q].x = pw | (1u << 9) | (nc << QP_PEND_SHIFT);
     const uint32_t region = ri.env % kRegions;
     const uint32_t idx0 = rows_claim(P, P.exec, region, nc);
-    P.q_row[qi] = idx0;
-    float b = __fdiv_rn(__int2float_rn(P.q_dl[qi] - t), __uint2float_rn(P.budget_norm));
-    b = fminf(fmaxf(b, -1.0f), 1.0f);
-    for (uint32_t j = 0; j < nc; j++) {
-        const uint32_t agent = a0 + j, g = row_gid(P.exec, region, idx0 + j);
-        P.exec.env[g] = ri.env;
-        P.exec.a[g] = q | (agent << 10) | (topo << 12) | (((roles >> (2 * agent)) & 3u) << 14) | (keff << 16) | (t_rel << 19);
-        P.exec.b[g] = b;
-        P.exec.c[g] = ri.c & 0xFFFFu;
-    }
-    atomicOr(&P.q_ready[(size_t)ri.env * P.QW + (q >> 5)], 1u << (q & 31));
+    write_exec_rows(P, region, idx0, ri.env, q, pw, ri.c & 0xFFFFu, ri.dl, t_rel, a0, nc);
 }
 
 // ================================================================================================ fp32 path (R22)
@@ -180,7 +194,7 @@ k_policy_f32(const Params P, const Weights W, uint32_t parity, int32_t t0, uint3
         bool ok[kF32RowsPerWarp];
 #pragma unroll
         for (int r = 0; r < kF32RowsPerWarp; r++) {
-            ok[r] = tile_row(sched, rb, tile, wib * kF32RowsPerWarp + r, kF32Rows, n_crit, ri[r]);
+            ok[r] = tile_row<EXEC>(P, sched, rb, tile, wib * kF32RowsPerWarp + r, kF32Rows, n_crit, t0, ri[r]);
             for (uint32_t k = lane; k < F; k += 32) x[r * F + k] = ok[r] ? feature(P, EXEC, ri[r], k) : 0.0f;
         }
         __syncwarp();
@@ -322,7 +336,7 @@ k_policy_bf16(const Params P, const Weights W, uint32_t parity, int32_t t0, uint
         __syncthreads();
         if (threadIdx.x < kBfRows) {
             RowInfo ri;
-            const bool ok = tile_row(sched, rb, tile, threadIdx.x, kBfRows, n_crit, ri);
+            const bool ok = tile_row<EXEC>(P, sched, rb, tile, threadIdx.x, kBfRows, n_crit, t0, ri);
             s_ri[threadIdx.x] = ri; s_ok[threadIdx.x] = ok;
         }
         __syncthreads();

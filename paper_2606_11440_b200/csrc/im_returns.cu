@@ -69,9 +69,10 @@ k_utility(const QLog ql, float mu, double *__restrict__ sums)
     double su = 0.0, su2 = 0.0, cn = 0.0;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const size_t g = (size_t)region * ql.regcap + i;
-        const uint32_t info = ql.info[g];
+        const uint4 rec = ql.rec[g];
+        const uint32_t info = rec.w;
         const float U = __fsub_rn(__uint2float_rn((info >> 16) & 1u),
-                                  __fdiv_rn(__fmul_rn(mu, __uint2float_rn(ql.sojourn[g])), __uint2float_rn(info & 0xFFFFu)));
+                                  __fdiv_rn(__fmul_rn(mu, __uint2float_rn(rec.z)), __uint2float_rn(info & 0xFFFFu)));
         ql.unorm[g] = U;
         su += (double)U; su2 += (double)U * (double)U; cn += 1.0;
     }
@@ -133,14 +134,15 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
     uint32_t n2cap = 32;
     while (n2cap < P.RCAP) n2cap <<= 1;
     unsigned long long *keys = s_keys + (size_t)wib * n2cap;
-    const uint32_t *r_meta = P.r_meta + (size_t)e * P.RCAP;
-    const int32_t *r_dl = P.r_dl + (size_t)e * P.RCAP, *r_issue = P.r_issue + (size_t)e * P.RCAP;
+    const uint8_t *rec = env_rec(P, e);
+    const uint32_t *hot = (const uint32_t *)(rec + P.off_hot), *rfree = (const uint32_t *)rec + P.hw_rfree;
+    const int32_t *r_dl = (const int32_t *)(rec + P.off_dl), *r_issue = (const int32_t *)(rec + P.off_issue);
     uint32_t n = 0;
     uint32_t per_model = 0;                       // lane k counts model k
     for (uint32_t i0 = 0; i0 < P.RCAP; i0 += 32) {
         const uint32_t i = i0 + lane;
-        const uint32_t m = r_meta[i];
-        const bool w = (m & 3u) == ST_WAIT;
+        const uint32_t m = hot[i] >> HOT_STATE_SHIFT;          // state | model << 2 (stale words of free slots are masked)
+        const bool w = (m & 3u) == ST_WAIT && !((rfree[i >> 5] >> (i & 31)) & 1u);
         const uint32_t bal = __ballot_sync(0xffffffffu, w);
         if (w) {
             const int32_t base = P.sched_mode ? r_dl[i] : r_issue[i];

@@ -65,7 +65,9 @@ def compare_chunk(gpu, orc, env_ids, n_ticks, blob, bf16: bool, stats: dict, che
         assert np.array_equal(gv, ov), "critic values differ (fp32 contract is bit-exact)"
     gc, oc = gpu.counters()[cols], orc.counters()
     oc[:, 14] = 0
-    assert np.array_equal(gc, oc), "counters differ"
+    if not np.array_equal(gc, oc):
+        bad = np.argwhere(gc != oc)
+        raise AssertionError(f"counters differ at (env_col, counter) {bad[:8].tolist()}: gpu {gc[gc != oc][:8].tolist()} oracle {oc[gc != oc][:8].tolist()}")
     if check_state:
         gs = gpu.state()[cols]
         os_ = orc.state()
