@@ -1,0 +1,253 @@
+// im_tc.cuh — sm_100a tensor-core building blocks of the bf16 policy path (reading R25):
+// inline-PTX wrappers for tcgen05 (TMEM allocation, UMMA issue, TMEM load/store, commit) and mbarrier, the shared
+// memory operand layout, and the three-layer MLP of one 128-row tile.
+//
+// Operand layout ("canonical K-major, no swizzle"): a [rows][K] bf16 matrix is stored as 16-byte chunks of 8
+// consecutive k, chunk-major:  byte offset(r, k) = (k / 8) * rows * 16 + r * 16 + (k % 8) * 2.
+// A core matrix (8 rows x 16 bytes) is then 128 contiguous bytes; in the UMMA shared-memory descriptor the stride
+// between 8-row groups (SBO) is 128 B and the stride between k-chunks (LBO) is rows * 16 B.
+//
+// Tile data flow (M = 128 rows = 128 TMEM lanes, one thread per row in the epilogues):
+//   A1 (features, smem) x W1 -> D1 (TMEM cols [0,H))        SS-mode UMMA, K1 / 16 instructions of N = H
+//   tanh(D1 + b1) -> bf16, packed two per column in place    TMEM cols [0,H/2)        (tcgen05.ld / tcgen05.st)
+//   A2 (TMEM) x W2 -> D2 (TMEM cols [H,2H))                  TS-mode UMMA, H / 16 instructions
+//   tanh(D2 + b2) -> bf16 in place                           TMEM cols [H,H+H/2)
+//   A3 (TMEM) x W3 -> D3 (TMEM cols [0,NO))                  TS-mode UMMA, N = NO
+//   logits = D3 + b3 -> registers of the row's thread
+// The hidden activations never touch shared memory: all three weight matrices stay resident in it instead.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace im {
+namespace tc {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// ---------------------------------------------------------------------------------------------- mbarrier
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "LAB_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra DONE;\n\t"
+        "bra LAB_WAIT;\n\t"
+        "DONE:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- fences
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// ---------------------------------------------------------------------------------------------- TMEM
+// one full warp allocates `cols` (power of two >= 32) columns; the base address lands in *slot (shared memory)
+__device__ __forceinline__ void tmem_alloc(uint32_t *slot, uint32_t cols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t base, uint32_t cols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(cols) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- descriptors
+// shared-memory matrix descriptor, K-major, SWIZZLE_NONE, version 1 (sm_100)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
+}
+// instruction descriptor of kind::f16: D fp32, A and B bf16, both K-major, dense
+__host__ __device__ constexpr uint32_t instr_desc_bf16(uint32_t M, uint32_t N)
+{
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((N >> 3) << 17) | ((M >> 4) << 24);
+}
+
+// D[tmem] (+)= A[smem] * B[smem]^T — issued by ONE thread
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]^T
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// all UMMAs issued so far by this thread arrive on `bar` when they complete (implies fence::before_thread_sync)
+__device__ __forceinline__ void umma_commit(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- TMEM <-> registers
+// warp-collective: lane i of the warp reads 32 consecutive columns of TMEM lane (taddr.lane + i)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
+          "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
+          "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
+        "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+
+__device__ __forceinline__ float tanh_approx(float x)
+{
+    float y;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
+{
+    const __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t *>(&p);
+}
+
+// byte offset of element (r, k) of a [rows][K] bf16 operand in the canonical layout
+__host__ __device__ constexpr uint32_t canon_off(uint32_t rows, uint32_t r, uint32_t k) { return (k >> 3) * rows * 16u + r * 16u + (k & 7u) * 2u; }
+
+
+// ---------------------------------------------------------------------------------------------- the MLP of one tile
+// Shared-memory image of one net (built once by k_pack_tc, copied verbatim by every CTA):
+//   [ W1 canon [H][K1] | W2 canon [H][H] | W3 canon [NO][H] | b1[H] b2[H] b3[NO] fp32 ]
+template <int K1, int H, int NO>
+struct TcMlp {
+    static_assert(K1 % 16 == 0 && H % 32 == 0 && NO % 16 == 0 && NO <= 64 && H <= 256, "shape");
+    static constexpr uint32_t kW1 = 0, kW2 = kW1 + H * K1 * 2, kW3 = kW2 + H * H * 2, kBias = kW3 + NO * H * 2;
+    static constexpr uint32_t kImageBytes = kBias + (2 * H + NO) * 4;
+    static constexpr uint32_t kA1Bytes = 128 * K1 * 2;
+    static constexpr uint32_t kTmemCols = 2 * H;                 // 512 for H = 256, 256 for H = 128 (powers of two)
+
+    // tanh(D + bias) of TMEM columns [col0, col0+H) -> bf16 pairs packed in place into [col0, col0+H/2).
+    // `tlane` = TMEM address of this warp's lane quarter at column 0 of the allocation.
+    static __device__ __forceinline__ void hidden_epilogue(uint32_t tlane, uint32_t col0, const float *bias)
+    {
+#pragma unroll 1
+        for (int j = 0; j < H / 32; j++) {
+            uint32_t v[32], o[16];
+            tmem_ld32(tlane + col0 + 32 * j, v);
+            tc_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 16; i++) {
+                const float2 b = *reinterpret_cast<const float2 *>(bias + 32 * j + 2 * i);
+                o[i] = pack_bf16(tanh_approx(__uint_as_float(v[2 * i]) + b.x), tanh_approx(__uint_as_float(v[2 * i + 1]) + b.y));
+            }
+            tmem_st16(tlane + col0 + 16 * j, o);   // in place: columns [16j,16j+16) lie below every column still to be read
+        }
+        tc_wait_st();
+    }
+
+    // Runs the three layers for the 128 rows whose features sit in `a1` (canonical [128][K1], written by the generic
+    // proxy).  All 128 threads call it; on return `logit[i]` = D3[row = threadIdx.x][i] + b3[i].  `phase` is the mbarrier
+    // parity, flipped three times.
+    static __device__ __forceinline__ void run(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar,
+                                               uint32_t &phase, float (&logit)[NO])
+    {
+        const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
+        const float *bias = reinterpret_cast<const float *>(image + kBias);
+        constexpr uint32_t idescH = instr_desc_bf16(128, H), idescO = instr_desc_bf16(128, NO);
+        // ---- layer 1 (SS)
+        fence_proxy_async_smem();
+        tc_fence_before();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            tc_fence_after();
+            const uint32_t sa = smem_u32(a1), sb = smem_u32(image + kW1);
+#pragma unroll
+            for (int k = 0; k < K1 / 16; k++)
+                umma_ss(tmem_base, smem_desc(sa + k * 2 * 128 * 16, 128 * 16, 128), smem_desc(sb + k * 2 * H * 16, H * 16, 128), idescH, k > 0);
+            umma_commit(bar);
+        }
+        mbar_wait(bar, phase); phase ^= 1u;
+        tc_fence_after();
+        hidden_epilogue(tlane, 0, bias);
+        // ---- layer 2 (TS): A2 = TMEM cols [0, H/2), D2 = cols [H, 2H)
+        tc_fence_before();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            tc_fence_after();
+            const uint32_t sb = smem_u32(image + kW2);
+#pragma unroll
+            for (int k = 0; k < H / 16; k++)
+                umma_ts(tmem_base + H, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16, H * 16, 128), idescH, k > 0);
+            umma_commit(bar);
+        }
+        mbar_wait(bar, phase); phase ^= 1u;
+        tc_fence_after();
+        hidden_epilogue(tlane, H, bias + H);
+        // ---- layer 3 (TS): A3 = TMEM cols [H, H + H/2), D3 = cols [0, NO)
+        tc_fence_before();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            tc_fence_after();
+            const uint32_t sb = smem_u32(image + kW3);
+#pragma unroll
+            for (int k = 0; k < H / 16; k++)
+                umma_ts(tmem_base, tmem_base + H + 8 * k, smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), idescO, k > 0);
+            umma_commit(bar);
+        }
+        mbar_wait(bar, phase); phase ^= 1u;
+        tc_fence_after();
+#pragma unroll
+        for (int j = 0; j < NO / 16; j++) {
+            uint32_t v[16];
+            tmem_ld16(tlane + 16 * j, v);
+            tc_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 16; i++) logit[16 * j + i] = __uint_as_float(v[i]) + bias[2 * H + 16 * j + i];
+        }
+        tc_fence_before();       // the next tile's layer-1 UMMA overwrites D3's columns: order these loads before it
+    }
+};
+
+}  // namespace tc
+}  // namespace im
