@@ -19,6 +19,9 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
 int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st);
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st);
 size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP);
+bool tc_supported(uint32_t F, uint32_t H);
+size_t tc_image_bytes(bool exec);
+void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t st);
 
 // empty pools: zero the header of every env record, free bitmaps all ones (free slots are defined by the bitmaps)
 __global__ void k_reset(const Params P)
@@ -274,6 +277,7 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
             w.W1 = cv.take<__nv_bfloat16>((size_t)F * H); w.W2 = cv.take<__nv_bfloat16>((size_t)H * H); w.W3 = cv.take<__nv_bfloat16>((size_t)H * w.n_out_pad);
         }
         w.b1 = cv.take<float>(H); w.b2 = cv.take<float>(H); w.b3 = cv.take<float>(w.n_out_pad);
+        if (s.policy_dtype == IM_DTYPE_BF16 && tc_supported(F, H)) w.tc_img = cv.take<uint8_t>(tc_image_bytes(net == 1));
     }
     uint8_t *d_blob = cv.take<uint8_t>(blob_size(s));
     uint32_t *qorder = cv.take<uint32_t>((size_t)E * (N + 1 + R));
@@ -424,6 +428,7 @@ static int upload_weights(im_ctx *c, const void *blob)
                                             (float *)w.W1t, (float *)w.W2t, (float *)w.W3t, (__nv_bfloat16 *)w.W1, (__nv_bfloat16 *)w.W2,
                                             (__nv_bfloat16 *)w.W3, (float *)w.b1, (float *)w.b2, (float *)w.b3);
         c->launches++;
+        if (w.tc_img) { launch_pack_tc(w, net == 1, c->spec.n_models, c->stream); c->launches++; }
     }
     CUDA_TRY(c, cudaGetLastError());
     return IM_OK;

@@ -6,6 +6,7 @@
 //   bf16 (R25): bf16 operands, fp32 accumulation on the tensor cores (mma.sync m16n8k16 in this version),
 //               tanh.approx, fp32 logits; sampling by the exact R24 sampler on those logits.
 #include "im_device.cuh"
+#include "im_tc.cuh"
 #include <cuda_bf16.h>
 
 namespace im {
@@ -98,20 +99,11 @@ __device__ __forceinline__ uint32_t sample_seq(const float *l, float *e, uint32_
     return a;
 }
 
-// executor / critic row: logits[0..3N) + value at 3N.  A decision becomes one issue record of its env (R18): the
-// simulation kernel only has to give it the canonical pool index.
-__device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri, const float *logits, float *scratch,
-                                              int32_t t0, uint32_t trow)
+// executor decision -> log row + one issue record of its env (R18): the simulation kernel only has to give the
+// request its canonical pool index.
+__device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, const Ph4 &d, uint32_t act, float logp, float value)
 {
-    const uint32_t n = 3 * P.N;
-    const float value = logits[n];
-    if (ri.critic) { P.val[(size_t)trow * P.E + ri.env] = value; return; }
     const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
-    const int32_t t = t0 + (int32_t)(ri.a >> 19);
-    if (P.exec.logits) for (uint32_t i = 0; i <= n; i++) P.exec.logits[(size_t)ri.gidx * P.exec.n_out + i] = logits[i];
-    const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
-    float logp;
-    const uint32_t act = sample_seq(logits, scratch, n, u24(d.x), logp);
     if (P.log_mode) {
         P.exec.row[ri.gidx].w = (ri.c & 0xFFFFu) | (act << 16);
         P.exec.logp[ri.gidx] = logp;
@@ -130,7 +122,42 @@ __device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri
         atomicOr(P.err_flag, 4u);
 }
 
-// planner row: 24 logits = [4 topology | 4 count | 4 agents x 4 roles] (R16); emits the stage-0 executor rows (R17)
+// executor / critic row: logits[0..3N) + value at 3N (shared-memory logits, sequential R24 sampler)
+__device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri, const float *logits, float *scratch,
+                                              int32_t t0, uint32_t trow)
+{
+    const uint32_t n = 3 * P.N;
+    const float value = logits[n];
+    if (ri.critic) { P.val[(size_t)trow * P.E + ri.env] = value; return; }
+    const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
+    const int32_t t = t0 + (int32_t)(ri.a >> 19);
+    if (P.exec.logits) for (uint32_t i = 0; i <= n; i++) P.exec.logits[(size_t)ri.gidx * P.exec.n_out + i] = logits[i];
+    const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
+    float logp;
+    const uint32_t act = sample_seq(logits, scratch, n, u24(d.x), logp);
+    exec_commit(P, ri, d, act, logp, value);
+}
+
+// planner decision -> log row, plan word of the query and the stage-0 executor rows (R17)
+__device__ __forceinline__ void plan_commit(const Params &P, const RowInfo &ri, uint32_t topo, uint32_t cnt, uint32_t roles, float lp)
+{
+    const uint32_t q = ri.a & 0x3FFu, t_rel = ri.a >> 19;
+    const uint32_t keff = keff_of(topo, cnt + 1), nst = nstages_of(topo, keff);
+    if (P.log_mode) {
+        P.plan.row[ri.gidx].w = (ri.c & 0xFFFFu) | ((topo | (cnt << 2) | (roles << 4)) << 16);
+        P.plan.logp[ri.gidx] = lp;
+    }
+    // stage 0 executor rows; the plan word records stage = 1, pending = calls of stage 0 (issued in phase D of this tick)
+    uint32_t a0, nc;
+    stage_calls(topo, keff, 0, a0, nc);
+    const uint32_t pw = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
+    env_q(P, ri.env)[q].x = pw | (1u << 9) | (nc << QP_PEND_SHIFT);
+    const uint32_t region = ri.env % kRegions;
+    const uint32_t idx0 = rows_claim(P, P.exec, region, nc);
+    write_exec_rows(P, region, idx0, ri.env, q, pw, ri.c & 0xFFFFu, ri.dl, t_rel, a0, nc);
+}
+
+// planner row: 24 logits = [4 topology | 4 count | 4 agents x 4 roles] (R16)
 __device__ __forceinline__ void plan_epilogue(const Params &P, const RowInfo &ri, const float *logits, float *scratch, int32_t t0)
 {
     const uint32_t q = ri.a & 0x3FFu, t_rel = ri.a >> 19;
@@ -145,22 +172,11 @@ __device__ __forceinline__ void plan_epilogue(const Params &P, const RowInfo &ri
     uint32_t roles = 0;
 #pragma unroll
     for (uint32_t a = 0; a < 4; a++) roles |= sample_seq(logits + 8 + 4 * a, scratch, 4, u24(ur[a]), lp_r[a]) << (2 * a);
-    const uint32_t keff = keff_of(topo, cnt + 1), nst = nstages_of(topo, keff);
+    const uint32_t keff = keff_of(topo, cnt + 1);
     float lp = __fadd_rn(lp_t, lp_c);
 #pragma unroll
     for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
-    if (P.log_mode) {
-        P.plan.row[ri.gidx].w = (ri.c & 0xFFFFu) | ((topo | (cnt << 2) | (roles << 4)) << 16);
-        P.plan.logp[ri.gidx] = lp;
-    }
-    // stage 0 executor rows; the plan word records stage = 1, pending = calls of stage 0 (issued in phase D of this tick)
-    uint32_t a0, nc;
-    stage_calls(topo, keff, 0, a0, nc);
-    const uint32_t pw = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
-    env_q(P, ri.env)[q].x = pw | (1u << 9) | (nc << QP_PEND_SHIFT);
-    const uint32_t region = ri.env % kRegions;
-    const uint32_t idx0 = rows_claim(P, P.exec, region, nc);
-    write_exec_rows(P, region, idx0, ri.env, q, pw, ri.c & 0xFFFFu, ri.dl, t_rel, a0, nc);
+    plan_commit(P, ri, topo, cnt, roles, lp);
 }
 
 // ================================================================================================ fp32 path (R22)
@@ -414,6 +430,249 @@ k_policy_bf16(const Params P, const Weights W, uint32_t parity, int32_t t0, uint
 template <int F, int H>
 static size_t bf16_smem_bytes() { return 2ull * kBfRows * (H + 8) * 2; }
 
+// ================================================================================================ tcgen05 path (R25)
+// F = 128, H = 256 (configs 4-5): a real dense GEMM, so it runs on the 5th-generation tensor cores (im_tc.cuh).
+// One persistent CTA per SM; the whole net (192 KB of bf16 weights) stays in shared memory for the lifetime of the
+// launch; a tile is 128 rows = 128 TMEM lanes = 128 threads, thread r owning row r from feature gather to sampling.
+// Layer 1 contracts only the first 64 features: rows are zero beyond 3N + 12 <= 60 (R15), so this is exact.
+constexpr int kTcK1 = 64, kTcH = 256, kTcThreads = 128;
+template <bool EXEC> using TcNet = tc::TcMlp<kTcK1, kTcH, EXEC ? 64 : 32>;
+
+bool tc_supported(uint32_t F, uint32_t H) { return F == 128 && H == 256; }
+size_t tc_image_bytes(bool exec) { return exec ? TcNet<true>::kImageBytes : TcNet<false>::kImageBytes; }
+
+// K order of layer 1 on this path: [snap(3N) | b | in_tok | topo(4) | role(4) | agent | keff | 0...] — the R15 features with
+// the budget feature moved behind the snapshot block, so that a row's snapshot floats land on 16-byte chunk boundaries.
+// fp32 accumulation order is unspecified under R25, so permuting k is free; W1's columns are permuted to match.
+__device__ __forceinline__ uint32_t tc_feature_src(uint32_t kp, uint32_t N3) { return kp < N3 ? kp + 1u : (kp == N3 ? 0u : kp); }
+
+// bf16 [o][k] row-major weights + fp32 biases (k_repack's output) -> the shared-memory image of im_tc.cuh
+template <bool EXEC>
+__global__ void k_pack_tc(const Weights W, uint32_t N3)
+{
+    using Net = TcNet<EXEC>;
+    constexpr uint32_t NO = EXEC ? 64 : 32, F = 128;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    uint8_t *img = W.tc_img;
+    for (uint32_t i = tid; i < kTcH * kTcK1; i += nth) {
+        const uint32_t o = i / kTcK1, kp = i % kTcK1;
+        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW1 + tc::canon_off(kTcH, o, kp)) = W.W1[o * F + tc_feature_src(kp, N3)];
+    }
+    for (uint32_t i = tid; i < kTcH * kTcH; i += nth) {
+        const uint32_t o = i / kTcH, k = i % kTcH;
+        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW2 + tc::canon_off(kTcH, o, k)) = W.W2[i];
+    }
+    for (uint32_t i = tid; i < NO * kTcH; i += nth) {
+        const uint32_t o = i / kTcH, k = i % kTcH;
+        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW3 + tc::canon_off(NO, o, k)) = o < W.n_out_pad ? W.W3[i] : __float2bfloat16(0.0f);
+    }
+    float *bias = reinterpret_cast<float *>(img + Net::kBias);
+    for (uint32_t i = tid; i < kTcH; i += nth) { bias[i] = W.b1[i]; bias[kTcH + i] = W.b2[i]; }
+    for (uint32_t i = tid; i < NO; i += nth) bias[2 * kTcH + i] = i < W.n_out_pad ? W.b3[i] : 0.0f;
+}
+
+void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t st)
+{
+    if (exec) k_pack_tc<true><<<64, 256, 0, st>>>(W, 3 * n_models);
+    else k_pack_tc<false><<<64, 256, 0, st>>>(W, 3 * n_models);
+}
+
+// R24 sampler on logits held in registers: l[off .. off+n), n <= NMAX.  Same operation sequence as sample_seq.
+template <int NMAX, int NO>
+__device__ __forceinline__ uint32_t sample_reg(const float (&l)[NO], int off, uint32_t n, float u, float &logp)
+{
+    float m = l[off];
+#pragma unroll
+    for (int i = 1; i < NMAX; i++) if ((uint32_t)i < n) m = fmaxf(m, l[off + i]);
+    float e[NMAX];
+#pragma unroll
+    for (int i = 0; i < NMAX; i++) e[i] = im_exp(__fsub_rn(l[off + i], m));
+    float Z = 0.0f;
+#pragma unroll
+    for (int i = 0; i < NMAX; i++) if ((uint32_t)i < n) Z = __fadd_rn(Z, e[i]);
+    const float th = __fmul_rn(u, Z);
+    uint32_t a = n - 1;
+    float la = l[off], c = 0.0f;
+    bool found = false;
+#pragma unroll
+    for (int i = 0; i < NMAX; i++) {
+        if ((uint32_t)i < n) {
+            c = __fadd_rn(c, e[i]);
+            const bool hit = !found && c > th;
+            if (hit || (!found && (uint32_t)i == n - 1)) { a = (uint32_t)i; la = l[off + i]; }
+            found = found || hit;
+        }
+    }
+    logp = __fsub_rn(__fsub_rn(la, m), logf(Z));
+    return a;
+}
+
+struct TcRaw { uint4 row; uint32_t env, gidx; bool ok, critic; };
+
+// row `r` of tile `tile`: issues the row load, decodes nothing (the consumer decodes after the latency has passed)
+__device__ __forceinline__ TcRaw tc_fetch_row(const TileSched &S, const RowBuf &rb, uint32_t tile, uint32_t r, uint32_t n_crit)
+{
+    TcRaw x;
+    x.row = make_uint4(0, 0, 0, 0); x.env = 0; x.gidx = 0; x.ok = false; x.critic = false;
+    if (tile >= S.total) return x;
+    if (tile < S.crit_tiles) {
+        const uint32_t env = tile * kTcThreads + r;
+        x.ok = env < n_crit; x.critic = true; x.env = env;
+        return x;
+    }
+    const uint32_t lt = tile - S.crit_tiles;
+    uint32_t lo = 0, hi = kRegions;
+    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
+    const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * kTcThreads + r;
+    if (idx >= rb.cnt[lo]) return x;
+    x.gidx = row_gid(rb, lo, idx);
+    x.row = rb.row[x.gidx];
+    x.ok = true;
+    return x;
+}
+
+template <bool EXEC>
+__device__ __forceinline__ RowInfo tc_decode_row(const Params &P, const TcRaw &x, int32_t t0)
+{
+    RowInfo ri;
+    ri.critic = x.critic; ri.gidx = x.gidx;
+    if (x.critic) { ri.env = x.env; ri.a = 0; ri.c = 0; ri.dl = 0; ri.b = 0.0f; return ri; }
+    ri.env = x.row.x; ri.a = x.row.y; ri.dl = (int32_t)x.row.z; ri.c = x.row.w;
+    const int32_t t = t0 + (int32_t)(x.row.y >> 19);
+    float b = __fdiv_rn(__int2float_rn(ri.dl - t), __uint2float_rn(P.budget_norm));
+    if (EXEC) b = fminf(fmaxf(b, -1.0f), 1.0f);
+    ri.b = b;
+    return ri;
+}
+
+template <bool EXEC>
+__global__ void __launch_bounds__(kTcThreads, 1)
+k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32_t trow)
+{
+    using Net = TcNet<EXEC>;
+    constexpr int NO = EXEC ? 64 : 32;
+    extern __shared__ __align__(1024) uint8_t smem_tc[];
+    __shared__ TileSched sched;
+    __shared__ uint64_t bar;
+    __shared__ uint32_t tmem_slot;
+    uint8_t *img = smem_tc, *a1 = smem_tc + ((Net::kImageBytes + 1023u) & ~1023u);
+    {
+        const uint4 *src = reinterpret_cast<const uint4 *>(W.tc_img);
+        uint4 *dst = reinterpret_cast<uint4 *>(img);
+        for (uint32_t i = threadIdx.x; i < Net::kImageBytes / 16; i += kTcThreads) dst[i] = __ldg(src + i);
+    }
+    if (threadIdx.x == 0) { tc::mbar_init(&bar, 1); tc::mbar_fence_init(); }
+    if (threadIdx.x < 32) tc::tmem_alloc(&tmem_slot, Net::kTmemCols);
+    const RowBuf &rb = EXEC ? P.exec : P.plan;
+    const uint32_t n_crit = EXEC ? P.E : 0u;
+    sched_init(sched, rb, parity, kTcThreads, n_crit);
+    tc::tc_fence_before();
+    __syncthreads();
+    tc::tc_fence_after();
+    const uint32_t tmem_base = tmem_slot;
+    const uint32_t N3 = 3 * P.N;
+    const bool vec = (N3 % 8u) == 0;                      // snapshot block = whole 16-byte chunks (N = 8, 16)
+    uint32_t phase = 0;
+
+    // snapshot floats of a row's env (R14): up to 12 float4 per thread, issued early, consumed one tile later
+    auto fetch_snap = [&](const TcRaw &x, float4 (&sn)[12]) {
+        const uint32_t env = x.critic ? x.env : x.row.x;
+        const float4 *src = reinterpret_cast<const float4 *>(P.snap + (size_t)env * N3);
+#pragma unroll
+        for (int j = 0; j < 12; j++) sn[j] = (x.ok && vec && (uint32_t)(4 * j) < N3) ? __ldg(src + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+    };
+
+    TcRaw cur = tc_fetch_row(sched, rb, blockIdx.x, threadIdx.x, n_crit);
+    float4 sn[12];
+    fetch_snap(cur, sn);
+    for (uint32_t tile = blockIdx.x; tile < sched.total; tile += gridDim.x) {
+        const RowInfo ri = tc_decode_row<EXEC>(P, cur, t0);
+        const bool ok = cur.ok;
+        // ---- features -> A1 (bf16 RNE), canonical layout: chunk c of row r at c * 2048 + r * 16
+        if (vec) {
+            float tl[16];                                 // the 12 features behind the snapshot block, then zeros
+#pragma unroll
+            for (int j = 0; j < 16; j++) tl[j] = (ok && j < 12) ? feature(P, EXEC, ri, j == 0 ? 0u : N3 + (uint32_t)j) : 0.0f;
+            const uint32_t c0 = N3 / 8;
+#pragma unroll
+            for (int c = 0; c < kTcK1 / 8; c++) {
+                float f[8];
+                if ((uint32_t)c < c0) {
+                    f[0] = sn[2 * c].x; f[1] = sn[2 * c].y; f[2] = sn[2 * c].z; f[3] = sn[2 * c].w;
+                    f[4] = sn[2 * c + 1].x; f[5] = sn[2 * c + 1].y; f[6] = sn[2 * c + 1].z; f[7] = sn[2 * c + 1].w;
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 8; j++) f[j] = (uint32_t)c == c0 ? tl[j] : ((uint32_t)c == c0 + 1 ? tl[8 + j] : 0.0f);
+                }
+                *reinterpret_cast<uint4 *>(a1 + c * (128 * 16) + threadIdx.x * 16) =
+                    make_uint4(tc::pack_bf16(f[0], f[1]), tc::pack_bf16(f[2], f[3]), tc::pack_bf16(f[4], f[5]), tc::pack_bf16(f[6], f[7]));
+            }
+        } else {
+#pragma unroll 1
+            for (int c = 0; c < kTcK1 / 8; c++) {
+                float f[8];
+#pragma unroll
+                for (int j = 0; j < 8; j++) f[j] = ok ? feature(P, EXEC, ri, tc_feature_src(8 * c + j, N3)) : 0.0f;
+                *reinterpret_cast<uint4 *>(a1 + c * (128 * 16) + threadIdx.x * 16) =
+                    make_uint4(tc::pack_bf16(f[0], f[1]), tc::pack_bf16(f[2], f[3]), tc::pack_bf16(f[4], f[5]), tc::pack_bf16(f[6], f[7]));
+            }
+        }
+        // ---- next tile's row: the load flies while the tensor cores work on this tile
+        const TcRaw nxt = tc_fetch_row(sched, rb, tile + gridDim.x, threadIdx.x, n_crit);
+        float l[NO];
+        Net::run(img, a1, tmem_base, &bar, phase, l);
+        fetch_snap(nxt, sn);                              // consumed at the top of the next iteration
+        // ---- epilogue of row `ri`: logits in registers
+        if (ok) {
+            if (EXEC) {
+                const uint32_t n = N3;
+                float value = 0.0f;
+#pragma unroll
+                for (int i = 0; i < NO; i++) if ((uint32_t)i == n) value = l[i];
+                if (ri.critic) {
+                    P.val[(size_t)trow * P.E + ri.env] = value;
+                } else {
+                    if (P.exec.logits) {
+#pragma unroll
+                        for (int i = 0; i < NO; i++) if ((uint32_t)i <= n) P.exec.logits[(size_t)ri.gidx * P.exec.n_out + i] = l[i];
+                    }
+                    const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
+                    const int32_t t = t0 + (int32_t)(ri.a >> 19);
+                    const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
+                    float logp;
+                    const uint32_t act = sample_reg<48, NO>(l, 0, n, u24(d.x), logp);
+                    exec_commit(P, ri, d, act, logp, value);
+                }
+            } else {
+                if (P.plan.logits) {
+#pragma unroll
+                    for (int i = 0; i < 24; i++) P.plan.logits[(size_t)ri.gidx * 24 + i] = l[i];
+                }
+                const uint32_t q = ri.a & 0x3FFu;
+                const int32_t t = t0 + (int32_t)(ri.a >> 19);
+                const uint32_t gid = P.env_id_base + ri.env;
+                const Ph4 d0 = draw(P, STREAM_PLAN, gid, t, q, 0), d1 = draw(P, STREAM_PLAN, gid, t, q, 1);
+                float lp_t, lp_c, lp_r[4];
+                const uint32_t topo = sample_reg<4, NO>(l, 0, 4, u24(d0.x), lp_t);
+                const uint32_t cnt = sample_reg<4, NO>(l, 4, 4, u24(d0.y), lp_c);
+                const uint32_t ur[4] = {d1.x, d1.y, d1.z, d1.w};
+                uint32_t roles = 0;
+#pragma unroll
+                for (int a = 0; a < 4; a++) roles |= sample_reg<4, NO>(l, 8 + 4 * a, 4, u24(ur[a]), lp_r[a]) << (2 * a);
+                const uint32_t keff = keff_of(topo, cnt + 1);
+                float lp = __fadd_rn(lp_t, lp_c);
+#pragma unroll
+                for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
+                plan_commit(P, ri, topo, cnt, roles, lp);
+            }
+        }
+        cur = nxt;
+    }
+    tc::tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x < 32) tc::tmem_dealloc(tmem_base, Net::kTmemCols);
+}
+
 // ------------------------------------------------------------------------------------------------ launchers
 int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm,
                   bool bf16, cudaStream_t st)
@@ -426,6 +685,17 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
         const uint32_t grid = (uint32_t)n_sm * 2;
         if (exec) k_policy_f32<true><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
         else k_policy_f32<false><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
+        return 0;
+    }
+    if (W.tc_img) {
+        const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes;
+        if (exec) {
+            cudaFuncSetAttribute(k_policy_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            k_policy_tc<true><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
+        } else {
+            cudaFuncSetAttribute(k_policy_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            k_policy_tc<false><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
+        }
         return 0;
     }
     const uint32_t grid = (uint32_t)n_sm;

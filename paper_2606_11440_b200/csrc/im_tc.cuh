@@ -190,11 +190,13 @@ struct TcMlp {
     // proxy).  All 128 threads call it; on return `logit[i]` = D3[row = threadIdx.x][i] + b3[i].  `phase` is the mbarrier
     // parity, flipped three times.
     static __device__ __forceinline__ void run(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar,
-                                               uint32_t &phase, float (&logit)[NO])
+                                               uint32_t &phase, float (&logit)[NO], long long *ts = nullptr)
     {
         const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
         const float *bias = reinterpret_cast<const float *>(image + kBias);
         constexpr uint32_t idescH = instr_desc_bf16(128, H), idescO = instr_desc_bf16(128, NO);
+#define IM_TS(i) do { if (ts && threadIdx.x == 0) ts[i] = clock64(); } while (0)
+        IM_TS(0);
         // ---- layer 1 (SS)
         fence_proxy_async_smem();
         tc_fence_before();
@@ -209,7 +211,9 @@ struct TcMlp {
         }
         mbar_wait(bar, phase); phase ^= 1u;
         tc_fence_after();
+        IM_TS(1);
         hidden_epilogue(tlane, 0, bias);
+        IM_TS(2);
         // ---- layer 2 (TS): A2 = TMEM cols [0, H/2), D2 = cols [H, 2H)
         tc_fence_before();
         __syncthreads();
@@ -223,7 +227,9 @@ struct TcMlp {
         }
         mbar_wait(bar, phase); phase ^= 1u;
         tc_fence_after();
+        IM_TS(3);
         hidden_epilogue(tlane, H, bias + H);
+        IM_TS(4);
         // ---- layer 3 (TS): A3 = TMEM cols [H, H + H/2), D3 = cols [0, NO)
         tc_fence_before();
         __syncthreads();
@@ -237,6 +243,7 @@ struct TcMlp {
         }
         mbar_wait(bar, phase); phase ^= 1u;
         tc_fence_after();
+        IM_TS(5);
 #pragma unroll
         for (int j = 0; j < NO / 16; j++) {
             uint32_t v[16];
@@ -245,6 +252,8 @@ struct TcMlp {
 #pragma unroll
             for (int i = 0; i < 16; i++) logit[16 * j + i] = __uint_as_float(v[i]) + bias[2 * H + 16 * j + i];
         }
+        IM_TS(6);
+#undef IM_TS
         tc_fence_before();       // the next tile's layer-1 UMMA overwrites D3's columns: order these loads before it
     }
 };
