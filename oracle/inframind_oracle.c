@@ -14,7 +14,9 @@
  * constraint violation C-bar of the dual update (Eq. 7).  The paper trains on a live
  * vLLM pool and has no simulator; the tick semantics are the numbered Readings R1..R34 of DESIGN.md
  * (from SURVEY.md §8(c)), which this file follows STEP BY STEP in the canonical order, loops ascending,
- * with no blocking, fusion or reordering.
+ * with no blocking, fusion or reordering.  Requests are the calls (query, agent) and live in a table indexed
+ * by query*4 + agent; a RUNNING request holds a slot of its model (R10) and its service draw is keyed by that
+ * slot (R2, R11).
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers (P1), Poisson/budget/lognormal
  * tables (P2-P4), M/M/1 mean sojourn 1/(mu-lambda) (P6), Little's law (P7), conservation (P8), EDF
@@ -86,8 +88,10 @@ typedef struct {
     uint32_t budget, in_tok;
 } oq_t;
 
+/* R10: a request is the call (query, agent); the table is indexed by query*4 + agent.  A RUNNING request
+ * occupies one of the S_k slots of its model (north_star (1): "per-model slots"). */
 typedef struct {
-    uint8_t state, model, depth, agent, succ;
+    uint8_t state, model, depth, agent, succ, slot;
     uint16_t query;
     int32_t deadline, issue;
     uint32_t remaining, out_total, prefill_us, in_tok;
@@ -422,17 +426,37 @@ static uint32_t lowest_free_query(const orc_ctx *c, const oenv_t *E)
     for (uint32_t i = 0; i < c->s.qcap; i++) if (!E->q[i].live) return i;
     return c->s.qcap;
 }
-static uint32_t lowest_free_request(const orc_ctx *c, const oenv_t *E)
+static uint32_t n_req(const orc_ctx *c) { return 4u * c->s.qcap; }
+
+/* R10: lowest free slot of model k (the slots taken are those of its RUNNING requests) */
+static uint32_t lowest_free_slot(const orc_ctx *c, const oenv_t *E, uint32_t k)
 {
-    for (uint32_t i = 0; i < c->s.rcap; i++) if (E->r[i].state == ST_FREE) return i;
-    return c->s.rcap;
+    for (uint32_t sl = 0; sl < c->s.model[k].slots; sl++) {
+        int taken = 0;
+        for (uint32_t i = 0; i < n_req(c); i++)
+            if (E->r[i].state == ST_RUN && E->r[i].model == k && E->r[i].slot == sl) taken = 1;
+        if (!taken) return sl;
+    }
+    return c->s.model[k].slots;
 }
 
-/* R20: key = ((deadline - t + 2^19) << 12) | ridx (EDF) or ((issue - t + 2^19) << 12) | ridx (FCFS) */
-static uint32_t queue_key(const orc_ctx *c, const or_t *r, uint32_t ridx, int32_t t)
+/* R2: the slots of all models are numbered consecutively, each model's range padded to a multiple of 8, so
+ * that one Philox call (8 sixteen-bit fields) serves 8 slots of one model */
+static uint32_t global_slot(const orc_ctx *c, uint32_t k, uint32_t sl)
 {
-    int32_t base = c->s.sched_mode ? r->deadline : r->issue;
-    return ((uint32_t)(base - t + (1 << 19)) << 12) | ridx;
+    uint32_t base = 0;
+    for (uint32_t j = 0; j < k; j++) base += (c->s.model[j].slots + 7u) & ~7u;
+    return base + sl;
+}
+
+/* R20: the queue of model k is ordered by (deadline, query*4+agent) (EDF) or by
+ * (issue, query*4+agent) (FCFS); the pair is unique, so there is exactly one correct order.  Since
+ * remaining budget = deadline - t, "earliest remaining budget first" at a fixed t is the same order. */
+static int key_less(const orc_ctx *c, const or_t *a, uint32_t ia, const or_t *b, uint32_t ib)
+{
+    int32_t ka = c->s.sched_mode ? a->deadline : a->issue, kb = c->s.sched_mode ? b->deadline : b->issue;
+    if (ka != kb) return ka < kb;
+    return ia < ib;
 }
 
 static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
@@ -564,9 +588,9 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
             uint64_t prod = (uint64_t)s->depth_median_tok[depth] * c->tab_mult[d.v[1] >> 22];
             uint32_t out_total = (uint32_t)(prod >> 16);
             if (out_total < 1) out_total = 1;
-            uint32_t ri = lowest_free_request(c, E);
+            uint32_t ri = qi * 4u + agent;             /* R10: the call (query, agent) */
             or_t *r = &E->r[ri];
-            r->state = ST_WAIT; r->model = (uint8_t)model; r->depth = (uint8_t)depth; r->agent = (uint8_t)agent;
+            r->state = ST_WAIT; r->slot = 0; r->model = (uint8_t)model; r->depth = (uint8_t)depth; r->agent = (uint8_t)agent;
             r->succ = d.v[2] < s->model[model].succ_thresh[depth];
             r->query = (uint16_t)qi; r->deadline = q->deadline; r->issue = t;
             r->remaining = out_total; r->out_total = out_total; r->prefill_us = 0; r->in_tok = q->in_tok;
@@ -582,16 +606,16 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
         om_t *m = &E->m[k];
         for (;;) {
             if (m->n_wait == 0) break;
-            uint32_t best = 0xFFFFFFFFu, bi = 0;
-            for (uint32_t i = 0; i < s->rcap; i++) {
+            int found = 0; uint32_t bi = 0;
+            for (uint32_t i = 0; i < n_req(c); i++) {
                 const or_t *r = &E->r[i];
                 if (r->state != ST_WAIT || r->model != k) continue;
-                uint32_t key = queue_key(c, r, i, t);
-                if (key < best) { best = key; bi = i; }
+                if (!found || key_less(c, r, i, &E->r[bi], bi)) { found = 1; bi = i; }
             }
             or_t *r = &E->r[bi];
             uint32_t need = r->in_tok + (r->out_total - r->remaining);  /* R12 */
             if (!(m->n_run < s->model[k].slots && m->kv_used + need <= s->model[k].kv_cap)) break;
+            r->slot = (uint8_t)lowest_free_slot(c, E, k);      /* R10 (n_run < slots, so one is free) */
             r->state = ST_RUN;
             r->prefill_us = (uint32_t)(((uint64_t)s->model[k].prefill_us_per_ktok * need) / 1000u);
             m->kv_used += need; m->n_wait--; m->n_run++;
@@ -599,7 +623,7 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
     }
 
     /* ---- F SERVE (R11): token-level service with stochastic rounding */
-    for (uint32_t i = 0; i < s->rcap; i++) {
+    for (uint32_t i = 0; i < n_req(c); i++) {
         or_t *r = &E->r[i];
         if (r->state != ST_RUN) continue;
         uint32_t usable = ORC_DT_US;
@@ -607,8 +631,11 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
         r->prefill_us -= d; usable -= d;
         uint32_t xx = s->model[r->model].rate_tok_s * usable;
         uint32_t base = xx / 1000000u, frac = xx % 1000000u;
-        uint32_t u = draw(c, STREAM_SVC, gid, t, i >> 2, 0).v[i & 3];
-        uint32_t extra = mulhi32(u, 1000000u) < frac ? 1u : 0u;
+        /* R2/R11: sixteen-bit uniform of the request's slot; Bernoulli(frac) to 2^-16 */
+        uint32_t gs = global_slot(c, r->model, r->slot), f = gs & 7u;
+        uint32_t u16 = (draw(c, STREAM_SVC, gid, t, gs >> 3, 0).v[f >> 1] >> (16u * (f & 1u))) & 0xFFFFu;
+        uint32_t thr = (uint32_t)(((uint64_t)frac << 16) / 1000000u);
+        uint32_t extra = u16 < thr ? 1u : 0u;
         uint32_t tok = base + extra;
         if (tok > r->remaining) tok = r->remaining;
         r->remaining -= tok;
@@ -617,7 +644,7 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
 
     /* ---- G COMPLETE (R1, R13, R27, R28) */
     uint32_t lat_sum[ORC_MAXN] = {0}, lat_n[ORC_MAXN] = {0};
-    for (uint32_t i = 0; i < s->rcap; i++) {
+    for (uint32_t i = 0; i < n_req(c); i++) {
         or_t *r = &E->r[i];
         if (r->state != ST_RUN || r->remaining != 0) continue;
         oq_t *q = &E->q[r->query];
@@ -660,7 +687,7 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
             om_t *m = &E->m[k];
             while (m->kv_used > s->model[k].kv_cap) {
                 int found = 0; uint32_t vi = 0; int32_t vd = 0;
-                for (uint32_t i = 0; i < s->rcap; i++) {
+                for (uint32_t i = 0; i < n_req(c); i++) {
                     const or_t *r = &E->r[i];
                     if (r->state != ST_RUN || r->model != k) continue;
                     if (!found || r->deadline > vd || (r->deadline == vd && i > vi)) { found = 1; vd = r->deadline; vi = i; }
@@ -668,7 +695,7 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
                 if (!found) break;
                 or_t *r = &E->r[vi];
                 m->kv_used -= r->in_tok + (r->out_total - r->remaining);
-                r->state = ST_WAIT; r->prefill_us = 0;
+                r->state = ST_WAIT; r->prefill_us = 0; r->slot = 0;
                 m->n_run--; m->n_wait++;
                 E->ctr[C_PREEMPT]++;
             }
@@ -686,7 +713,7 @@ static void env_tick(orc_ctx *c, uint32_t ei, int32_t t, uint32_t trow)
     if (done) {                                            /* hard reset, live queries abandoned */
         for (uint32_t i = 0; i < s->qcap; i++) E->ctr[C_ABANDONED] += E->q[i].live;
         memset(E->q, 0, sizeof(oq_t) * s->qcap);
-        memset(E->r, 0, sizeof(or_t) * s->rcap);
+        memset(E->r, 0, sizeof(or_t) * n_req(c));
         memset(E->m, 0, sizeof(E->m));
     }
 }
@@ -696,7 +723,7 @@ int orc_create(const orc_spec *spec, uint32_t n_envs, const uint32_t *env_ids, c
                uint64_t seed, orc_ctx **out)
 {
     if (!spec || !out || !n_envs || !env_ids || !env_level) return -1;
-    if (spec->n_models == 0 || spec->n_models > ORC_MAXN || spec->rcap < 3 * spec->qcap || spec->rcap > 4096 ||
+    if (spec->n_models == 0 || spec->n_models > ORC_MAXN || spec->rcap < 3 * spec->qcap || spec->rcap > 4096 || spec->qcap > 1024 ||
         spec->f_in > 512 || spec->hidden > 512 || spec->f_in < 3 * spec->n_models + 12) return -2;
     orc_ctx *c = (orc_ctx *)calloc(1, sizeof(orc_ctx));
     c->s = *spec;
@@ -710,7 +737,7 @@ int orc_create(const orc_spec *spec, uint32_t n_envs, const uint32_t *env_ids, c
     c->env = (oenv_t *)calloc(n_envs, sizeof(oenv_t));
     for (uint32_t i = 0; i < n_envs; i++) {
         c->env[i].q = (oq_t *)calloc(spec->qcap, sizeof(oq_t));
-        c->env[i].r = (or_t *)calloc(spec->rcap, sizeof(or_t));
+        c->env[i].r = (or_t *)calloc(4u * spec->qcap, sizeof(or_t));
     }
     size_t rows = (size_t)spec->max_ticks + 1;
     c->rew = (float *)calloc(rows * n_envs, 4); c->cost = (float *)calloc(rows * n_envs, 4);
@@ -736,7 +763,7 @@ int orc_reset(orc_ctx *c)
     for (uint32_t i = 0; i < c->n_envs; i++) {
         oenv_t *E = &c->env[i];
         memset(E->q, 0, sizeof(oq_t) * c->s.qcap);
-        memset(E->r, 0, sizeof(or_t) * c->s.rcap);
+        memset(E->r, 0, sizeof(or_t) * n_req(c));
         memset(E->m, 0, sizeof(E->m));
         memset(E->ctr, 0, sizeof(E->ctr));
         E->n_desync = E->n_hard = E->n_near = 0; E->max_logit_diff = E->max_value_diff = 0.0;
@@ -837,7 +864,7 @@ int orc_returns(orc_ctx *c, double gamma, double lam, double mu)
 enum { ORC_REW = 1, ORC_COST, ORC_VAL, ORC_DONE, ORC_MISS, ORC_ADV, ORC_RET, ORC_COUNTERS, ORC_SNAPSHOT, ORC_STATE,
        ORC_SCALARS, ORC_STATS };
 
-size_t orc_state_words(const orc_ctx *c) { return 4u * c->s.n_models + 4u * c->s.qcap + 5u * c->s.rcap; }
+size_t orc_state_words(const orc_ctx *c) { return 4u * c->s.n_models + 4u * c->s.qcap + 5u * 4u * c->s.qcap; }
 
 static void dump_state(const orc_ctx *c, const oenv_t *E, uint32_t *w)
 {
@@ -853,13 +880,14 @@ static void dump_state(const orc_ctx *c, const oenv_t *E, uint32_t *w)
                ((uint32_t)q->succ << 17) | (roles << 18);
         *w++ = (uint32_t)q->deadline; *w++ = (uint32_t)q->arrive; *w++ = q->budget | (q->in_tok << 16);
     }
-    for (uint32_t i = 0; i < c->s.rcap; i++) {
+    for (uint32_t i = 0; i < n_req(c); i++) {
         const or_t *r = &E->r[i];
         if (r->state == ST_FREE) { w[0] = w[1] = w[2] = w[3] = w[4] = 0; w += 5; continue; }
         *w++ = r->state | ((uint32_t)r->model << 2) | ((uint32_t)r->depth << 6) | ((uint32_t)r->agent << 8) |
                ((uint32_t)r->succ << 10) | ((uint32_t)r->query << 16);
         *w++ = (uint32_t)r->deadline; *w++ = (uint32_t)r->issue;
-        *w++ = r->remaining | (r->prefill_us << 16); *w++ = r->out_total | (r->in_tok << 16);
+        /* prefill is sub-tick (R11), hence 0 at every tick boundary; the field carries slot+1 of a RUNNING request */
+        *w++ = r->remaining | ((r->state == ST_RUN ? (uint32_t)r->slot + 1u : 0u) << 16); *w++ = r->out_total | (r->in_tok << 16);
     }
 }
 
@@ -951,20 +979,20 @@ int orc_read_queries(const orc_ctx *c, uint32_t *env, int32_t *arrive, uint32_t 
 int orc_queue_order(const orc_ctx *c, uint32_t ei, uint32_t k, int32_t t, uint32_t *ridx_out, uint32_t cap)
 {
     const oenv_t *E = &c->env[ei];
-    uint32_t n = 0;
-    uint32_t last = 0; int have_last = 0;
+    uint32_t n = 0, last = 0;
+    int have_last = 0;
+    (void)t;                 /* the order at a fixed t does not depend on t (R20) */
     for (;;) {
-        uint32_t best = 0xFFFFFFFFu, bi = 0; int found = 0;
-        for (uint32_t i = 0; i < c->s.rcap; i++) {
+        uint32_t bi = 0; int found = 0;
+        for (uint32_t i = 0; i < n_req(c); i++) {
             const or_t *r = &E->r[i];
             if (r->state != ST_WAIT || r->model != k) continue;
-            uint32_t key = queue_key(c, r, i, t);
-            if (have_last && key <= last) continue;
-            if (key < best) { best = key; bi = i; found = 1; }
+            if (have_last && !key_less(c, &E->r[last], last, r, i)) continue;   /* only those after `last` */
+            if (!found || key_less(c, r, i, &E->r[bi], bi)) { bi = i; found = 1; }
         }
         if (!found) break;
         if (n < cap) ridx_out[n] = bi;
-        n++; last = best; have_last = 1;
+        n++; last = bi; have_last = 1;
     }
     return (int)n;
 }

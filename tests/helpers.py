@@ -14,7 +14,7 @@ ST_FREE, ST_WAIT, ST_RUN = 0, 1, 2
 
 
 def decode_state(words: np.ndarray, N: int, qcap: int, rcap: int):
-    """words: [n_envs][4N + 4*qcap + 5*rcap] u32 -> dict of arrays."""
+    """words: [n_envs][4N + 4*qcap + 5*rcap] u32 -> dict of arrays; rcap = 4*qcap, request row = query*4 + agent."""
     w = np.asarray(words, dtype=np.uint32)
     n = w.shape[0]
     m = w[:, : 4 * N].reshape(n, N, 4)
@@ -30,7 +30,7 @@ def decode_state(words: np.ndarray, N: int, qcap: int, rcap: int):
         q_budget=q[:, :, 3] & 0xFFFF, q_in_tok=q[:, :, 3] >> 16,
         r_state=r0 & 3, r_model=(r0 >> 2) & 15, r_depth=(r0 >> 6) & 3, r_agent=(r0 >> 8) & 3, r_succ=(r0 >> 10) & 1,
         r_query=r0 >> 16, r_deadline=r[:, :, 1].astype(np.int32), r_issue=r[:, :, 2].astype(np.int32),
-        r_remaining=r[:, :, 3] & 0xFFFF, r_prefill_us=r[:, :, 3] >> 16, r_out_total=r[:, :, 4] & 0xFFFF,
+        r_remaining=r[:, :, 3] & 0xFFFF, r_slot1=r[:, :, 3] >> 16, r_out_total=r[:, :, 4] & 0xFFFF,
         r_in_tok=r[:, :, 4] >> 16,
     )
 

@@ -149,7 +149,7 @@ def test_p3_budget_mixture_cfg5(orc):
     spec = make_pool_spec(5, n_envs=64, n_ticks=64)
     o = orc.Oracle(spec, seed=0)
     o.rollout(make_policy_blob(spec), 64)
-    st = decode_state(o.state(), spec.n_models, spec.qcap, spec.rcap)
+    st = decode_state(o.state(), spec.n_models, spec.qcap, 4 * spec.qcap)
     b = st["q_budget"][st["q_live"] == 1].astype(np.int64)
     tight = (b >= 100) & (b <= 300)
     relaxed = (b >= 800) & (b <= 2400)
@@ -220,6 +220,11 @@ def _check_conservation(spec, st, c, tick_end):
         assert np.array_equal(kv, st["kv_used"][:, k])
         if spec.kv_preempt:
             assert np.all(st["kv_used"][:, k] <= spec.kv_cap[k])
+        # R10: every RUNNING request of model k holds a distinct slot < S_k; WAITING requests hold none
+        for e in range(run_k.shape[0]):
+            sl = st["r_slot1"][e][run_k[e]].astype(np.int64) - 1
+            assert np.all((sl >= 0) & (sl < spec.slots[k])) and np.unique(sl).size == sl.size
+        assert np.all(st["r_slot1"][wait_k] == 0)
     # pending of each live query == its in-flight requests
     for e in range(st["q_live"].shape[0]):
         act = st["r_state"][e] != 0
@@ -235,7 +240,7 @@ def test_p8_conservation_every_tick(orc, cfg):
     o = orc.Oracle(spec, seed=0)
     for step in range(80):
         o.rollout(blob, 3)
-        st = decode_state(o.state(), spec.n_models, spec.qcap, spec.rcap)
+        st = decode_state(o.state(), spec.n_models, spec.qcap, 4 * spec.qcap)
         _check_conservation(spec, st, o.counters(), o.tick)
 
 
@@ -244,7 +249,7 @@ def test_p7_little_identity(orc):
     o = orc.Oracle(spec, seed=3)
     o.rollout(make_policy_blob(spec), 400)
     c = o.counters()
-    st = decode_state(o.state(), spec.n_models, spec.qcap, spec.rcap)
+    st = decode_state(o.state(), spec.n_models, spec.qcap, 4 * spec.qcap)
     still = ((400 - st["q_arrive"]) * st["q_live"]).sum(axis=1)
     assert np.array_equal(c[:, CN["sum_live_mid"]], c[:, CN["sum_sojourn"]] + still.astype(np.uint64))
     assert c[:, CN["dropped"]].sum() > 0
@@ -268,7 +273,7 @@ def test_p9_queue_order_and_admission_brute_force(orc, sched_mode):
     prev = None
     for t in range(300):
         o.rollout(blob, 1)
-        st = decode_state(o.state(), 2, spec.qcap, spec.rcap)
+        st = decode_state(o.state(), 2, spec.qcap, 4 * spec.qcap)
         tnow = t + 1                               # keys for the NEXT tick's admission
         for e in range(8):
             for k in range(2):
@@ -310,10 +315,10 @@ def test_p10_action_decode(orc):
     blob = make_policy_blob(spec, scale=3.0)
     o = orc.Oracle(spec, seed=2)
     seen = set()
-    prev = decode_state(o.state(), 5, spec.qcap, spec.rcap)
+    prev = decode_state(o.state(), 5, spec.qcap, 4 * spec.qcap)
     for t in range(200):
         o.rollout(blob, 1)
-        st = decode_state(o.state(), 5, spec.qcap, spec.rcap)
+        st = decode_state(o.state(), 5, spec.qcap, 4 * spec.qcap)
         d = o.decisions(1)
         assert np.all(d["payload"] < 15)
         for j in range(d["t"].size):
@@ -506,12 +511,12 @@ def test_p18_prefill_reduces_first_tick_tokens(orc):
     seen = 0
     for t in range(40):
         o.rollout(blob, 1)
-        st = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+        st = decode_state(o.state(), 1, spec.qcap, 4 * spec.qcap)
         new = (st["r_state"] == ST_RUN) & (st["r_issue"] == t)
         if new.any():
             # prefill = 10000 us/ktok * 1000 tok / 1000 = 10000 us => usable 40000 us * 200 tok/s = 8 tokens
             assert np.all((st["r_out_total"] - st["r_remaining"])[new] == 8)
-            assert np.all(st["r_prefill_us"][new] == 0)
+            assert np.all(st["r_slot1"][new] >= 1)      # RUNNING requests hold a slot (R10)
             seen += int(new.sum())
     assert seen > 5
 
@@ -526,7 +531,7 @@ def test_p19_preemption_victim_and_token_conservation(orc):
     prev_c = np.zeros(8, np.uint64)
     for t in range(400):
         o.rollout(blob, 1)
-        st = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+        st = decode_state(o.state(), 1, spec.qcap, 4 * spec.qcap)
         c = o.counters()[:, CN["preemptions"]]
         assert np.all(st["kv_used"][:, 0] <= 700)
         if prev is not None:
@@ -551,6 +556,47 @@ def test_p19_preemption_victim_and_token_conservation(orc):
     assert np.array_equal(cc[:, CN["calls_issued"]], cc[:, CN["calls_done"]] + (st["n_wait"] + st["n_run"])[:, 0])
 
 
+# ------------------------------------------------------------------------------------------- R10 / R2 slots
+def test_r10_lowest_free_slot_and_slot_keyed_service_draw(orc):
+    """R10: admissions of tick t take, in queue order, the lowest slots that were free at the end of tick t-1.
+    R2/R11: a request RUNNING in slot s of model k decodes base + [u16 < thr] tokens, u16 = field (gs & 7) of
+    Philox(SVC; env, t, gs >> 3), gs = (slots of the models before k, padded to 8) + s  -- retyped here."""
+    S = [4, 12]
+    spec = tiny_spec(n_envs=6, N=2, n_ticks=200, qcap=16, rcap=48, rate_tick=0.3, slots=S, rates=[130, 57],
+                     budget=(3000, 3000), medians=(400, 600, 800), seed=11)
+    blob = make_policy_blob(spec, seed=3)
+    seed = 21
+    o = orc.Oracle(spec, seed=seed)
+    prev = decode_state(o.state(), 2, spec.qcap, 4 * spec.qcap)
+    n_adm = n_srv = 0
+    for t in range(200):
+        o.rollout(blob, 1)
+        st = decode_state(o.state(), 2, spec.qcap, 4 * spec.qcap)
+        for e in range(6):
+            for k in range(2):
+                was = (prev["r_state"][e] == ST_RUN) & (prev["r_model"][e] == k)
+                now = (st["r_state"][e] == ST_RUN) & (st["r_model"][e] == k)
+                same = was & now & (prev["r_issue"][e] == st["r_issue"][e])
+                newly = np.nonzero(now & ~same)[0]
+                if len(newly):
+                    free = sorted(set(range(S[k])) - set((prev["r_slot1"][e][was] - 1).tolist()))
+                    order = newly[np.lexsort((newly, st["r_deadline"][e][newly]))]
+                    assert (st["r_slot1"][e][order] - 1).tolist() == free[: len(order)]
+                    n_adm += len(order)
+                base_gs = 0 if k == 0 else 8        # ceil8(4)
+                x = int(spec.rate_tok_s[k]) * 50000
+                b, thr = x // 1000000, ((x % 1000000) << 16) // 1000000
+                for i in np.nonzero(same)[0]:
+                    assert st["r_slot1"][e][i] == prev["r_slot1"][e][i]          # a running request keeps its slot
+                    gs = base_gs + int(st["r_slot1"][e][i]) - 1
+                    w = orc.philox(e, t, gs >> 3, 0, seed & 0xFFFFFFFF, (seed >> 32) ^ 5)[(gs & 7) >> 1]
+                    u16 = (int(w) >> (16 * (gs & 1))) & 0xFFFF
+                    assert int(prev["r_remaining"][e][i]) - int(st["r_remaining"][e][i]) == b + (1 if u16 < thr else 0)
+                    n_srv += 1
+        prev = st
+    assert n_adm > 100 and n_srv > 2000
+
+
 # ------------------------------------------------------------------------------------------- P20
 def test_p20_service_rate_stochastic_rounding(orc):
     """Long-run tokens/tick of a running request = rate*DT (R11): 130 tok/s = 6.5 tok/tick."""
@@ -561,10 +607,10 @@ def test_p20_service_rate_stochastic_rounding(orc):
     blob = forced_single_blob(spec)
     o.rollout(blob, 10)
     tot, n = 0, 0
-    prev = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+    prev = decode_state(o.state(), 1, spec.qcap, 4 * spec.qcap)
     for _ in range(50):
         o.rollout(blob, 5)
-        st = decode_state(o.state(), 1, spec.qcap, spec.rcap)
+        st = decode_state(o.state(), 1, spec.qcap, 4 * spec.qcap)
         both = (prev["r_state"] == ST_RUN) & (st["r_state"] == ST_RUN) & (prev["r_issue"] == st["r_issue"])
         tot += int((prev["r_remaining"].astype(np.int64) - st["r_remaining"])[both].sum())
         n += int(both.sum()) * 5
