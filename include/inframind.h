@@ -69,7 +69,8 @@ typedef struct im_pool_spec {
     uint32_t abi_version;            /* IM_ABI_VERSION */
     uint32_t n_models;               /* N <= 16 */
     uint32_t qcap;                   /* query-table slots per env, multiple of 32, <= 1024 (R9) */
-    uint32_t rcap;                   /* request-pool slots per env, multiple of 128, >= 3*qcap, <= 4096 (R9, R20) */
+    uint32_t rcap;                   /* waiting-list capacity per env, multiple of 128, >= 3*qcap, <= 4096: a query has at most
+                                        3 calls in flight (R17), so the list never overflows (R9) */
     uint32_t max_ticks;              /* trajectory capacity of one im_rollout, <= 8191 */
     uint32_t sched_mode;             /* IM_SCHED_* (R20) */
     uint32_t kv_preempt;             /* 1: evict when kv_used > kv_cap (R21) */
@@ -143,8 +144,8 @@ typedef enum im_telemetry {
     IM_TEL_DECISIONS_PLAN = 12, /* u32 [n][6]: env(global), t(abs), q, topo | cnt<<2 | roles<<4, logp(f32 bits), 0 */
     IM_TEL_QUERIES = 13,   /* u32 [n][4]: env(global), arrive, sojourn, budget | solved<<16 | topo<<17 | keff<<19 */
     IM_TEL_UNORM = 14,     /* f32 [n]: normalised utility of each QUERIES record, same order (after im_returns) */
-    IM_TEL_STATE = 15,     /* u32 [E][4N + 4*QCAP + 5*RCAP]: canonical full state dump, layout below */
-    IM_TEL_QUEUE_ORDER = 16,/* u32 [E][N+1 + RCAP]: per env N+1 segment offsets, then the WAITING request indices
+    IM_TEL_STATE = 15,     /* u32 [E][4N + 4*QCAP + 5*(4*QCAP)]: canonical full state dump, layout below */
+    IM_TEL_QUEUE_ORDER = 16,/* u32 [E][N+1 + RCAP]: per env N+1 segment offsets, then the WAITING request ids (4*query + agent)
                               of model 0, model 1, ... each in slack (R20 key) order; unused tail = 0xFFFFFFFF */
     IM_TEL_TABLES = 17,    /* u32: out_tok_mult_q16[1024], in_tok[1024], arr_cdf[n_levels*32] as uploaded */
     IM_TEL_LOGITS_EXEC = 18,/* f32 [n][3N+1], same order as DECISIONS_EXEC (needs IM_FLAG_LOG_LOGITS) */
@@ -155,8 +156,11 @@ typedef enum im_telemetry {
  *   model k : n_wait, n_run, kv_used, ewma_q8
  *   query i : w0 = live | planned<<1 | topo<<2 | (K-1)<<4 | keff<<6 | stage<<9 | n_stages<<12 | pending<<15 |
  *                  solved<<17 | roles(4x2b)<<18 ; w1 = deadline ; w2 = arrive ; w3 = budget | in_tok<<16
- *   request i: w0 = state(0 free,1 waiting,2 running) | model<<2 | depth<<6 | agent<<8 | succ<<10 | query<<16 ;
- *              w1 = deadline ; w2 = issue ; w3 = remaining | prefill_us<<16 ; w4 = out_total | in_tok<<16 */
+ *   request i = 4*query + agent (R10), i < 4*QCAP:
+ *              w0 = state(0 free,1 waiting,2 running) | model<<2 | depth<<6 | agent<<8 | succ<<10 | query<<16 ;
+ *              w1 = deadline ; w2 = issue ; w3 = remaining | (slot+1 if running else 0)<<16 ; w4 = out_total | in_tok<<16
+ * Device-side limits: slots <= 64 per model, input / output tokens <= 8191 per call, absolute tick + largest budget
+ * < 65536 (im_rollout returns IM_ERR_CAPACITY beyond; im_reset restarts the clock). */
 
 /* Synchronise the stream and copy the selected telemetry to caller-owned HOST memory `dst`.
  * *written receives the byte count (or the needed size with IM_ERR_CAPACITY). dst == NULL queries the size. */

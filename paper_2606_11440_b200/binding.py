@@ -207,7 +207,7 @@ class InfraMind:
     def ret(self): return self.read(IM_TEL_RET, np.float32, (self.T, self.E))
     def counters(self): return self.read(IM_TEL_COUNTERS, np.uint64, (self.E, 16))
     def snapshot(self): return self.read(IM_TEL_SNAPSHOT, np.uint32, (self.E, self.N, 4))
-    def state(self): return self.read(IM_TEL_STATE, np.uint32, (self.E, 4 * self.N + 4 * self.spec.qcap + 5 * self.spec.rcap))
+    def state(self): return self.read(IM_TEL_STATE, np.uint32, (self.E, 4 * self.N + 4 * self.spec.qcap + 20 * self.spec.qcap))
     def queue_order(self): return self.read(IM_TEL_QUEUE_ORDER, np.uint32, (self.E, self.N + 1 + self.spec.rcap))
 
     def scalars(self):

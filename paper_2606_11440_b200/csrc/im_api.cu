@@ -23,14 +23,14 @@ bool tc_supported(uint32_t F, uint32_t H);
 size_t tc_image_bytes(bool exec);
 void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t st);
 
-// empty pools: zero the header of every env record, free bitmaps all ones (free slots are defined by the bitmaps)
+// empty pools: zero the header of every env record (no slot taken, empty waiting list), query bitmap all free
 __global__ void k_reset(const Params P)
 {
     const size_t n = (size_t)P.E * P.hdr_words;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const uint32_t e = (uint32_t)(i / P.hdr_words), w = (uint32_t)(i % P.hdr_words);
         uint32_t v = 0;
-        if ((w >= P.hw_rfree && w < P.hw_rfree + P.RW) || (w >= P.hw_qfree && w < P.hw_qfree + P.QW)) v = 0xFFFFFFFFu;
+        if (w >= P.hw_qfree && w < P.hw_qfree + P.QW) v = 0xFFFFFFFFu;
         reinterpret_cast<uint32_t *>(env_rec(P, e))[w] = v;
     }
 }
@@ -171,7 +171,8 @@ static int validate(const im_pool_spec *s, uint32_t E)
     if (!s->out_tok_mult_q16 || !s->arr_cdf || !s->env_level) return fail(nullptr, IM_ERR_INVALID_ARG, "null table pointer");
     for (uint32_t k = 0; k < s->n_models; k++) {
         const im_model_spec &m = s->model[k];
-        if (m.slots == 0 || m.kv_cap == 0 || m.rate_tok_s == 0 || m.rate_tok_s > 80000) return fail(nullptr, IM_ERR_BAD_SPEC, "model %u: zero slots/kv/rate or rate too large", k);
+        if (m.slots == 0 || m.slots > 64 || m.kv_cap == 0 || m.rate_tok_s == 0 || m.rate_tok_s > 80000)
+            return fail(nullptr, IM_ERR_BAD_SPEC, "model %u: slots out of 1..64, zero kv/rate or rate too large", k);
     }
     for (int i = 0; i < 2; i++)
         if (s->mix_lo[i] == 0 || s->mix_hi[i] < s->mix_lo[i] || s->mix_hi[i] > 65535) return fail(nullptr, IM_ERR_BAD_SPEC, "budget component %d out of range", i);
@@ -180,11 +181,18 @@ static int validate(const im_pool_spec *s, uint32_t E)
             if (s->arr_cdf[l * 32 + j] < s->arr_cdf[l * 32 + j - 1]) return fail(nullptr, IM_ERR_BAD_SPEC, "arr_cdf row %u not monotone", l);
     for (uint32_t e = 0; e < E; e++)
         if (s->env_level[e] >= s->n_levels) return fail(nullptr, IM_ERR_BAD_SPEC, "env_level[%u] out of range", e);
+    uint64_t max_out = 1, max_in = s->in_tok_table ? 0 : s->in_tok_const;
     for (int i = 0; i < 1024; i++) {
-        const uint64_t v = ((uint64_t)s->depth_median_tok[2] * s->out_tok_mult_q16[i]) >> 16;
-        if (v > 65535) return fail(nullptr, IM_ERR_BAD_SPEC, "output tokens exceed 65535");
-        if (s->in_tok_table && s->in_tok_table[i] > 65535) return fail(nullptr, IM_ERR_BAD_SPEC, "input tokens exceed 65535");
+        for (int d = 0; d < 3; d++) {
+            const uint64_t v = ((uint64_t)s->depth_median_tok[d] * s->out_tok_mult_q16[i]) >> 16;
+            max_out = v > max_out ? v : max_out;
+        }
+        if (s->in_tok_table) max_in = s->in_tok_table[i] > max_in ? s->in_tok_table[i] : max_in;
     }
+    if (max_out > 8191 || max_in > 8191) return fail(nullptr, IM_ERR_BAD_SPEC, "output / input tokens exceed 8191 (13-bit fields)");
+    for (uint32_t k = 0; k < s->n_models; k++)       // R11: prefill is sub-tick
+        if ((uint64_t)s->model[k].prefill_us_per_ktok * (max_in + max_out) / 1000u > 50000u)
+            return fail(nullptr, IM_ERR_BAD_SPEC, "model %u: prefill of the largest request exceeds one tick", k);
     if (s->sched_mode > 1) return fail(nullptr, IM_ERR_BAD_SPEC, "sched_mode");
     return IM_OK;
 }
@@ -221,16 +229,18 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     const size_t T1 = (size_t)s.max_ticks + 1;
     auto up4 = [](uint32_t w) { return (w + 3u) & ~3u; };
     // ---- per-env record (im_device.cuh): header words, then the arrays
-    P.RW = R / 32; P.QW = Q / 32;
-    P.hw_rfree = 4 * N; P.hw_qfree = P.hw_rfree + up4(P.RW); P.hw_qready = P.hw_qfree + up4(P.QW);
+    P.QW = Q / 32;
+    P.slot_base[0] = 0;
+    for (uint32_t k = 0; k < kMaxModels; k++) P.slot_base[k + 1] = P.slot_base[k] + (k < N ? ((s.model[k].slots + 7u) & ~7u) : 0u);
+    P.SP = P.slot_base[N];
+    P.hw_occ = 4 * N; P.hw_qfree = P.hw_occ + up4(2 * N); P.hw_qready = P.hw_qfree + up4(P.QW);
     P.hw_misc = P.hw_qready + up4(P.QW); P.hw_ctr = P.hw_misc + 4; P.hdr_words = P.hw_ctr + 32;
     uint32_t off = (P.hdr_words * 4 + 127u) & ~127u;
-    P.off_iss = off; off += kIssueCap * 16;
-    P.off_hot = off; off += R * 4;
-    P.off_dl = off; off += R * 4;
-    P.off_issue = off; off += R * 4;
-    P.off_tok = off; off += R * 4;
-    P.off_aux = off; off += R * 4;
+    P.off_iss = off; off += kIssueCap * 8;
+    P.off_hot = off; off += ((P.SP * 4 + 127u) & ~127u);
+    P.off_cold = off; off += ((P.SP * 8 + 127u) & ~127u);
+    P.off_wkey = off; off += R * 4;
+    P.off_waux = off; off += R * 8;
     P.off_q = off; off += Q * 16;
     P.env_stride = (off + 127u) & ~127u;
     P.env_base = cv.take<uint8_t>((size_t)E * P.env_stride);
@@ -439,6 +449,10 @@ int im_rollout(im_ctx *c, const void *policy_weights, uint32_t n_ticks)
     if (!c || !policy_weights) return fail(c, IM_ERR_INVALID_ARG, "null ctx or weights");
     if (!c->bound) return fail(c, IM_ERR_STATE, "im_rollout before im_bind");
     if (n_ticks == 0 || n_ticks > c->spec.max_ticks) return fail(c, IM_ERR_CAPACITY, "n_ticks %u out of 1..max_ticks=%u", n_ticks, c->spec.max_ticks);
+    {   // absolute ticks (issue, deadline) are 16-bit fields of the device state
+        const uint32_t hi = c->spec.mix_hi[0] > c->spec.mix_hi[1] ? c->spec.mix_hi[0] : c->spec.mix_hi[1];
+        if ((uint64_t)c->tick + n_ticks + hi >= 65536u) return fail(c, IM_ERR_CAPACITY, "tick %d + %u + budget %u reaches 65536: im_reset first", c->tick, n_ticks, hi);
+    }
     int rc = upload_weights(c, policy_weights);
     if (rc != IM_OK) return rc;
     cudaStream_t st = c->stream;
@@ -612,7 +626,8 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         return IM_OK;
     }
     case IM_TEL_STATE: {
-        const size_t words = 4 * N + 4 * Q + 5 * R, bytes = 4 * words * E;
+        const size_t RD = 4 * Q;                                  // canonical request table: row = 4*query + agent
+        const size_t words = 4 * N + 4 * Q + 5 * RD, bytes = 4 * words * E;
         if (written) *written = bytes;
         if (!dst) return IM_OK;
         if (dst_bytes < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, bytes);
@@ -625,19 +640,34 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
             CUDA_TRY(c, cudaMemcpy(buf.data(), P.env_base + e0 * P.env_stride, ne * P.env_stride, cudaMemcpyDeviceToHost));
             for (size_t e = 0; e < ne; e++) {
                 const uint8_t *rec = buf.data() + e * P.env_stride;
-                const uint32_t *hdr = (const uint32_t *)rec, *rfree = hdr + P.hw_rfree, *qfree = hdr + P.hw_qfree;
-                const uint32_t *hot = (const uint32_t *)(rec + P.off_hot), *dl = (const uint32_t *)(rec + P.off_dl), *is = (const uint32_t *)(rec + P.off_issue);
-                const uint32_t *tok = (const uint32_t *)(rec + P.off_tok), *aux = (const uint32_t *)(rec + P.off_aux);
+                const uint32_t *hdr = (const uint32_t *)rec, *occ = hdr + P.hw_occ, *qfree = hdr + P.hw_qfree;
+                const uint32_t *hot = (const uint32_t *)(rec + P.off_hot), *wkey = (const uint32_t *)(rec + P.off_wkey);
+                const uint2 *cold = (const uint2 *)(rec + P.off_cold), *waux = (const uint2 *)(rec + P.off_waux);
                 const uint4 *qt = (const uint4 *)(rec + P.off_q);
                 memcpy(w, hdr, 16 * N); w += 4 * N;
                 for (size_t i = 0; i < Q; i++, w += 4) {
                     if ((qfree[i >> 5] >> (i & 31)) & 1u) { w[0] = w[1] = w[2] = w[3] = 0; continue; }
                     w[0] = qt[i].x; w[1] = qt[i].z; w[2] = qt[i].w; w[3] = qt[i].y;
                 }
-                for (size_t i = 0; i < R; i++, w += 5) {
-                    if ((rfree[i >> 5] >> (i & 31)) & 1u) { w[0] = w[1] = w[2] = w[3] = w[4] = 0; continue; }
-                    w[0] = (aux[i] & ~3u) | ((hot[i] >> HOT_STATE_SHIFT) & 3u); w[1] = dl[i]; w[2] = is[i]; w[3] = hot[i] & 0xFFFFu; w[4] = tok[i];
+                memset(w, 0, 4 * 5 * RD);
+                auto put = [&](uint32_t id, uint32_t state, uint32_t model, uint32_t sw, uint32_t dl, uint32_t issue, uint32_t rem, uint32_t slot1) {
+                    uint32_t *r = w + 5 * (size_t)id;
+                    r[0] = state | (model << 2) | (((sw >> SW_DEPTH_SHIFT) & 3u) << 6) | ((id & 3u) << 8) | (((sw >> SW_SUCC_SHIFT) & 1u) << 10) | ((id >> 2) << 16);
+                    r[1] = dl; r[2] = issue; r[3] = rem | (slot1 << 16);
+                    r[4] = (sw & SW_TOK_MASK) | (((sw >> SW_IN_SHIFT) & SW_TOK_MASK) << 16);
+                };
+                for (uint32_t k = 0; k < N; k++)
+                    for (uint32_t sl = 0; sl < c->spec.model[k].slots; sl++) {
+                        if (!((occ[2 * k + (sl >> 5)] >> (sl & 31)) & 1u)) continue;
+                        const uint32_t gs = P.slot_base[k] + sl;
+                        put((hot[gs] >> 16) & 0xFFFu, ST_RUN, k, cold[gs].y, cold[gs].x >> 16, cold[gs].x & 0xFFFFu, hot[gs] & 0xFFFFu, sl + 1);
+                    }
+                const uint32_t nw = hdr[P.hw_misc + 2];
+                for (uint32_t j = 0; j < nw && j < R; j++) {
+                    const uint32_t id = wkey[j] & 0xFFFu, tm = (wkey[j] >> 12) & 0xFFFFu;
+                    put(id, ST_WAIT, wkey[j] >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
                 }
+                w += 5 * RD;
             }
         }
         return IM_OK;

@@ -3,15 +3,21 @@
 // DESIGN.md readings R2, R3, R23, R24.
 //
 // HBM layout of the environment state: one contiguous record per env,
-//   [ header | issue list | hot[RCAP] | r_dl[RCAP] | r_issue[RCAP] | r_tok[RCAP] | r_aux[RCAP] | q[QCAP] (uint4) ]
-// so that the group of lanes that owns an env streams `header` and `hot[0..hwm)` with 128-bit coalesced loads and
-// touches the cold arrays only for the few requests that change state in a tick.
-//   header (u32 words): m[N] as uint4 {n_wait, n_run, kv_used, ewma_q8} | rfree[RW] | qfree[QW] | qready[QW] |
-//                       misc[4] {drops, icnt, -, -} | counters u64[16]
-//   hot[i]   = remaining(16) | state(2)<<16 | model(4)<<18        — the only per-request word the service phase touches
-//   r_tok[i] = out_total | in_tok<<16 ; r_aux[i] = model<<2 | depth<<6 | agent<<8 | succ<<10 | query<<16
+//   [ header | issue list | hot[SP] | cold[SP] (uint2) | wkey[RCAP] | waux[RCAP] (uint2) | q[QCAP] (uint4) ]
+// SP = sum over models of ceil8(S_k): the slots of all models, numbered consecutively (R10).  The group of lanes
+// that owns an env streams `header` and `hot` with 128-bit coalesced loads and touches the other arrays only for the
+// few requests that change state in a tick.
+//   header (u32 words): m[N] as uint4 {n_wait, n_run, kv_used, ewma_q8} | occ[N] (u64: bit s = slot s taken) |
+//                       qfree[QW] | qready[QW] | misc[4] {drops, icnt, nw, -} | counters u64[16]
+//   hot[gs]  = remaining(16) | id<<16, id = 4*query + agent   — the only per-request word the service phase touches
+//   cold[gs] = {issue(16) | deadline<<16, sw}      sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
+//   wkey[j]  = model<<28 | time(16)<<12 | id       time = deadline (EDF) or issue tick (FCFS): one u32 compare orders
+//                                                   the waiting list by (model, R20 key)
+//   waux[j]  = {issue(16) | remaining<<16, sw}
+//   issue[j] = {wkey, sw}                          written by the executor kernel, appended to the list in phase D
 //   q[i]     = {plan word, budget | in_tok<<16, deadline, arrive}
-// Free slots are defined by the bitmaps (a set bit = free); arrays of free slots hold stale data.
+// The waiting list wkey/waux[0..nw) is compact and unordered; free query slots are defined by the qfree bitmap and
+// free service slots by occ (their words hold stale data).  Absolute ticks are < 65536 on the device.
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
@@ -25,7 +31,7 @@ constexpr uint32_t kDtUs = 50000;
 constexpr uint32_t kIssueCap = 128;      // issue records per env per tick (31 arrivals x 3 calls + continuing stages)
 
 constexpr uint32_t ST_FREE = 0, ST_WAIT = 1, ST_RUN = 2;
-constexpr uint32_t HOT_STATE_SHIFT = 16, HOT_MODEL_SHIFT = 18;
+constexpr uint32_t SW_IN_SHIFT = 13, SW_SUCC_SHIFT = 26, SW_DEPTH_SHIFT = 27, SW_TOK_MASK = 0x1FFFu;
 // query plan word: live0 planned1 topo2-3 cnt4-5 keff6-8 stage9-11 nst12-14 pending15-16 solved17 roles18-25
 constexpr uint32_t QP_LIVE = 1u, QP_PLANNED = 2u;
 constexpr uint32_t QP_PEND_SHIFT = 15, QP_SUCC_SHIFT = 17, QP_ROLE_SHIFT = 18;
@@ -64,17 +70,18 @@ struct QLog {
 };
 
 struct Params {
-    uint32_t E, N, QCAP, RCAP, QW, RW;
+    uint32_t E, N, QCAP, RCAP, QW, SP;                 // SP = padded slot count of the pool
     uint32_t sched_mode, kv_preempt, cost_mode, episode_ticks, budget_norm, in_tok_const, mix_thresh, env_id_base;
     uint32_t mix_lo[2], mix_hi[2], depth_median[3];
     uint32_t flags, has_intok, seed_lo, seed_hi;
     uint32_t f_in, hidden, log_mode, pad0;
     ModelTab model[kMaxModels];
+    uint32_t slot_base[kMaxModels + 1];      // first global slot of each model (multiples of 8)
     // per-env record
     uint8_t *env_base;
     unsigned long long env_stride;           // bytes, multiple of 128
-    uint32_t hw_rfree, hw_qfree, hw_qready, hw_misc, hw_ctr, hdr_words;   // header word offsets (m at word 0)
-    uint32_t off_iss, off_hot, off_dl, off_issue, off_tok, off_aux, off_q; // byte offsets inside the record
+    uint32_t hw_occ, hw_qfree, hw_qready, hw_misc, hw_ctr, hdr_words;     // header word offsets (m at word 0)
+    uint32_t off_iss, off_hot, off_cold, off_wkey, off_waux, off_q;       // byte offsets inside the record
     float *snap;                             // [E][3N] telemetry features of the current tick (R14)
     const uint32_t *tab_mult, *tab_intok, *tab_cdf;
     const uint8_t *env_level;

@@ -99,9 +99,9 @@ __device__ __forceinline__ uint32_t sample_seq(const float *l, float *e, uint32_
     return a;
 }
 
-// executor decision -> log row + one issue record of its env (R18): the simulation kernel only has to give the
-// request its canonical pool index.
-__device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, const Ph4 &d, uint32_t act, float logp, float value)
+// executor decision -> log row + one issue record of its env (R18): {waiting-list key, static word} (im_device.cuh);
+// phase D of the simulation kernel appends it to the env's waiting list.
+__device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, const Ph4 &d, uint32_t act, float logp, float value, int32_t t)
 {
     const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
     if (P.log_mode) {
@@ -115,9 +115,11 @@ __device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, 
     const uint32_t succ = d.z < P.model[model].succ[depth] ? 1u : 0u;
     uint8_t *rec = env_rec(P, ri.env);
     const uint32_t slot = atomicAdd(reinterpret_cast<uint32_t *>(rec) + P.hw_misc + 1, 1u);
+    const uint32_t tm = (uint32_t)(P.sched_mode ? ri.dl : t) & 0xFFFFu;             // R20: deadline (EDF) or issue tick (FCFS)
     if (slot < kIssueCap)
-        reinterpret_cast<uint4 *>(rec + P.off_iss)[slot] =
-            make_uint4(out_total | ((ri.c & 0xFFFFu) << 16), (model << 2) | (depth << 6) | (agent << 8) | (succ << 10) | (q << 16), (uint32_t)ri.dl, 0u);
+        reinterpret_cast<uint2 *>(rec + P.off_iss)[slot] =
+            make_uint2((model << 28) | (tm << 12) | (q << 2) | agent,
+                       out_total | ((ri.c & 0xFFFFu) << SW_IN_SHIFT) | (succ << SW_SUCC_SHIFT) | (depth << SW_DEPTH_SHIFT));
     else
         atomicOr(P.err_flag, 4u);
 }
@@ -135,7 +137,7 @@ __device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri
     const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
     float logp;
     const uint32_t act = sample_seq(logits, scratch, n, u24(d.x), logp);
-    exec_commit(P, ri, d, act, logp, value);
+    exec_commit(P, ri, d, act, logp, value, t);
 }
 
 // planner decision -> log row, plan word of the query and the stage-0 executor rows (R17)
@@ -641,7 +643,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
                     const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
                     float logp;
                     const uint32_t act = sample_reg<48, NO>(l, 0, n, u24(d.x), logp);
-                    exec_commit(P, ri, d, act, logp, value);
+                    exec_commit(P, ri, d, act, logp, value, t);
                 }
             } else {
                 if (P.plan.logits) {

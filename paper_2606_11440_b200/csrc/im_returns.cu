@@ -118,46 +118,29 @@ int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Slack-ordered queue (R20): per env, all WAITING requests sorted by (model, key) with a warp-level segmented bitonic
-// sort — shared-memory staging, strides >= 32 exchanged through shared memory, strides < 32 by warp shuffles.
-// Serves IM_TEL_QUEUE_ORDER; the admission phase of k_sim extracts only the few smallest keys it can admit.
+// Slack-ordered queue (R20): per env, the waiting list sorted with a warp-level bitonic sort — shared-memory staging,
+// strides >= 32 exchanged through shared memory, strides < 32 by warp shuffles.  The list key is
+// model<<28 | time<<12 | id (im_device.cuh), so ONE u32 sort yields every model's queue in slack order, segment after
+// segment.  Serves IM_TEL_QUEUE_ORDER; the admission phase of k_sim extracts only the few smallest keys it can admit.
 // ------------------------------------------------------------------------------------------------------------------
 constexpr int kQoWarps = 4;
 
 __global__ void __launch_bounds__(kQoWarps * 32)
 k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
 {
-    extern __shared__ __align__(16) unsigned long long s_keys[];
+    extern __shared__ __align__(16) uint32_t s_keys[];
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const uint32_t e = blockIdx.x * kQoWarps + wib;
     if (e >= P.E) return;
     uint32_t n2cap = 32;
     while (n2cap < P.RCAP) n2cap <<= 1;
-    unsigned long long *keys = s_keys + (size_t)wib * n2cap;
+    uint32_t *keys = s_keys + (size_t)wib * n2cap;
     const uint8_t *rec = env_rec(P, e);
-    const uint32_t *hot = (const uint32_t *)(rec + P.off_hot), *rfree = (const uint32_t *)rec + P.hw_rfree;
-    const int32_t *r_dl = (const int32_t *)(rec + P.off_dl), *r_issue = (const int32_t *)(rec + P.off_issue);
-    uint32_t n = 0;
-    uint32_t per_model = 0;                       // lane k counts model k
-    for (uint32_t i0 = 0; i0 < P.RCAP; i0 += 32) {
-        const uint32_t i = i0 + lane;
-        const uint32_t m = hot[i] >> HOT_STATE_SHIFT;          // state | model << 2 (stale words of free slots are masked)
-        const bool w = (m & 3u) == ST_WAIT && !((rfree[i >> 5] >> (i & 31)) & 1u);
-        const uint32_t bal = __ballot_sync(0xffffffffu, w);
-        if (w) {
-            const int32_t base = P.sched_mode ? r_dl[i] : r_issue[i];
-            const uint32_t key = ((uint32_t)(base - t + (1 << 19)) << 12) | i;
-            keys[n + __popc(bal & ((1u << lane) - 1u))] = ((unsigned long long)((m >> 2) & 15u) << 32) | key;
-        }
-        for (uint32_t k = 0; k < P.N; k++) {
-            const uint32_t c = __popc(__ballot_sync(0xffffffffu, w && ((m >> 2) & 15u) == k));
-            if (lane == k) per_model += c;
-        }
-        n += __popc(bal);
-    }
+    const uint32_t *hdr = (const uint32_t *)rec, *wkey = (const uint32_t *)(rec + P.off_wkey);
+    const uint32_t n = min(hdr[P.hw_misc + 2], P.RCAP);
     uint32_t n2 = 32;
     while (n2 < n) n2 <<= 1;
-    for (uint32_t i = n + lane; i < n2; i += 32) keys[i] = ~0ull;
+    for (uint32_t i = lane; i < n2; i += 32) keys[i] = i < n ? wkey[i] : 0xFFFFFFFFu;
     __syncwarp();
     for (uint32_t k = 2; k <= n2; k <<= 1) {
         uint32_t j = k >> 1;
@@ -165,7 +148,7 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
             for (uint32_t i = lane; i < n2; i += 32) {
                 const uint32_t p = i ^ j;
                 if (p > i) {
-                    const unsigned long long a = keys[i], b = keys[p];
+                    const uint32_t a = keys[i], b = keys[p];
                     const bool up = (i & k) == 0;
                     if ((a > b) == up) { keys[i] = b; keys[p] = a; }
                 }
@@ -174,10 +157,10 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
         }
         for (uint32_t it = 0; it < n2; it += 32) { // warp-shuffle exchanges within 32 consecutive keys
             const uint32_t i = it + lane;
-            unsigned long long v = keys[i];
+            uint32_t v = keys[i];
             const bool up = (i & k) == 0;
             for (uint32_t jj = j; jj > 0; jj >>= 1) {
-                const unsigned long long o = __shfl_xor_sync(0xffffffffu, v, jj);
+                const uint32_t o = __shfl_xor_sync(0xffffffffu, v, jj);
                 const bool lower = (lane & jj) == 0;
                 v = (lower == up) ? (v < o ? v : o) : (v > o ? v : o);
             }
@@ -186,17 +169,18 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
         __syncwarp();
     }
     uint32_t *o = out + (size_t)e * (P.N + 1 + P.RCAP);
+    const uint32_t per_model = lane < P.N ? hdr[4 * lane] : 0u;               // n_wait of model `lane`
     const uint32_t inc = [&] { uint32_t v = per_model; for (int s = 1; s < 32; s <<= 1) { const uint32_t u = __shfl_up_sync(0xffffffffu, v, s); if (lane >= (uint32_t)s) v += u; } return v; }();
     if (lane < P.N) o[lane + 1] = inc;
     if (lane == 0) o[0] = 0;
-    for (uint32_t i = lane; i < P.RCAP; i += 32) o[P.N + 1 + i] = i < n ? (uint32_t)(keys[i] & 0xFFFu) : 0xFFFFFFFFu;
+    for (uint32_t i = lane; i < P.RCAP; i += 32) o[P.N + 1 + i] = i < n ? (keys[i] & 0xFFFu) : 0xFFFFFFFFu;
 }
 
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st)
 {
     uint32_t n2cap = 32;
     while (n2cap < P.RCAP) n2cap <<= 1;
-    const size_t smem = (size_t)kQoWarps * n2cap * 8;
+    const size_t smem = (size_t)kQoWarps * n2cap * 4;
     cudaFuncSetAttribute(k_queue_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_queue_order<<<(P.E + kQoWarps - 1) / kQoWarps, kQoWarps * 32, smem, st>>>(P, t, out);
     return 1;

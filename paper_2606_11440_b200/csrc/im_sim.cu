@@ -1,21 +1,21 @@
-// im_sim.cu — the fixed-tick simulation kernel: one group of G lanes (a warp or a half-warp) per environment.
+// im_sim.cu — the fixed-tick simulation kernel: one group of G lanes (a half-warp) per environment.
 //
 // One launch runs, for every env, the environment half of the canonical tick:
-//   post(t):  D-issue (requests of the decisions the executor kernel took for tick t), E admit (slack-ordered
-//             queue, R20/R21), F serve (token-level service, R11), G complete (latency, cost, EWMA, finalise,
-//             R13/R27/R28), H preempt (R21), I record (R27/R28/R33)
+//   post(t):  D-issue (the calls the executor kernel decided for tick t join the waiting list), E admit
+//             (slack-ordered queue, R20/R21), F serve (token-level service, R11), G complete (latency, cost, EWMA,
+//             finalise, R13/R27/R28), H preempt (R21), I record (R27/R28/R33)
 //   pre(t+1): A arrive (Poisson count, budgets, input tokens; R5-R9), B snapshot (R14), and the emission of the
 //             work lists: one planner row per new query, executor rows for every query whose previous stage
 //             completed (R17).
 // The decision half (C plan, D decide) runs between two launches in im_policy.cu.
 //
-// Shape of the work: the only O(pool) work of a tick is ONE streaming pass over hot[0..hwm) —
-// 128-bit coalesced loads, one Philox call per 4 slots — which serves every RUNNING request, buckets the WAITING
-// requests of the models that can admit, and lists the requests that completed.  Everything else (issue, admission,
-// completion, preemption, arrivals) touches only the few requests that change state, in batches across the lanes so
-// that a phase costs one memory round trip, not one per request.  Order-dependent definitions (j-th new item takes the
-// j-th lowest free index, R9/R18; smallest key first, R20) are computed by ranked selection / repeated arg-min, every
-// accumulation is an integer sum, so lanes may commit in any order (R12, R13, R28).
+// Shape of the work: the only O(pool) work of a tick is ONE streaming pass over hot[0..SP), the
+// per-model service slots (R10) — 128-bit coalesced loads, a lane owns 8 consecutive slots of ONE model, one Philox
+// call per 8 slots (sixteen-bit fields, R2/R11), no per-slot decode.  Everything else (issue, admission, completion,
+// preemption, arrivals) touches only the few requests that change state.  The waiting list is a compact unordered
+// array of u32 keys model|time|id: admission takes per-model minima of it (all admitting models in parallel, one lane
+// per model), removal fills the holes from the tail.  Every accumulation is an integer sum, so lanes may commit in any
+// order (R12, R13, R28).
 #include "im_device.cuh"
 
 namespace im {
@@ -24,20 +24,20 @@ constexpr int kSimThreads = 128;
 
 // ---- per-group shared memory layout (bytes)
 struct SimLayout {
-    uint32_t o_hdr, o_prefA, o_prefB, o_small, o_bucket, o_clist, total;
+    uint32_t o_hdr, o_pref, o_small, o_clist, total;
 };
-constexpr uint32_t kSmallWords = 9 * 16 + 8;
-__host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t RW, uint32_t QW, uint32_t RCAP, uint32_t G)
+// small per-env arrays (u32 words): 16 per model-indexed array
+enum : uint32_t { SM_LATSUM = 0, SM_LATN = 16, SM_RELKV = 32, SM_RELNRUN = 48, SM_KVADD = 64, SM_OCCCLR = 80, SM_AMIN = 112,
+                  SM_AIDX = 128, SM_ALAST = 144, SM_CTR = 160, SM_SC = 176, SM_RM = 184, SM_MV = 200, kSmallWords = 216 };
+__host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW, uint32_t G)
 {
     auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
     SimLayout L;
     uint32_t o = 0;
     L.o_hdr = o; o += up(hdr_words * 4);
-    L.o_prefA = o; o += up((RW + 1) * 4);
-    L.o_prefB = o; o += up((QW + 1) * 4);
+    L.o_pref = o; o += up((QW + 1) * 4);
     L.o_small = o; o += up(kSmallWords * 4);
-    L.o_bucket = o; o += up(RCAP * 2);
-    L.o_clist = o; o += up(5 * G * 2);
+    L.o_clist = o; o += up(9 * G * 4);
     L.total = o;
     return L;
 }
@@ -52,7 +52,6 @@ struct Grp {
     }
     template <typename T> __device__ __forceinline__ T shfl(T v, int src) const { return __shfl_sync(gmask, v, src, G); }
     template <typename T> __device__ __forceinline__ T shfl_up(T v, int d) const { return __shfl_up_sync(gmask, v, d, G); }
-    template <typename T> __device__ __forceinline__ T shfl_xor(T v, int d) const { return __shfl_xor_sync(gmask, v, d, G); }
     __device__ __forceinline__ void sync() const { __syncwarp(gmask); }
     __device__ __forceinline__ uint32_t incl_scan(uint32_t v) const
     {
@@ -61,7 +60,6 @@ struct Grp {
         return v;
     }
     __device__ __forceinline__ uint32_t sum(uint32_t v) const { return __reduce_add_sync(gmask, v); }
-    __device__ __forceinline__ uint32_t umin(uint32_t v) const { return __reduce_min_sync(gmask, v); }
     __device__ __forceinline__ uint32_t umax(uint32_t v) const { return __reduce_max_sync(gmask, v); }
 };
 
@@ -93,18 +91,33 @@ __device__ __forceinline__ uint32_t find_nth(const uint32_t *bm, uint32_t nw, co
     return lo * 32 + __fns(bm[lo], 0, (int)(j - pref[lo]) + 1);
 }
 
+// sixteen-bit field f (0..7) of a Philox output (R2: word f>>1, low half first)
+__device__ __forceinline__ uint32_t u16_field(const Ph4 &u, uint32_t f)
+{
+    const uint32_t w = (f >> 1) == 0 ? u.x : ((f >> 1) == 1 ? u.y : ((f >> 1) == 2 ? u.z : u.w));
+    return (f & 1u) ? (w >> 16) : (w & 0xFFFFu);
+}
+
 // tick arguments: t_post < 0 => no post phases; pre_mode 0 none, 1 full (A, B, rows), 2 snapshot only
 template <int G>
-__global__ void __launch_bounds__(kSimThreads)
+__global__ void __launch_bounds__(kSimThreads, 8)
 k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ ModelTab s_model[kMaxModels];
-    __shared__ uint32_t s_base[kMaxModels], s_frac[kMaxModels];
+    __shared__ uint32_t s_base[kMaxModels], s_thr[kMaxModels], s_sbase[kMaxModels + 1];
+    __shared__ uint8_t s_gmodel[128];                                       // group of 8 slots -> model
     if (threadIdx.x < P.N) {
         s_model[threadIdx.x] = P.model[threadIdx.x];
-        const uint32_t x = P.model[threadIdx.x].rate * kDtUs;            // rate <= 80000 => fits 32 bits
-        s_base[threadIdx.x] = x / 1000000u; s_frac[threadIdx.x] = x % 1000000u;
+        const uint32_t x = P.model[threadIdx.x].rate * kDtUs;               // rate <= 80000 => fits 32 bits
+        s_base[threadIdx.x] = x / 1000000u;
+        s_thr[threadIdx.x] = (uint32_t)(((unsigned long long)(x % 1000000u) << 16) / 1000000u);   // R11: Bernoulli to 2^-16
+    }
+    if (threadIdx.x <= kMaxModels) s_sbase[threadIdx.x] = P.slot_base[threadIdx.x];
+    if (threadIdx.x < (P.SP >> 3)) {
+        uint32_t k = 0;
+        while (P.slot_base[k + 1] <= threadIdx.x * 8) k++;
+        s_gmodel[threadIdx.x] = (uint8_t)k;
     }
     __syncthreads();
     constexpr uint32_t GPB = kSimThreads / G;
@@ -112,28 +125,29 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     g.lane = threadIdx.x & 31; g.gl = threadIdx.x % G; g.gbase = g.lane - g.gl;
     g.gmask = G == 32 ? 0xffffffffu : (((1u << (G & 31)) - 1u) << g.gbase);
     const uint32_t gl = g.gl;
+    const uint32_t lt_mask = (1u << gl) - 1u;
     const uint32_t e = blockIdx.x * GPB + threadIdx.x / G;
     if (e >= P.E) return;
     const uint32_t gid = P.env_id_base + e;
-    const uint32_t N = P.N, RW = P.RW, QW = P.QW, RCAP = P.RCAP, QCAP = P.QCAP;
+    const uint32_t N = P.N, QW = P.QW, QCAP = P.QCAP;
     const uint32_t region = e % kRegions;
 
-    const SimLayout L = sim_layout(P.hdr_words, RW, QW, RCAP, G);
+    const SimLayout L = sim_layout(P.hdr_words, QW, G);
     unsigned char *sm = smem_raw + (size_t)(threadIdx.x / G) * L.total;
     uint32_t *s_hdr = (uint32_t *)(sm + L.o_hdr);
-    uint32_t *s_rfree = s_hdr + P.hw_rfree, *s_qfree = s_hdr + P.hw_qfree, *s_qready = s_hdr + P.hw_qready, *s_misc = s_hdr + P.hw_misc;
-    uint32_t *prefA = (uint32_t *)(sm + L.o_prefA), *prefB = (uint32_t *)(sm + L.o_prefB);
+    uint32_t *s_occ = s_hdr + P.hw_occ, *s_qfree = s_hdr + P.hw_qfree, *s_qready = s_hdr + P.hw_qready, *s_misc = s_hdr + P.hw_misc;
+    uint32_t *prefB = (uint32_t *)(sm + L.o_pref);
     uint32_t *s_small = (uint32_t *)(sm + L.o_small);
-    uint32_t *s_boff = s_small, *s_bcnt = s_small + 16, *s_latsum = s_small + 32, *s_latn = s_small + 48;
-    int32_t *s_kvcorr = (int32_t *)(s_small + 64);
-    uint32_t *s_relkv = s_small + 80, *s_relnrun = s_small + 96, *s_ext = s_small + 112, *s_ctr = s_small + 128;
-    uint32_t *s_sc = s_small + 144;                  // [0] ccnt, [1] rew, [2] miss, [4..5] cost (u64)
+    uint32_t *s_latsum = s_small + SM_LATSUM, *s_latn = s_small + SM_LATN, *s_relkv = s_small + SM_RELKV, *s_relnrun = s_small + SM_RELNRUN;
+    uint32_t *s_kvadd = s_small + SM_KVADD, *s_occclr = s_small + SM_OCCCLR, *s_amin = s_small + SM_AMIN, *s_aidx = s_small + SM_AIDX;
+    uint32_t *s_alast = s_small + SM_ALAST, *s_ctr = s_small + SM_CTR, *s_rm = s_small + SM_RM, *s_mv = s_small + SM_MV;
+    uint32_t *s_sc = s_small + SM_SC;                 // [0] ccnt, [1] rew, [2] miss, [3] removals, [4..5] cost (u64)
     unsigned long long *s_cost = (unsigned long long *)(s_sc + 4);
-    uint16_t *s_bucket = (uint16_t *)(sm + L.o_bucket), *s_clist = (uint16_t *)(sm + L.o_clist);
+    uint32_t *s_clist = (uint32_t *)(sm + L.o_clist); // completed requests: global slot | id << 16
 
     uint8_t *rec = env_rec(P, e);
-    uint32_t *hot = (uint32_t *)(rec + P.off_hot), *r_tok = (uint32_t *)(rec + P.off_tok), *r_aux = (uint32_t *)(rec + P.off_aux);
-    int32_t *r_dl = (int32_t *)(rec + P.off_dl), *r_issue = (int32_t *)(rec + P.off_issue);
+    uint32_t *hot = (uint32_t *)(rec + P.off_hot), *wkey = (uint32_t *)(rec + P.off_wkey);
+    uint2 *cold = (uint2 *)(rec + P.off_cold), *waux = (uint2 *)(rec + P.off_waux);
     uint4 *qtab = (uint4 *)(rec + P.off_q);
 
     // ---- load the header
@@ -177,20 +191,20 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             const uint32_t ccnt = s_sc[0];
             const uint32_t nb = ccnt < (uint32_t)G ? ccnt : (uint32_t)G;
             const bool act = gl < nb;
-            uint32_t q = 0x10000u + gl, model = 0, succ = 0;
+            uint32_t q = 0x10000u + gl, succ = 0;
             uint4 qr = make_uint4(0, 0, 0, 0);
             if (act) {
                 const uint32_t ent = s_clist[ccnt - nb + gl];
-                const uint32_t ridx = ent & 0xFFFu;
-                model = ent >> 12;
-                const int32_t issue = r_issue[ridx];
-                const uint32_t tk = r_tok[ridx], aux = r_aux[ridx];
-                q = aux >> 16; succ = (aux >> 10) & 1u;
+                const uint32_t gs = ent & 0xFFFFu, model = s_gmodel[gs >> 3], sl = gs - s_sbase[model];
+                q = ent >> 18;                                               // id = 4 q + agent
+                const uint2 cd = cold[gs];
                 qr = qtab[q];
-                const uint32_t ell = (uint32_t)(t + 1 - issue);
+                succ = (cd.y >> SW_SUCC_SHIFT) & 1u;
+                const uint32_t ell = (uint32_t)(t + 1) - (cd.x & 0xFFFFu);
                 atomicAdd(s_cost, ((unsigned long long)ell << 16) / (qr.y & 0xFFFFu));   // C_k = l_k / beta, Q16 (R28)
                 atomicAdd(&s_latsum[model], ell); atomicAdd(&s_latn[model], 1u);
-                atomicAdd(&s_relkv[model], (tk >> 16) + (tk & 0xFFFFu)); atomicAdd(&s_relnrun[model], 1u);
+                atomicAdd(&s_relkv[model], (cd.y & SW_TOK_MASK) + ((cd.y >> SW_IN_SHIFT) & SW_TOK_MASK)); atomicAdd(&s_relnrun[model], 1u);
+                atomicOr(&s_occclr[2 * model + (sl >> 5)], 1u << (sl & 31));  // the slot is free from the next tick on
                 atomicAdd(&s_ctr[C_CALLS_DONE], 1u);
             }
             // calls of one query that complete in the same tick are folded by the lowest lane holding them
@@ -222,7 +236,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                     atomicAdd(&s_sc[1], solved); atomicAdd(&s_sc[2], late);
                     atomicAdd(&s_ctr[C_FINISHED], 1u); atomicAdd(&s_ctr[C_SOLVED], solved); atomicAdd(&s_ctr[C_MISSED], late);
                     atomicAdd(&s_ctr[C_SUM_SOJOURN], sojourn);
-                    const uint32_t li = lbase + __popc(finm & ((1u << gl) - 1u));
+                    const uint32_t li = lbase + __popc(finm & lt_mask);
                     P.qlog.rec[(size_t)region * P.qlog.regcap + (li % P.qlog.regcap)] =
                         make_uint4(gid, qr.w, sojourn, (qr.y & 0xFFFFu) | (solved << 16) | (((pw >> 2) & 3u) << 17) | (((pw >> 6) & 7u) << 19));
                     atomicOr(&s_qfree[q >> 5], 1u << (q & 31));
@@ -234,197 +248,159 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             g.sync();
         };
 
-        // =============================================================== D-issue (R18): canonical request indices
+        // =============================================================== D-issue (R18): the new calls join the waiting list
         const uint32_t icnt = min(s_misc[1], kIssueCap);        // the executor kernel flags an overflow (err_flag)
         if (icnt) {
-            const uint4 *iss = (const uint4 *)(rec + P.off_iss);
-            build_prefix(g, s_rfree, RW, prefA);
-            uint16_t *skey = s_bucket;                        // scratch: (q << 2 | agent) of every record
-            for (uint32_t j = gl; j < icnt; j += G) { const uint32_t aux = iss[j].y; skey[j] = (uint16_t)(((aux >> 16) << 2) | ((aux >> 8) & 3u)); }
-            g.sync();
-            for (uint32_t j = gl; j < icnt; j += G) {
-                const uint4 r = iss[j];
-                const uint32_t key = skey[j];
-                uint32_t rank = 0;
-                for (uint32_t i = 0; i < icnt; i++) rank += skey[i] < key ? 1u : 0u;
-                const uint32_t ridx = find_nth(s_rfree, RW, prefA, rank);
-                const uint32_t model = (r.y >> 2) & 15u;
-                r_tok[ridx] = r.x; r_aux[ridx] = r.y; r_dl[ridx] = (int32_t)r.z; r_issue[ridx] = t;
-                hot[ridx] = (r.x & 0xFFFFu) | (ST_WAIT << HOT_STATE_SHIFT) | (model << HOT_MODEL_SHIFT);
-                atomicAdd(&M_NWAIT(model), 1u);
-            }
-            g.sync();
-            // the icnt lowest free indices are exactly the ones taken: clear them word by word
-            for (uint32_t w = gl; w < RW; w += G) {
-                const uint32_t before = prefA[w], cntw = prefA[w + 1] - before;
-                if (before < icnt) {
-                    const uint32_t take = min(icnt - before, cntw);
-                    uint32_t bm = s_rfree[w];
-                    if (take == cntw) bm = 0; else for (uint32_t i = 0; i < take; i++) bm &= bm - 1;
-                    s_rfree[w] = bm;
+            const uint2 *iss = (const uint2 *)(rec + P.off_iss);
+            const uint32_t nw0 = s_misc[2];
+            if (nw0 + icnt > P.RCAP) { if (gl == 0) atomicOr(P.err_flag, 8u); }      // cannot happen: rcap >= 3 qcap (R9)
+            else
+                for (uint32_t j = gl; j < icnt; j += G) {
+                    const uint2 r = iss[j];
+                    wkey[nw0 + j] = r.x;
+                    waux[nw0 + j] = make_uint2(((uint32_t)t & 0xFFFFu) | ((r.y & SW_TOK_MASK) << 16), r.y);   // issue = t, remaining = out_total
+                    atomicAdd(&M_NWAIT(r.x >> 28), 1u);
                 }
-            }
-            if (gl == 0) { s_ctr[C_ISSUED] += icnt; s_ctr[C_EXEC_DEC] += icnt; s_misc[1] = 0; }
+            g.sync();
+            if (gl == 0) { s_ctr[C_ISSUED] += icnt; s_ctr[C_EXEC_DEC] += icnt; s_misc[1] = 0; s_misc[2] = nw0 + icnt; }
             g.sync();
         }
-        // high-water mark of the request pool (highest occupied index + 1)
-        uint32_t hwm = 0;
-        for (uint32_t w = gl; w < RW; w += G) {
-            const uint32_t occ = ~s_rfree[w];
-            if (occ) hwm = max(hwm, w * 32 + 32 - __clz(occ));
-        }
-        hwm = g.umax(hwm);
-        const uint32_t n_chunks = (hwm + 4 * G - 1) / (4 * G);
 
-        // models that can admit (R21) and the offsets of their buckets
-        const bool adm = gl < N && M_NWAIT(gl) > 0 && M_NRUN(gl) < s_model[gl].slots && M_KV(gl) <= s_model[gl].kv_cap;
-        const uint32_t madm = g.ballot(adm);
-        const uint32_t nrun_pre = gl < N ? M_NRUN(gl) : 0u;
-        {
-            const uint32_t nw = adm ? M_NWAIT(gl) : 0u;
-            const uint32_t inc = g.incl_scan(nw);
-            if (gl < 16) s_boff[gl] = inc - nw;
-        }
-        g.sync();
+        // models that can admit (R21), judged on the state before this tick's service
+        const uint32_t madm = g.ballot(gl < N && M_NWAIT(gl) > 0 && M_NRUN(gl) < s_model[gl].slots && M_KV(gl) <= s_model[gl].kv_cap);
 
-        // =============================================================== F serve (R11): one streaming pass over hot[0..hwm)
-        unsigned long long ext_lo = 0, ext_hi = 0;             // per-lane count of stochastic extra tokens, 8 bits per model
+        // =============================================================== F serve (R11): one streaming pass over the slots
         {
             uint4 *hot4 = (uint4 *)hot;
-            uint4 hn = make_uint4(0, 0, 0, 0);
-            if (n_chunks) hn = hot4[gl];
-            for (uint32_t c = 0; c < n_chunks; c++) {
-                const uint32_t i0 = (c * G + gl) * 4;
-                const uint4 h4 = hn;
-                if (c + 1 < n_chunks) hn = hot4[(c + 1) * G + gl];
-                uint32_t hh[4] = {h4.x, h4.y, h4.z, h4.w};
-                {   // free slots are defined by the bitmap: their words may be stale (reset, episode boundary)
-                    const uint32_t fr = s_rfree[i0 >> 5] >> (i0 & 31);
+            const uint32_t n_grp = P.SP >> 3;
+            auto occ8_of = [&](uint32_t gi) -> uint32_t {
+                const uint32_t k = s_gmodel[gi], sl0 = gi * 8 - s_sbase[k];       // first slot of the group within its model
+                return (s_occ[2 * k + (sl0 >> 5)] >> (sl0 & 31)) & 0xFFu;
+            };
+            uint4 na = make_uint4(0, 0, 0, 0), nb = na;
+            uint32_t nocc = 0;
+            if (gl < n_grp) { nocc = occ8_of(gl); if (nocc) { na = hot4[2 * gl]; nb = hot4[2 * gl + 1]; } }
+            for (uint32_t g0 = 0; g0 < n_grp; g0 += G) {
+                const uint32_t gi = g0 + gl;
+                const uint4 ha = na, hb = nb;
+                const uint32_t occ8 = nocc;
+                nocc = 0;
+                if (gi + G < n_grp) { nocc = occ8_of(gi + G); if (nocc) { na = hot4[2 * (gi + G)]; nb = hot4[2 * (gi + G) + 1]; } }
+                if (occ8) {
+                    const uint32_t k = s_gmodel[gi], base = s_base[k], thr = s_thr[k];
+                    const Ph4 u4 = draw(P, STREAM_SVC, gid, t, gi, 0);
+                    const uint32_t uw[4] = {u4.x, u4.y, u4.z, u4.w};
+                    uint32_t hh[8] = {ha.x, ha.y, ha.z, ha.w, hb.x, hb.y, hb.z, hb.w};
+                    uint32_t tot = 0;
 #pragma unroll
-                    for (int s = 0; s < 4; s++) if ((fr >> s) & 1u) hh[s] = 0;
-                }
-                const uint32_t stor = (hh[0] | hh[1] | hh[2] | hh[3]) >> HOT_STATE_SHIFT;   // any non-free slot?
-                bool dirty = false;
-                if (stor & 3u) {
-                    const bool any_run = (((hh[0] >> 17) | (hh[1] >> 17) | (hh[2] >> 17) | (hh[3] >> 17)) & 1u) != 0;
-                    Ph4 u4 = Ph4{0, 0, 0, 0};
-                    if (any_run) u4 = draw(P, STREAM_SVC, gid, t, i0 >> 2, 0);
-                    const uint32_t uu[4] = {u4.x, u4.y, u4.z, u4.w};
-#pragma unroll
-                    for (int s = 0; s < 4; s++) {
-                        const uint32_t w = hh[s];
-                        const uint32_t st = (w >> HOT_STATE_SHIFT) & 3u, model = (w >> HOT_MODEL_SHIFT) & 15u;
-                        if (st == ST_RUN) {
-                            const uint32_t rem = w & 0xFFFFu;
-                            const uint32_t extra = __umulhi(uu[s], 1000000u) < s_frac[model] ? 1u : 0u;
-                            const uint32_t tok = s_base[model] + extra;
-                            if (model < 8) ext_lo += (unsigned long long)extra << (8 * model); else ext_hi += (unsigned long long)extra << (8 * (model - 8));
+                    for (int s = 0; s < 8; s++) {
+                        if ((occ8 >> s) & 1u) {
+                            const uint32_t w = hh[s], rem = w & 0xFFFFu;
+                            const uint32_t u16 = (s & 1) ? (uw[s >> 1] >> 16) : (uw[s >> 1] & 0xFFFFu);
+                            const uint32_t tok = base + (u16 < thr ? 1u : 0u);
                             if (tok >= rem) {                                    // completes: only `rem` tokens are decoded
-                                if (tok != rem) atomicAdd(&s_kvcorr[model], (int32_t)rem - (int32_t)tok);
-                                const uint32_t pos = atomicAdd(&s_sc[0], 1u);
-                                s_clist[pos] = (uint16_t)((model << 12) | (i0 + s));
-                                atomicOr(&s_rfree[(i0 + s) >> 5], 1u << ((i0 + s) & 31));
-                                hh[s] = 0;
+                                tot += rem;
+                                s_clist[atomicAdd(&s_sc[0], 1u)] = (gi * 8 + s) | (w & 0xFFFF0000u);
+                                hh[s] = w & 0xFFFF0000u;
                             } else {
+                                tot += tok;
                                 hh[s] = w - tok;
                             }
-                            dirty = true;
-                        } else if (st == ST_WAIT && ((madm >> model) & 1u)) {
-                            const uint32_t pos = s_boff[model] + atomicAdd(&s_bcnt[model], 1u);
-                            s_bucket[pos] = (uint16_t)((model << 12) | (i0 + s));
                         }
                     }
+                    atomicAdd(&s_kvadd[k], tot);
+                    hot4[2 * gi] = make_uint4(hh[0], hh[1], hh[2], hh[3]);
+                    hot4[2 * gi + 1] = make_uint4(hh[4], hh[5], hh[6], hh[7]);
                 }
-                if (dirty) hot4[c * G + gl] = make_uint4(hh[0], hh[1], hh[2], hh[3]);
                 g.sync();
                 while (s_sc[0] >= (uint32_t)G) flush();
             }
         }
-        // per-model totals of the extra tokens
-        {
-            const uint32_t lo0 = (uint32_t)ext_lo, lo1 = (uint32_t)(ext_lo >> 32), hi0 = (uint32_t)ext_hi, hi1 = (uint32_t)(ext_hi >> 32);
-            const uint32_t v[8] = {lo0 & 0x00FF00FFu, (lo0 >> 8) & 0x00FF00FFu, lo1 & 0x00FF00FFu, (lo1 >> 8) & 0x00FF00FFu,
-                                   hi0 & 0x00FF00FFu, (hi0 >> 8) & 0x00FF00FFu, hi1 & 0x00FF00FFu, (hi1 >> 8) & 0x00FF00FFu};
-            uint32_t r[8];
-#pragma unroll
-            for (int i = 0; i < 8; i++) r[i] = g.sum(v[i]);
-            if (gl == 0) {
-#pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    const int m0 = (i >> 1) * 4 + (i & 1);       // v[i] holds models m0 (low half) and m0 + 2 (high half)
-                    s_ext[m0] = r[i] & 0xFFFFu; s_ext[m0 + 2] = r[i] >> 16;
-                }
-            }
-        }
-        g.sync();
 
         // =============================================================== E admit (R20, R21): smallest key first, per model
-        {
+        if (madm) {
+            uint32_t nw = s_misc[2];
             uint32_t mleft = madm;
+            // lane k tracks model k (state before this tick's service: admission precedes service, R21)
+            uint32_t a_nw = 0, a_nr = 0, a_kv = 0, a_tok = 0, a_olo = 0, a_ohi = 0;
+            if (gl < N) { a_nw = M_NWAIT(gl); a_nr = M_NRUN(gl); a_kv = M_KV(gl); a_olo = s_occ[2 * gl]; a_ohi = s_occ[2 * gl + 1]; }
             while (mleft) {
-                const uint32_t k = __ffs(mleft) - 1;
-                mleft &= mleft - 1;
-                const uint32_t off = s_boff[k], cnt = s_bcnt[k];
-                uint32_t nw = M_NWAIT(k), nr = M_NRUN(k), kv = M_KV(k), tok_adm = 0;   // tokens served to this tick's admissions (phase F)
-                const uint32_t slots = s_model[k].slots, cap = s_model[k].kv_cap;
-                auto scan_min = [&](uint32_t last, bool first) {
-                    uint32_t best = 0xFFFFFFFFu;
-                    for (uint32_t j = gl; j < cnt; j += G) {
-                        const uint32_t ridx = s_bucket[off + j] & 0xFFFu;
-                        const int32_t bt = P.sched_mode ? r_dl[ridx] : r_issue[ridx];
-                        const uint32_t key = ((uint32_t)(bt - t + (1 << 19)) << 12) | ridx;
-                        if ((first || key > last) && key < best) best = key;
-                    }
-                    return best;
-                };
-                uint32_t best = scan_min(0, true);
-                for (;;) {
-                    const uint32_t wkey = g.umin(best);
-                    if (wkey == 0xFFFFFFFFu) break;
-                    const uint32_t ridx = wkey & 0xFFFu;
-                    const uint32_t tk = r_tok[ridx], hw = hot[ridx];
-                    uint32_t rem = hw & 0xFFFFu;
-                    const uint32_t need = (tk >> 16) + ((tk & 0xFFFFu) - rem);           // R12
-                    if (!(nr < slots && kv + need <= cap)) break;                         // stop at the first misfit (R21)
-                    // admitted: prefill, then its first tick of service (R11)
-                    const uint32_t pf = (uint32_t)(((unsigned long long)s_model[k].prefill * need) / 1000u);
-                    const uint32_t usable = kDtUs - min(pf, kDtUs);
-                    const uint32_t x = s_model[k].rate * usable;
-                    const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
-                    const Ph4 u4 = draw(P, STREAM_SVC, gid, t, ridx >> 2, 0);
-                    const uint32_t uu = (ridx & 3u) == 0 ? u4.x : ((ridx & 3u) == 1 ? u4.y : ((ridx & 3u) == 2 ? u4.z : u4.w));
-                    const uint32_t tok = min(bs + (__umulhi(uu, 1000000u) < fr ? 1u : 0u), rem);
-                    rem -= tok;
-                    kv += need; tok_adm += tok; nw -= 1; nr += 1;
-                    if (gl == 0) {
-                        if (rem == 0) {
-                            s_clist[s_sc[0]] = (uint16_t)((k << 12) | ridx);
-                            s_sc[0] += 1;
-                            s_rfree[ridx >> 5] |= 1u << (ridx & 31);
-                            hot[ridx] = 0;
-                        } else {
-                            hot[ridx] = rem | (ST_RUN << HOT_STATE_SHIFT) | (k << HOT_MODEL_SHIFT);
-                        }
-                    }
-                    if (rem == 0) {
-                        g.sync();
-                        while (s_sc[0] >= (uint32_t)G) flush();
-                    }
-                    if (nw == 0 || nr >= slots) break;
-                    if (best == wkey) best = scan_min(wkey, false);
+                if (gl < kMaxModels) s_amin[gl] = 0xFFFFFFFFu;
+                if (gl == 0) s_sc[3] = 0;
+                g.sync();
+                for (uint32_t j = gl; j < nw; j += G) {                      // per-model minimum of the keys not yet admitted
+                    const uint32_t key = wkey[j], k = key >> 28;
+                    if (((mleft >> k) & 1u) && key >= s_alast[k]) atomicMin(&s_amin[k], key);
                 }
-                if (gl == 0) { M_NWAIT(k) = nw; M_NRUN(k) = nr; M_KV(k) = kv + tok_adm; }
+                g.sync();
+                for (uint32_t j = gl; j < nw; j += G) {                      // keys are unique: one writer per model
+                    const uint32_t key = wkey[j], k = key >> 28;
+                    if (((mleft >> k) & 1u) && key == s_amin[k]) s_aidx[k] = j;
+                }
+                g.sync();
+                bool still = false;
+                if (gl < N && ((mleft >> gl) & 1u) && s_amin[gl] != 0xFFFFFFFFu) {
+                    const uint32_t k = gl, key = s_amin[k], j = s_aidx[k], id = key & 0xFFFu;
+                    const uint2 wa = waux[j];
+                    const uint32_t sw = wa.y, rem0 = wa.x >> 16;
+                    const uint32_t need = ((sw >> SW_IN_SHIFT) & SW_TOK_MASK) + ((sw & SW_TOK_MASK) - rem0);     // R12
+                    if (a_nr < s_model[k].slots && a_kv + need <= s_model[k].kv_cap) {     // else: stop at the first misfit (R21)
+                        // lowest free slot of the model (R10)
+                        const uint32_t sl = ~a_olo ? (uint32_t)__ffs(~a_olo) - 1u : 31u + (uint32_t)__ffs(~a_ohi);
+                        if (sl < 32) a_olo |= 1u << sl; else a_ohi |= 1u << (sl - 32);
+                        const uint32_t gs = s_sbase[k] + sl;
+                        const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
+                        // prefill, then its first tick of service (R11)
+                        const uint32_t pf = (uint32_t)(((unsigned long long)s_model[k].prefill * need) / 1000u);
+                        const uint32_t usable = kDtUs - min(pf, kDtUs);
+                        const uint32_t x = s_model[k].rate * usable;
+                        const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
+                        const uint32_t thr = (uint32_t)(((unsigned long long)fr << 16) / 1000000u);
+                        const uint32_t u16 = u16_field(draw(P, STREAM_SVC, gid, t, gs >> 3, 0), gs & 7u);
+                        const uint32_t tok = min(bs + (u16 < thr ? 1u : 0u), rem0);
+                        const uint32_t rem = rem0 - tok;
+                        a_kv += need; a_tok += tok; a_nw -= 1; a_nr += 1;
+                        hot[gs] = rem | (id << 16);
+                        cold[gs] = make_uint2((wa.x & 0xFFFFu) | (dl << 16), sw);
+                        if (rem == 0) s_clist[atomicAdd(&s_sc[0], 1u)] = gs | (id << 16);
+                        s_rm[atomicAdd(&s_sc[3], 1u)] = j;
+                        s_alast[k] = key + 1u;
+                        still = a_nw > 0 && a_nr < s_model[k].slots;
+                    }
+                }
+                mleft = g.ballot(still);
+                g.sync();
+                // remove the admitted entries: the holes below the new length are filled from the tail
+                const uint32_t a = s_sc[3];
+                if (a) {
+                    const uint32_t new_len = nw - a;
+                    const bool isl = gl < a;
+                    const uint32_t h = isl ? s_rm[gl] : 0xFFFFFFFFu, p = new_len + gl;
+                    bool tail_hole = false;
+                    for (uint32_t x = 0; x < a; x++) tail_hole |= (g.shfl(h, (int)x) == p);
+                    const bool live = isl && !tail_hole, low = isl && h < new_len;
+                    const uint32_t lm = g.ballot(live), hm = g.ballot(low);
+                    if (live) s_mv[__popc(lm & lt_mask)] = p;
+                    g.sync();
+                    if (low) { const uint32_t src = s_mv[__popc(hm & lt_mask)]; wkey[h] = wkey[src]; waux[h] = waux[src]; }
+                    nw = new_len;
+                    g.sync();
+                }
+                while (s_sc[0] >= (uint32_t)G) flush();
             }
+            if (gl < N) { M_NWAIT(gl) = a_nw; M_NRUN(gl) = a_nr; M_KV(gl) = a_kv + a_tok; s_occ[2 * gl] = a_olo; s_occ[2 * gl + 1] = a_ohi; }
+            if (gl == 0) s_misc[2] = nw;
             g.sync();
         }
         // service totals of the requests that were RUNNING before this tick's admissions
-        if (gl < N) M_KV(gl) = (uint32_t)((int32_t)(M_KV(gl) + nrun_pre * s_base[gl] + s_ext[gl]) + s_kvcorr[gl]);
+        if (gl < N) M_KV(gl) += s_kvadd[gl];
         g.sync();
 
         // =============================================================== G complete: the rest of the list, then EWMA (R13)
         while (s_sc[0] > 0) flush();
         if (gl < N) {
             M_KV(gl) -= s_relkv[gl]; M_NRUN(gl) -= s_relnrun[gl];
+            s_occ[2 * gl] &= ~s_occclr[2 * gl]; s_occ[2 * gl + 1] &= ~s_occclr[2 * gl + 1];
             if (s_latn[gl] > 0) {
                 const int32_t mean_q8 = (int32_t)((s_latsum[gl] << 8) / s_latn[gl]);
                 int32_t ew = (int32_t)M_EWMA(gl);
@@ -440,47 +416,49 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             while (mover) {
                 const uint32_t k = __ffs(mover) - 1;
                 mover &= mover - 1;
-                // list the RUNNING requests of model k (second pass over hot, now in L2)
-                if (gl == 0) s_bcnt[0] = 0;
-                g.sync();
-                const uint4 *hot4 = (const uint4 *)hot;
-                for (uint32_t c = 0; c < n_chunks; c++) {
-                    const uint32_t i0 = (c * G + gl) * 4;
-                    const uint4 h4 = hot4[c * G + gl];
-                    const uint32_t hh[4] = {h4.x, h4.y, h4.z, h4.w};
-                    const uint32_t fr = s_rfree[i0 >> 5] >> (i0 & 31);
+                const uint32_t S = s_model[k].slots, sb = s_sbase[k], cap = s_model[k].kv_cap;
+                // candidates: the RUNNING requests of model k, <= 64 / G per lane; key = (deadline, id) + 1, 0 = none
+                constexpr int CPL = (64 + G - 1) / G;
+                uint32_t ckey[CPL], ckv[CPL];
 #pragma unroll
-                    for (int s = 0; s < 4; s++)
-                        if (!((fr >> s) & 1u) && ((hh[s] >> HOT_STATE_SHIFT) & 3u) == ST_RUN && ((hh[s] >> HOT_MODEL_SHIFT) & 15u) == k)
-                            s_bucket[atomicAdd(&s_bcnt[0], 1u)] = (uint16_t)(i0 + s);
+                for (int c = 0; c < CPL; c++) {
+                    const uint32_t sl = c * G + gl;
+                    ckey[c] = 0; ckv[c] = 0;
+                    if (sl < S && ((s_occ[2 * k + (sl >> 5)] >> (sl & 31)) & 1u)) {
+                        const uint32_t h = hot[sb + sl];
+                        const uint2 cd = cold[sb + sl];
+                        ckey[c] = (((cd.x >> 16) << 12) | (h >> 16)) + 1u;
+                        ckv[c] = ((cd.y >> SW_IN_SHIFT) & SW_TOK_MASK) + ((cd.y & SW_TOK_MASK) - (h & 0xFFFFu));
+                    }
+                }
+                uint32_t kv = M_KV(k), npre = 0;
+                const uint32_t nw_list = s_misc[2];
+                while (kv > cap) {
+                    uint32_t best = 0;
+#pragma unroll
+                    for (int c = 0; c < CPL; c++) best = max(best, ckey[c]);
+                    const uint32_t wbest = g.umax(best);
+                    if (wbest == 0) break;
+                    uint32_t mykv = 0;
+#pragma unroll
+                    for (int c = 0; c < CPL; c++) {
+                        if (ckey[c] == wbest) {                              // keys are unique: exactly one lane, one candidate
+                            const uint32_t sl = c * G + gl, gs = sb + sl;
+                            const uint32_t h = hot[gs];
+                            const uint2 cd = cold[gs];
+                            const uint32_t tm = P.sched_mode ? (cd.x >> 16) : (cd.x & 0xFFFFu);
+                            wkey[nw_list + npre] = (k << 28) | (tm << 12) | (h >> 16);
+                            waux[nw_list + npre] = make_uint2((cd.x & 0xFFFFu) | ((h & 0xFFFFu) << 16), cd.y);   // keeps progress and issue tick
+                            atomicAnd(&s_occ[2 * k + (sl >> 5)], ~(1u << (sl & 31)));
+                            mykv = ckv[c];
+                            ckey[c] = 0;
+                        }
+                    }
+                    kv -= g.sum(mykv);
+                    npre++;
                 }
                 g.sync();
-                const uint32_t cnt = s_bcnt[0];
-                uint32_t kv = M_KV(k), nr = M_NRUN(k), nw = M_NWAIT(k), npre = 0;
-                // victim = largest (deadline, ridx); candidates strictly below the previous victim on later rounds
-                auto scan_max = [&](uint32_t lim_d, uint32_t lim_i, bool first, uint32_t &bd, uint32_t &bi) {
-                    bd = 0; bi = 0; bool have = false;
-                    for (uint32_t j = gl; j < cnt; j += G) {
-                        const uint32_t ridx = s_bucket[j];
-                        const uint32_t d = (uint32_t)r_dl[ridx] + 0x80000000u;
-                        const bool below = first || d < lim_d || (d == lim_d && ridx < lim_i);
-                        if (below && (!have || d > bd || (d == bd && ridx > bi))) { bd = d; bi = ridx; have = true; }
-                    }
-                    return have;
-                };
-                uint32_t bd, bi;
-                bool have = scan_max(0, 0, true, bd, bi);
-                while (kv > s_model[k].kv_cap) {
-                    if (!g.ballot(have)) break;
-                    const uint32_t wd = g.umax(have ? bd : 0u);
-                    const uint32_t wi = g.umax((have && bd == wd) ? bi + 1u : 0u) - 1u;
-                    const uint32_t tk = r_tok[wi], hw = hot[wi];
-                    kv -= (tk >> 16) + ((tk & 0xFFFFu) - (hw & 0xFFFFu));
-                    nr -= 1; nw += 1; npre += 1;
-                    if (gl == 0) hot[wi] = (hw & ~(3u << HOT_STATE_SHIFT)) | (ST_WAIT << HOT_STATE_SHIFT);
-                    if (have && bd == wd && bi == wi) have = scan_max(wd, wi, false, bd, bi);
-                }
-                if (gl == 0) { M_KV(k) = kv; M_NRUN(k) = nr; M_NWAIT(k) = nw; s_ctr[C_PREEMPT] += npre; }
+                if (gl == 0) { M_KV(k) = kv; M_NRUN(k) -= npre; M_NWAIT(k) += npre; s_ctr[C_PREEMPT] += npre; s_misc[2] = nw_list + npre; }
                 g.sync();
             }
         }
@@ -501,14 +479,13 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             if (gl == 0) { s_ctr[C_SUM_RUNNING] += nr_sum; s_ctr[C_SUM_WAITING] += nw_sum; }
             g.sync();
             if (done) {
-                // hard reset: live queries abandoned, tables emptied (free slots are defined by the bitmaps)
+                // hard reset: live queries abandoned, pools emptied (free slots are defined by occ / the bitmaps)
                 uint32_t live = 0;
                 for (uint32_t w = gl; w < QW; w += G) live += __popc(~s_qfree[w]);
                 live = g.sum(live);
-                if (gl == 0) s_ctr[C_ABANDONED] += live;
-                for (uint32_t w = gl; w < RW; w += G) s_rfree[w] = 0xFFFFFFFFu;
+                if (gl == 0) { s_ctr[C_ABANDONED] += live; s_misc[2] = 0; }
                 for (uint32_t w = gl; w < QW; w += G) { s_qfree[w] = 0xFFFFFFFFu; s_qready[w] = 0; }
-                if (gl < N) { M_NWAIT(gl) = 0; M_NRUN(gl) = 0; M_KV(gl) = 0; M_EWMA(gl) = 0; }
+                if (gl < N) { M_NWAIT(gl) = 0; M_NRUN(gl) = 0; M_KV(gl) = 0; M_EWMA(gl) = 0; s_occ[2 * gl] = 0; s_occ[2 * gl + 1] = 0; }
             }
             if (gl == 0) s_misc[0] = 0;
             g.sync();
@@ -540,36 +517,43 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             uint32_t n = 0;
             for (uint32_t j = gl; j < 31; j += G) n += xr >= __ldg(&cdf[j]) ? 1u : 0u;
             n = g.sum(n);
-            const uint32_t n_free = build_prefix(g, s_qfree, QW, prefB);
-            const uint32_t n_ok = min(n, n_free);
-            uint32_t pidx0 = 0;
-            if (gl == 0 && n_ok) pidx0 = rows_claim(P, P.plan, region, n_ok);
-            pidx0 = g.shfl(pidx0, 0);
-            for (uint32_t j = gl; j < n_ok; j += G) {
-                const uint32_t q = find_nth(s_qfree, QW, prefB, j);
-                const Ph4 d = draw(P, STREAM_QRY, gid, t, j, 0);
-                const uint32_t comp = d.z < P.mix_thresh ? 0u : 1u;
-                const uint32_t budget = P.mix_lo[comp] + __umulhi(d.x, P.mix_hi[comp] - P.mix_lo[comp] + 1u);
-                const uint32_t in_tok = P.has_intok ? __ldg(&P.tab_intok[d.y >> 22]) : P.in_tok_const;
-                const int32_t dl = t + (int32_t)budget;                  // PAPER.md:117 deadline = t_arrive + beta
-                qtab[q] = make_uint4(QP_LIVE, budget | (in_tok << 16), (uint32_t)dl, (uint32_t)t);
-                P.plan.row[row_gid(P.plan, region, pidx0 + j)] = make_uint4(e, q | (t_rel << 19), (uint32_t)dl, in_tok);
-            }
-            g.sync();
-            // the n_ok lowest free query indices are the ones taken
-            for (uint32_t w = gl; w < QW; w += G) {
-                const uint32_t before = prefB[w], cntw = prefB[w + 1] - before;
-                if (before < n_ok) {
-                    const uint32_t take = min(n_ok - before, cntw);
-                    uint32_t bm = s_qfree[w];
-                    if (take == cntw) bm = 0; else for (uint32_t i = 0; i < take; i++) bm &= bm - 1;
-                    s_qfree[w] = bm;
+            if (n) {
+                const uint32_t n_free = build_prefix(g, s_qfree, QW, prefB);
+                const uint32_t n_ok = min(n, n_free);
+                uint32_t pidx0 = 0;
+                if (gl == 0 && n_ok) pidx0 = rows_claim(P, P.plan, region, n_ok);
+                pidx0 = g.shfl(pidx0, 0);
+                for (uint32_t j = gl; j < n_ok; j += G) {
+                    const uint32_t q = find_nth(s_qfree, QW, prefB, j);
+                    const Ph4 d = draw(P, STREAM_QRY, gid, t, j, 0);
+                    const uint32_t comp = d.z < P.mix_thresh ? 0u : 1u;
+                    const uint32_t budget = P.mix_lo[comp] + __umulhi(d.x, P.mix_hi[comp] - P.mix_lo[comp] + 1u);
+                    const uint32_t in_tok = P.has_intok ? __ldg(&P.tab_intok[d.y >> 22]) : P.in_tok_const;
+                    const int32_t dl = t + (int32_t)budget;                  // PAPER.md:117 deadline = t_arrive + beta
+                    qtab[q] = make_uint4(QP_LIVE, budget | (in_tok << 16), (uint32_t)dl, (uint32_t)t);
+                    P.plan.row[row_gid(P.plan, region, pidx0 + j)] = make_uint4(e, q | (t_rel << 19), (uint32_t)dl, in_tok);
                 }
-            }
-            if (gl == 0) {
-                s_ctr[C_ARRIVALS] += n; s_ctr[C_DROPPED] += n - n_ok; s_ctr[C_PLANS] += n_ok;
-                s_ctr[C_SUM_LIVE_MID] += QCAP - n_free + n_ok;
-                s_misc[0] = n - n_ok;                                   // drops carried to phase I of this tick
+                g.sync();
+                // the n_ok lowest free query indices are the ones taken
+                for (uint32_t w = gl; w < QW; w += G) {
+                    const uint32_t before = prefB[w], cntw = prefB[w + 1] - before;
+                    if (before < n_ok) {
+                        const uint32_t take = min(n_ok - before, cntw);
+                        uint32_t bm = s_qfree[w];
+                        if (take == cntw) bm = 0; else for (uint32_t i = 0; i < take; i++) bm &= bm - 1;
+                        s_qfree[w] = bm;
+                    }
+                }
+                if (gl == 0) {
+                    s_ctr[C_ARRIVALS] += n; s_ctr[C_DROPPED] += n - n_ok; s_ctr[C_PLANS] += n_ok;
+                    s_ctr[C_SUM_LIVE_MID] += QCAP - n_free + n_ok;
+                    s_misc[0] = n - n_ok;                                   // drops carried to phase I of this tick
+                }
+            } else {
+                uint32_t live = 0;
+                for (uint32_t w = gl; w < QW; w += G) live += __popc(~s_qfree[w]);
+                live = g.sum(live);
+                if (gl == 0) s_ctr[C_SUM_LIVE_MID] += live;
             }
             g.sync();
         }
@@ -600,22 +584,18 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
 
 void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st)
 {
-    // a half-warp per env doubles the envs in flight at the same register footprint; the packed 8-bit extra-token
-    // counters bound the slots one lane may serve to 255 (4 * RCAP / (4 * G) <= 255)
-    const bool half = P.N <= 16 && P.RCAP / 16 <= 255;
-    const uint32_t G = half ? 16 : 32;
-    const SimLayout L = sim_layout(P.hdr_words, P.RW, P.QW, P.RCAP, G);
+    // a half-warp per env: one lane per model in the admission and EWMA phases (N <= 16), 8 envs per 128-thread CTA
+    constexpr uint32_t G = 16;
+    const SimLayout L = sim_layout(P.hdr_words, P.QW, G);
     const uint32_t gpb = kSimThreads / G;
     const size_t smem = (size_t)gpb * L.total;
     const uint32_t blocks = (P.E + gpb - 1) / gpb;
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(k_sim<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        cudaFuncSetAttribute(k_sim<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         attr_set = true;
     }
-    if (half) k_sim<16><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
-    else k_sim<32><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
+    k_sim<16><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
 }
 
 }  // namespace im
