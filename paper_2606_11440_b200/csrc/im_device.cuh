@@ -163,6 +163,13 @@ __device__ __forceinline__ void stage_calls(uint32_t topo, uint32_t keff, uint32
 }
 
 __device__ __forceinline__ uint32_t row_gid(const RowBuf &rb, uint32_t region, uint32_t idx) { return region * rb.regcap + (idx % rb.regcap); }
+// the same for base + j with base already reduced modulo regcap and j <= regcap (one division per claim, not per row)
+__device__ __forceinline__ uint32_t row_gid_wrapped(const RowBuf &rb, uint32_t region, uint32_t base_mod, uint32_t j)
+{
+    uint32_t r = base_mod + j;
+    if (r >= rb.regcap) r -= rb.regcap;
+    return region * rb.regcap + r;
+}
 
 // claim n consecutive rows of region `region`; flags overflow in log mode
 __device__ __forceinline__ uint32_t rows_claim(const Params &P, const RowBuf &rb, uint32_t region, uint32_t n)
@@ -172,15 +179,17 @@ __device__ __forceinline__ uint32_t rows_claim(const Params &P, const RowBuf &rb
     return idx;
 }
 
-// executor rows of one stage of query q (R17); `pw` is the query's plan word with stage = the stage to dispatch
+// executor rows of one stage of query q (R17); `pw` is the query's plan word with stage = the stage to dispatch;
+// idx0 is the claimed ring position already reduced modulo regcap
 __device__ __forceinline__ void write_exec_rows(const Params &P, uint32_t region, uint32_t idx0, uint32_t e, uint32_t q, uint32_t pw,
                                                 uint32_t in_tok, int32_t dl, uint32_t t_rel, uint32_t a0, uint32_t nc)
 {
     const uint32_t topo = (pw >> 2) & 3u, keff = (pw >> 6) & 7u, roles = (pw >> QP_ROLE_SHIFT) & 0xFFu;
+#pragma unroll 1
     for (uint32_t j = 0; j < nc; j++) {
         const uint32_t agent = a0 + j;
         const uint32_t a = q | (agent << 10) | (topo << 12) | (((roles >> (2 * agent)) & 3u) << 14) | (keff << 16) | (t_rel << 19);
-        P.exec.row[row_gid(P.exec, region, idx0 + j)] = make_uint4(e, a, (uint32_t)dl, in_tok);
+        P.exec.row[row_gid_wrapped(P.exec, region, idx0, j)] = make_uint4(e, a, (uint32_t)dl, in_tok);
     }
 }
 

@@ -155,7 +155,7 @@ __device__ __forceinline__ void plan_commit(const Params &P, const RowInfo &ri, 
     const uint32_t pw = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
     env_q(P, ri.env)[q].x = pw | (1u << 9) | (nc << QP_PEND_SHIFT);
     const uint32_t region = ri.env % kRegions;
-    const uint32_t idx0 = rows_claim(P, P.exec, region, nc);
+    const uint32_t idx0 = rows_claim(P, P.exec, region, nc) % P.exec.regcap;
     write_exec_rows(P, region, idx0, ri.env, q, pw, ri.c & 0xFFFFu, ri.dl, t_rel, a0, nc);
 }
 

@@ -17,6 +17,7 @@
 // per model), removal fills the holes from the tail.  Every accumulation is an integer sum, so lanes may commit in any
 // order (R12, R13, R28).
 #include "im_device.cuh"
+#include <cstdlib>
 
 namespace im {
 
@@ -29,7 +30,7 @@ struct SimLayout {
 // small per-env arrays (u32 words): 16 per model-indexed array
 enum : uint32_t { SM_LATSUM = 0, SM_LATN = 16, SM_RELKV = 32, SM_RELNRUN = 48, SM_KVADD = 64, SM_OCCCLR = 80, SM_AMIN = 112,
                   SM_AIDX = 128, SM_ALAST = 144, SM_CTR = 160, SM_SC = 176, SM_RM = 184, SM_MV = 200, kSmallWords = 216 };
-__host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW, uint32_t G)
+__host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW, uint32_t SP)
 {
     auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
     SimLayout L;
@@ -37,7 +38,7 @@ __host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW,
     L.o_hdr = o; o += up(hdr_words * 4);
     L.o_pref = o; o += up((QW + 1) * 4);
     L.o_small = o; o += up(kSmallWords * 4);
-    L.o_clist = o; o += up(9 * G * 4);
+    L.o_clist = o; o += up(SP * 2);              // every slot may complete in one tick
     L.total = o;
     return L;
 }
@@ -68,6 +69,7 @@ template <int G>
 __device__ __forceinline__ uint32_t build_prefix(const Grp<G> &g, const uint32_t *bm, uint32_t nw, uint32_t *pref)
 {
     uint32_t carry = 0;
+#pragma unroll 1
     for (uint32_t w0 = 0; w0 < nw; w0 += G) {
         const uint32_t w = w0 + g.gl;
         const uint32_t pc = w < nw ? __popc(bm[w]) : 0u;
@@ -84,6 +86,7 @@ __device__ __forceinline__ uint32_t build_prefix(const Grp<G> &g, const uint32_t
 __device__ __forceinline__ uint32_t find_nth(const uint32_t *bm, uint32_t nw, const uint32_t *pref, uint32_t j)
 {
     uint32_t lo = 0, hi = nw;         // invariant: pref[lo] <= j < pref[hi]
+#pragma unroll 1
     while (hi - lo > 1) {
         const uint32_t mid = (lo + hi) >> 1;
         if (pref[mid] <= j) lo = mid; else hi = mid;
@@ -132,7 +135,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     const uint32_t N = P.N, QW = P.QW, QCAP = P.QCAP;
     const uint32_t region = e % kRegions;
 
-    const SimLayout L = sim_layout(P.hdr_words, QW, G);
+    const SimLayout L = sim_layout(P.hdr_words, QW, P.SP);
     unsigned char *sm = smem_raw + (size_t)(threadIdx.x / G) * L.total;
     uint32_t *s_hdr = (uint32_t *)(sm + L.o_hdr);
     uint32_t *s_occ = s_hdr + P.hw_occ, *s_qfree = s_hdr + P.hw_qfree, *s_qready = s_hdr + P.hw_qready, *s_misc = s_hdr + P.hw_misc;
@@ -143,7 +146,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     uint32_t *s_alast = s_small + SM_ALAST, *s_ctr = s_small + SM_CTR, *s_rm = s_small + SM_RM, *s_mv = s_small + SM_MV;
     uint32_t *s_sc = s_small + SM_SC;                 // [0] ccnt, [1] rew, [2] miss, [3] removals, [4..5] cost (u64)
     unsigned long long *s_cost = (unsigned long long *)(s_sc + 4);
-    uint32_t *s_clist = (uint32_t *)(sm + L.o_clist); // completed requests: global slot | id << 16
+    uint16_t *s_clist = (uint16_t *)(sm + L.o_clist); // completed requests: global slot index
 
     uint8_t *rec = env_rec(P, e);
     uint32_t *hot = (uint32_t *)(rec + P.off_hot), *wkey = (uint32_t *)(rec + P.off_wkey);
@@ -154,7 +157,9 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     {
         const uint4 *src = (const uint4 *)rec;
         uint4 *dst = (uint4 *)s_hdr;
+#pragma unroll 1
         for (uint32_t i = gl; i < P.hdr_words / 4; i += G) dst[i] = src[i];
+#pragma unroll 1
         for (uint32_t i = gl; i < kSmallWords; i += G) s_small[i] = 0;
     }
     g.sync();
@@ -171,8 +176,9 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
         const uint32_t tot = g.shfl(inc, G - 1);
         if (tot == 0) return;
         uint32_t idx0 = 0;
-        if (gl == 0) idx0 = rows_claim(P, P.exec, region, tot);
+        if (gl == 0) idx0 = rows_claim(P, P.exec, region, tot) % P.exec.regcap;
         idx0 = g.shfl(idx0, 0) + inc - nc;
+        if (idx0 >= P.exec.regcap) idx0 -= P.exec.regcap;
         if (valid) {
             write_exec_rows(P, region, idx0, e, q, pw, in_tok, dl, t_rel, a0, nc);
             // stage++, pending = nc: the calls are issued in phase D of the coming tick
@@ -194,14 +200,13 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             uint32_t q = 0x10000u + gl, succ = 0;
             uint4 qr = make_uint4(0, 0, 0, 0);
             if (act) {
-                const uint32_t ent = s_clist[ccnt - nb + gl];
-                const uint32_t gs = ent & 0xFFFFu, model = s_gmodel[gs >> 3], sl = gs - s_sbase[model];
-                q = ent >> 18;                                               // id = 4 q + agent
+                const uint32_t gs = s_clist[ccnt - nb + gl], model = s_gmodel[gs >> 3], sl = gs - s_sbase[model];
                 const uint2 cd = cold[gs];
+                q = hot[gs] >> 18;                                           // id = 4 q + agent (the word was just written: L1/L2)
                 qr = qtab[q];
                 succ = (cd.y >> SW_SUCC_SHIFT) & 1u;
                 const uint32_t ell = (uint32_t)(t + 1) - (cd.x & 0xFFFFu);
-                atomicAdd(s_cost, ((unsigned long long)ell << 16) / (qr.y & 0xFFFFu));   // C_k = l_k / beta, Q16 (R28)
+                atomicAdd(s_cost, (unsigned long long)((ell << 16) / (qr.y & 0xFFFFu)));   // C_k = l_k / beta, Q16 (R28); l < 2^16
                 atomicAdd(&s_latsum[model], ell); atomicAdd(&s_latn[model], 1u);
                 atomicAdd(&s_relkv[model], (cd.y & SW_TOK_MASK) + ((cd.y >> SW_IN_SHIFT) & SW_TOK_MASK)); atomicAdd(&s_relnrun[model], 1u);
                 atomicOr(&s_occclr[2 * model + (sl >> 5)], 1u << (sl & 31));  // the slot is free from the next tick on
@@ -255,6 +260,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             const uint32_t nw0 = s_misc[2];
             if (nw0 + icnt > P.RCAP) { if (gl == 0) atomicOr(P.err_flag, 8u); }      // cannot happen: rcap >= 3 qcap (R9)
             else
+#pragma unroll 1
                 for (uint32_t j = gl; j < icnt; j += G) {
                     const uint2 r = iss[j];
                     wkey[nw0 + j] = r.x;
@@ -300,7 +306,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                             const uint32_t tok = base + (u16 < thr ? 1u : 0u);
                             if (tok >= rem) {                                    // completes: only `rem` tokens are decoded
                                 tot += rem;
-                                s_clist[atomicAdd(&s_sc[0], 1u)] = (gi * 8 + s) | (w & 0xFFFF0000u);
+                                s_clist[atomicAdd(&s_sc[0], 1u)] = (uint16_t)(gi * 8 + s);
                                 hh[s] = w & 0xFFFF0000u;
                             } else {
                                 tot += tok;
@@ -312,9 +318,8 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                     hot4[2 * gi] = make_uint4(hh[0], hh[1], hh[2], hh[3]);
                     hot4[2 * gi + 1] = make_uint4(hh[4], hh[5], hh[6], hh[7]);
                 }
-                g.sync();
-                while (s_sc[0] >= (uint32_t)G) flush();
             }
+            g.sync();
         }
 
         // =============================================================== E admit (R20, R21): smallest key first, per model
@@ -328,14 +333,36 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 if (gl < kMaxModels) s_amin[gl] = 0xFFFFFFFFu;
                 if (gl == 0) s_sc[3] = 0;
                 g.sync();
-                for (uint32_t j = gl; j < nw; j += G) {                      // per-model minimum of the keys not yet admitted
-                    const uint32_t key = wkey[j], k = key >> 28;
-                    if (((mleft >> k) & 1u) && key >= s_alast[k]) atomicMin(&s_amin[k], key);
+                // per-model minimum of the keys not yet admitted: 128-bit loads, two in flight per lane
+                const uint4 *wk4 = (const uint4 *)wkey;
+                const uint32_t n4 = (nw + 3) >> 2;
+#pragma unroll 1
+                for (uint32_t j0 = 0; j0 < n4; j0 += 2 * G) {
+                    const uint32_t ja = j0 + gl, jb = ja + G;
+                    uint4 ka = make_uint4(~0u, ~0u, ~0u, ~0u), kb = ka;
+                    if (ja < n4) ka = wk4[ja];
+                    if (jb < n4) kb = wk4[jb];
+                    const uint32_t kk[8] = {ka.x, ka.y, ka.z, ka.w, kb.x, kb.y, kb.z, kb.w};
+#pragma unroll
+                    for (int i = 0; i < 8; i++) {
+                        const uint32_t j = ((i < 4 ? ja : jb) << 2) + (i & 3), key = kk[i], k = key >> 28;
+                        if (j < nw && ((mleft >> k) & 1u) && key >= s_alast[k]) atomicMin(&s_amin[k], key);
+                    }
                 }
                 g.sync();
-                for (uint32_t j = gl; j < nw; j += G) {                      // keys are unique: one writer per model
-                    const uint32_t key = wkey[j], k = key >> 28;
-                    if (((mleft >> k) & 1u) && key == s_amin[k]) s_aidx[k] = j;
+                // index of each minimum (keys are unique: one writer per model); the list is now in L1
+#pragma unroll 1
+                for (uint32_t j0 = 0; j0 < n4; j0 += 2 * G) {
+                    const uint32_t ja = j0 + gl, jb = ja + G;
+                    uint4 ka = make_uint4(~0u, ~0u, ~0u, ~0u), kb = ka;
+                    if (ja < n4) ka = wk4[ja];
+                    if (jb < n4) kb = wk4[jb];
+                    const uint32_t kk[8] = {ka.x, ka.y, ka.z, ka.w, kb.x, kb.y, kb.z, kb.w};
+#pragma unroll
+                    for (int i = 0; i < 8; i++) {
+                        const uint32_t j = ((i < 4 ? ja : jb) << 2) + (i & 3), key = kk[i], k = key >> 28;
+                        if (j < nw && ((mleft >> k) & 1u) && key == s_amin[k]) s_aidx[k] = j;
+                    }
                 }
                 g.sync();
                 bool still = false;
@@ -362,7 +389,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                         a_kv += need; a_tok += tok; a_nw -= 1; a_nr += 1;
                         hot[gs] = rem | (id << 16);
                         cold[gs] = make_uint2((wa.x & 0xFFFFu) | (dl << 16), sw);
-                        if (rem == 0) s_clist[atomicAdd(&s_sc[0], 1u)] = gs | (id << 16);
+                        if (rem == 0) s_clist[atomicAdd(&s_sc[0], 1u)] = (uint16_t)gs;
                         s_rm[atomicAdd(&s_sc[3], 1u)] = j;
                         s_alast[k] = key + 1u;
                         still = a_nw > 0 && a_nr < s_model[k].slots;
@@ -377,6 +404,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                     const bool isl = gl < a;
                     const uint32_t h = isl ? s_rm[gl] : 0xFFFFFFFFu, p = new_len + gl;
                     bool tail_hole = false;
+#pragma unroll 1
                     for (uint32_t x = 0; x < a; x++) tail_hole |= (g.shfl(h, (int)x) == p);
                     const bool live = isl && !tail_hole, low = isl && h < new_len;
                     const uint32_t lm = g.ballot(live), hm = g.ballot(low);
@@ -386,7 +414,6 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                     nw = new_len;
                     g.sync();
                 }
-                while (s_sc[0] >= (uint32_t)G) flush();
             }
             if (gl < N) { M_NWAIT(gl) = a_nw; M_NRUN(gl) = a_nr; M_KV(gl) = a_kv + a_tok; s_occ[2 * gl] = a_olo; s_occ[2 * gl + 1] = a_ohi; }
             if (gl == 0) s_misc[2] = nw;
@@ -481,9 +508,11 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             if (done) {
                 // hard reset: live queries abandoned, pools emptied (free slots are defined by occ / the bitmaps)
                 uint32_t live = 0;
+#pragma unroll 1
                 for (uint32_t w = gl; w < QW; w += G) live += __popc(~s_qfree[w]);
                 live = g.sum(live);
                 if (gl == 0) { s_ctr[C_ABANDONED] += live; s_misc[2] = 0; }
+#pragma unroll 1
                 for (uint32_t w = gl; w < QW; w += G) { s_qfree[w] = 0xFFFFFFFFu; s_qready[w] = 0; }
                 if (gl < N) { M_NWAIT(gl) = 0; M_NRUN(gl) = 0; M_KV(gl) = 0; M_EWMA(gl) = 0; s_occ[2 * gl] = 0; s_occ[2 * gl + 1] = 0; }
             }
@@ -499,6 +528,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
         // ---- executor rows of queries left ready by an earlier rollout (pending == 0, stages left)
         {
             const uint32_t n_ready = build_prefix(g, s_qready, QW, prefB);
+#pragma unroll 1
             for (uint32_t b0 = 0; b0 < n_ready; b0 += G) {
                 const uint32_t o = b0 + gl;
                 uint32_t q = 0;
@@ -507,7 +537,10 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 emit_ready(o < n_ready, q, qr.x, qr.y >> 16, (int32_t)qr.z, t_rel);
             }
             g.sync();
-            if (n_ready) for (uint32_t w = gl; w < QW; w += G) s_qready[w] = 0;
+            if (n_ready) {
+#pragma unroll 1
+                for (uint32_t w = gl; w < QW; w += G) s_qready[w] = 0;
+            }
             g.sync();
         }
         // ---- A arrive (R5, R7, R8, R9)
@@ -515,14 +548,16 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             const uint32_t xr = draw(P, STREAM_ARR, gid, t, 0, 0).x;
             const uint32_t *cdf = P.tab_cdf + 32u * P.env_level[e];
             uint32_t n = 0;
+#pragma unroll 1
             for (uint32_t j = gl; j < 31; j += G) n += xr >= __ldg(&cdf[j]) ? 1u : 0u;
             n = g.sum(n);
             if (n) {
                 const uint32_t n_free = build_prefix(g, s_qfree, QW, prefB);
                 const uint32_t n_ok = min(n, n_free);
                 uint32_t pidx0 = 0;
-                if (gl == 0 && n_ok) pidx0 = rows_claim(P, P.plan, region, n_ok);
+                if (gl == 0 && n_ok) pidx0 = rows_claim(P, P.plan, region, n_ok) % P.plan.regcap;
                 pidx0 = g.shfl(pidx0, 0);
+#pragma unroll 1
                 for (uint32_t j = gl; j < n_ok; j += G) {
                     const uint32_t q = find_nth(s_qfree, QW, prefB, j);
                     const Ph4 d = draw(P, STREAM_QRY, gid, t, j, 0);
@@ -531,16 +566,21 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                     const uint32_t in_tok = P.has_intok ? __ldg(&P.tab_intok[d.y >> 22]) : P.in_tok_const;
                     const int32_t dl = t + (int32_t)budget;                  // PAPER.md:117 deadline = t_arrive + beta
                     qtab[q] = make_uint4(QP_LIVE, budget | (in_tok << 16), (uint32_t)dl, (uint32_t)t);
-                    P.plan.row[row_gid(P.plan, region, pidx0 + j)] = make_uint4(e, q | (t_rel << 19), (uint32_t)dl, in_tok);
+                    P.plan.row[row_gid_wrapped(P.plan, region, pidx0, j)] = make_uint4(e, q | (t_rel << 19), (uint32_t)dl, in_tok);
                 }
                 g.sync();
                 // the n_ok lowest free query indices are the ones taken
+#pragma unroll 1
                 for (uint32_t w = gl; w < QW; w += G) {
                     const uint32_t before = prefB[w], cntw = prefB[w + 1] - before;
                     if (before < n_ok) {
                         const uint32_t take = min(n_ok - before, cntw);
                         uint32_t bm = s_qfree[w];
-                        if (take == cntw) bm = 0; else for (uint32_t i = 0; i < take; i++) bm &= bm - 1;
+                        if (take == cntw) bm = 0;
+                    else {
+#pragma unroll 1
+                        for (uint32_t i = 0; i < take; i++) bm &= bm - 1;
+                    }
                         s_qfree[w] = bm;
                     }
                 }
@@ -551,6 +591,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 }
             } else {
                 uint32_t live = 0;
+#pragma unroll 1
                 for (uint32_t w = gl; w < QW; w += G) live += __popc(~s_qfree[w]);
                 live = g.sum(live);
                 if (gl == 0) s_ctr[C_SUM_LIVE_MID] += live;
@@ -574,6 +615,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     {
         uint4 *dst = (uint4 *)rec;
         const uint4 *src = (const uint4 *)s_hdr;
+#pragma unroll 1
         for (uint32_t i = gl; i < P.hdr_words / 4; i += G) dst[i] = src[i];
     }
 #undef M_NWAIT
@@ -584,18 +626,21 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
 
 void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st)
 {
-    // a half-warp per env: one lane per model in the admission and EWMA phases (N <= 16), 8 envs per 128-thread CTA
-    constexpr uint32_t G = 16;
-    const SimLayout L = sim_layout(P.hdr_words, P.QW, G);
+    // G lanes per env: one lane per model in the admission and EWMA phases (N <= 16 <= G)
+    static int G = 0;
+    if (!G) {
+        const char *ev = getenv("IM_SIM_G");
+        G = ev ? atoi(ev) : 16;
+        if (G != 32) G = 16;
+        cudaFuncSetAttribute(k_sim<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_sim<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    }
+    const SimLayout L = sim_layout(P.hdr_words, P.QW, P.SP);
     const uint32_t gpb = kSimThreads / G;
     const size_t smem = (size_t)gpb * L.total;
     const uint32_t blocks = (P.E + gpb - 1) / gpb;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_sim<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        attr_set = true;
-    }
-    k_sim<16><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
+    if (G == 16) k_sim<16><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
+    else k_sim<32><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
 }
 
 }  // namespace im
