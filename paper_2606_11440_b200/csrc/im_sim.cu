@@ -62,6 +62,7 @@ struct Grp {
     }
     __device__ __forceinline__ uint32_t sum(uint32_t v) const { return __reduce_add_sync(gmask, v); }
     __device__ __forceinline__ uint32_t umax(uint32_t v) const { return __reduce_max_sync(gmask, v); }
+    __device__ __forceinline__ uint32_t umin(uint32_t v) const { return __reduce_min_sync(gmask, v); }
 };
 
 // exclusive prefix of popcounts of bm[0..nw) into pref[0..nw]; returns the total
@@ -153,14 +154,24 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     uint2 *cold = (uint2 *)(rec + P.off_cold), *waux = (uint2 *)(rec + P.off_waux);
     uint4 *qtab = (uint4 *)(rec + P.off_q);
 
-    // ---- load the header
+    // ---- load the header; the first group of slots of every lane is fetched with it (one round trip, not two)
+    uint4 pre_a = make_uint4(0, 0, 0, 0), pre_b = pre_a;
     {
         const uint4 *src = (const uint4 *)rec;
         uint4 *dst = (uint4 *)s_hdr;
+        const uint32_t nh = P.hdr_words / 4;                      // <= 49 uint4
+        uint4 h0, h1, h2, h3;
+        if (gl < nh) h0 = src[gl];
+        if (gl + G < nh) h1 = src[gl + G];
+        if (gl + 2 * G < nh) h2 = src[gl + 2 * G];
+        if (gl + 3 * G < nh) h3 = src[gl + 3 * G];
+        if (t_post >= 0 && gl < (P.SP >> 3)) { pre_a = ((const uint4 *)hot)[2 * gl]; pre_b = ((const uint4 *)hot)[2 * gl + 1]; }
 #pragma unroll 1
-        for (uint32_t i = gl; i < P.hdr_words / 4; i += G) dst[i] = src[i];
-#pragma unroll 1
-        for (uint32_t i = gl; i < kSmallWords; i += G) s_small[i] = 0;
+        for (uint32_t i = gl; i < kSmallWords / 4; i += G) ((uint4 *)s_small)[i] = make_uint4(0, 0, 0, 0);
+        if (gl < nh) dst[gl] = h0;
+        if (gl + G < nh) dst[gl + G] = h1;
+        if (gl + 2 * G < nh) dst[gl + 2 * G] = h2;
+        if (gl + 3 * G < nh) dst[gl + 3 * G] = h3;
     }
     g.sync();
 #define M_NWAIT(k) s_hdr[4 * (k) + 0]
@@ -285,7 +296,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             };
             uint4 na = make_uint4(0, 0, 0, 0), nb = na;
             uint32_t nocc = 0;
-            if (gl < n_grp) { nocc = occ8_of(gl); if (nocc) { na = hot4[2 * gl]; nb = hot4[2 * gl + 1]; } }
+            if (gl < n_grp) { nocc = occ8_of(gl); na = pre_a; nb = pre_b; }
             for (uint32_t g0 = 0; g0 < n_grp; g0 += G) {
                 const uint32_t gi = g0 + gl;
                 const uint4 ha = na, hb = nb;
@@ -333,36 +344,40 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 if (gl < kMaxModels) s_amin[gl] = 0xFFFFFFFFu;
                 if (gl == 0) s_sc[3] = 0;
                 g.sync();
-                // per-model minimum of the keys not yet admitted: 128-bit loads, two in flight per lane
+                // per-model minimum of the waiting keys and its list index, two admitting models per pass over the list
+                // (128-bit loads, two in flight per lane).  The keys of model k are those in [k<<28, (k+1)<<28): for them,
+                // and only for them, key - (k<<28) is below 2^28 - 1 in unsigned arithmetic.
                 const uint4 *wk4 = (const uint4 *)wkey;
                 const uint32_t n4 = (nw + 3) >> 2;
+                uint32_t mscan = mleft;
 #pragma unroll 1
-                for (uint32_t j0 = 0; j0 < n4; j0 += 2 * G) {
-                    const uint32_t ja = j0 + gl, jb = ja + G;
-                    uint4 ka = make_uint4(~0u, ~0u, ~0u, ~0u), kb = ka;
-                    if (ja < n4) ka = wk4[ja];
-                    if (jb < n4) kb = wk4[jb];
-                    const uint32_t kk[8] = {ka.x, ka.y, ka.z, ka.w, kb.x, kb.y, kb.z, kb.w};
-#pragma unroll
-                    for (int i = 0; i < 8; i++) {
-                        const uint32_t j = ((i < 4 ? ja : jb) << 2) + (i & 3), key = kk[i], k = key >> 28;
-                        if (j < nw && ((mleft >> k) & 1u) && key >= s_alast[k]) atomicMin(&s_amin[k], key);
-                    }
-                }
-                g.sync();
-                // index of each minimum (keys are unique: one writer per model); the list is now in L1
+                while (mscan) {
+                    const uint32_t k0 = __ffs(mscan) - 1;
+                    mscan &= mscan - 1;
+                    const uint32_t k1 = mscan ? __ffs(mscan) - 1 : k0;
+                    mscan &= mscan - 1;
+                    const uint32_t b0 = k0 << 28, b1 = k1 << 28;
+                    uint32_t d0 = 0x0FFFFFFFu, d1 = 0x0FFFFFFFu, i0 = 0, i1 = 0;
 #pragma unroll 1
-                for (uint32_t j0 = 0; j0 < n4; j0 += 2 * G) {
-                    const uint32_t ja = j0 + gl, jb = ja + G;
-                    uint4 ka = make_uint4(~0u, ~0u, ~0u, ~0u), kb = ka;
-                    if (ja < n4) ka = wk4[ja];
-                    if (jb < n4) kb = wk4[jb];
-                    const uint32_t kk[8] = {ka.x, ka.y, ka.z, ka.w, kb.x, kb.y, kb.z, kb.w};
+                    for (uint32_t j0 = 0; j0 < n4; j0 += 2 * G) {
+                        const uint32_t ja = j0 + gl, jb = ja + G;
+                        uint4 ka = make_uint4(~0u, ~0u, ~0u, ~0u), kb = ka;
+                        if (ja < n4) ka = wk4[ja];
+                        if (jb < n4) kb = wk4[jb];
+                        if (ja < n4 && nw - 4 * ja < 4) { const uint32_t v = nw - 4 * ja; if (v < 2) ka.y = ~0u; if (v < 3) ka.z = ~0u; ka.w = ~0u; }
+                        if (jb < n4 && nw - 4 * jb < 4) { const uint32_t v = nw - 4 * jb; if (v < 2) kb.y = ~0u; if (v < 3) kb.z = ~0u; kb.w = ~0u; }
+                        const uint32_t kk[8] = {ka.x, ka.y, ka.z, ka.w, kb.x, kb.y, kb.z, kb.w};
 #pragma unroll
-                    for (int i = 0; i < 8; i++) {
-                        const uint32_t j = ((i < 4 ? ja : jb) << 2) + (i & 3), key = kk[i], k = key >> 28;
-                        if (j < nw && ((mleft >> k) & 1u) && key == s_amin[k]) s_aidx[k] = j;
+                        for (int i = 0; i < 8; i++) {
+                            const uint32_t j = ((i < 4 ? ja : jb) << 2) + (i & 3);
+                            const uint32_t da = kk[i] - b0, db = kk[i] - b1;
+                            if (da < d0) { d0 = da; i0 = j; }
+                            if (db < d1) { d1 = db; i1 = j; }
+                        }
                     }
+                    const uint32_t m0 = g.umin(d0), m1 = g.umin(d1);
+                    if (m0 != 0x0FFFFFFFu && d0 == m0) { s_amin[k0] = b0 + m0; s_aidx[k0] = i0; }     // keys are unique: one lane
+                    if (k1 != k0 && m1 != 0x0FFFFFFFu && d1 == m1) { s_amin[k1] = b1 + m1; s_aidx[k1] = i1; }
                 }
                 g.sync();
                 bool still = false;
@@ -391,7 +406,6 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                         cold[gs] = make_uint2((wa.x & 0xFFFFu) | (dl << 16), sw);
                         if (rem == 0) s_clist[atomicAdd(&s_sc[0], 1u)] = (uint16_t)gs;
                         s_rm[atomicAdd(&s_sc[3], 1u)] = j;
-                        s_alast[k] = key + 1u;
                         still = a_nw > 0 && a_nr < s_model[k].slots;
                     }
                 }
