@@ -437,7 +437,7 @@ static size_t bf16_smem_bytes() { return 2ull * kBfRows * (H + 8) * 2; }
 // One persistent CTA per SM; the whole net (192 KB of bf16 weights) stays in shared memory for the lifetime of the
 // launch; a tile is 128 rows = 128 TMEM lanes = 128 threads, thread r owning row r from feature gather to sampling.
 // Layer 1 contracts only the first 64 features: rows are zero beyond 3N + 12 <= 60 (R15), so this is exact.
-constexpr int kTcK1 = 64, kTcH = 256, kTcThreads = 128;
+constexpr int kTcK1 = 64, kTcH = 256, kTcThreads = 256;
 template <bool EXEC> using TcNet = tc::TcMlp<kTcK1, kTcH, EXEC ? 64 : 32>;
 
 bool tc_supported(uint32_t F, uint32_t H) { return F == 128 && H == 256; }
@@ -518,14 +518,14 @@ __device__ __forceinline__ TcRaw tc_fetch_row(const TileSched &S, const RowBuf &
     x.row = make_uint4(0, 0, 0, 0); x.env = 0; x.gidx = 0; x.ok = false; x.critic = false;
     if (tile >= S.total) return x;
     if (tile < S.crit_tiles) {
-        const uint32_t env = tile * kTcThreads + r;
+        const uint32_t env = tile * 128u + r;
         x.ok = env < n_crit; x.critic = true; x.env = env;
         return x;
     }
     const uint32_t lt = tile - S.crit_tiles;
     uint32_t lo = 0, hi = kRegions;
     while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
-    const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * kTcThreads + r;
+    const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * 128u + r;
     if (idx >= rb.cnt[lo]) return x;
     x.gidx = row_gid(rb, lo, idx);
     x.row = rb.row[x.gidx];
@@ -547,6 +547,9 @@ __device__ __forceinline__ RowInfo tc_decode_row(const Params &P, const TcRaw &x
     return ri;
 }
 
+// Row handed from the gathering warpgroup to the sampling warpgroup through shared memory
+struct TcRowSlot { uint4 row; uint32_t env, gidx, flags, pad; };           // flags: bit 0 ok, bit 1 critic
+
 template <bool EXEC>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32_t trow)
@@ -555,26 +558,33 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     constexpr int NO = EXEC ? 64 : 32;
     extern __shared__ __align__(1024) uint8_t smem_tc[];
     __shared__ TileSched sched;
-    __shared__ uint64_t bar;
+    __shared__ uint64_t bars[5];                          // layer 1 half a / b, layer 2 half a / b, layer 3
     __shared__ uint32_t tmem_slot;
     uint8_t *img = smem_tc, *a1 = smem_tc + ((Net::kImageBytes + 1023u) & ~1023u);
+    TcRowSlot *rowbuf = reinterpret_cast<TcRowSlot *>(a1 + Net::kA1Bytes);     // [2][128]
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(W.tc_img);
         uint4 *dst = reinterpret_cast<uint4 *>(img);
         for (uint32_t i = threadIdx.x; i < Net::kImageBytes / 16; i += kTcThreads) dst[i] = __ldg(src + i);
     }
-    if (threadIdx.x == 0) { tc::mbar_init(&bar, 1); tc::mbar_fence_init(); }
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 5; i++) tc::mbar_init(&bars[i], 1);
+        tc::mbar_fence_init();
+    }
     if (threadIdx.x < 32) tc::tmem_alloc(&tmem_slot, Net::kTmemCols);
     const RowBuf &rb = EXEC ? P.exec : P.plan;
     const uint32_t n_crit = EXEC ? P.E : 0u;
-    sched_init(sched, rb, parity, kTcThreads, n_crit);
+    sched_init(sched, rb, parity, 128, n_crit);
     tc::tc_fence_before();
     __syncthreads();
     tc::tc_fence_after();
     const uint32_t tmem_base = tmem_slot;
     const uint32_t N3 = 3 * P.N;
     const bool vec = (N3 % 8u) == 0;                      // snapshot block = whole 16-byte chunks (N = 8, 16)
-    uint32_t phase = 0;
+    const uint32_t wg = threadIdx.x >> 7, r = threadIdx.x & 127u;
+    const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
+    const float *bias = reinterpret_cast<const float *>(img + Net::kBias);
+    const uint32_t total = sched.total;
 
     // snapshot floats of a row's env (R14): up to 12 float4 per thread, issued early, consumed one tile later
     auto fetch_snap = [&](const TcRaw &x, float4 (&sn)[12]) {
@@ -583,14 +593,11 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
 #pragma unroll
         for (int j = 0; j < 12; j++) sn[j] = (x.ok && vec && (uint32_t)(4 * j) < N3) ? __ldg(src + j) : make_float4(0.f, 0.f, 0.f, 0.f);
     };
-
-    TcRaw cur = tc_fetch_row(sched, rb, blockIdx.x, threadIdx.x, n_crit);
-    float4 sn[12];
-    fetch_snap(cur, sn);
-    for (uint32_t tile = blockIdx.x; tile < sched.total; tile += gridDim.x) {
+    // features of row `cur` -> A1 (bf16 RNE), canonical layout: chunk c of row r at c * 2048 + r * 16; row -> rowbuf
+    auto build_a1 = [&](const TcRaw &cur, const float4 (&sn)[12], TcRowSlot *slot) {
         const RowInfo ri = tc_decode_row<EXEC>(P, cur, t0);
         const bool ok = cur.ok;
-        // ---- features -> A1 (bf16 RNE), canonical layout: chunk c of row r at c * 2048 + r * 16
+        slot[r].row = cur.row; slot[r].env = cur.env; slot[r].gidx = cur.gidx; slot[r].flags = (ok ? 1u : 0u) | (cur.critic ? 2u : 0u);
         if (vec) {
             float tl[16];                                 // the 12 features behind the snapshot block, then zeros
 #pragma unroll
@@ -606,7 +613,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
 #pragma unroll
                     for (int j = 0; j < 8; j++) f[j] = (uint32_t)c == c0 ? tl[j] : ((uint32_t)c == c0 + 1 ? tl[8 + j] : 0.0f);
                 }
-                *reinterpret_cast<uint4 *>(a1 + c * (128 * 16) + threadIdx.x * 16) =
+                *reinterpret_cast<uint4 *>(a1 + c * (128 * 16) + r * 16) =
                     make_uint4(tc::pack_bf16(f[0], f[1]), tc::pack_bf16(f[2], f[3]), tc::pack_bf16(f[4], f[5]), tc::pack_bf16(f[6], f[7]));
             }
         } else {
@@ -615,60 +622,106 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
                 float f[8];
 #pragma unroll
                 for (int j = 0; j < 8; j++) f[j] = ok ? feature(P, EXEC, ri, tc_feature_src(8 * c + j, N3)) : 0.0f;
-                *reinterpret_cast<uint4 *>(a1 + c * (128 * 16) + threadIdx.x * 16) =
+                *reinterpret_cast<uint4 *>(a1 + c * (128 * 16) + r * 16) =
                     make_uint4(tc::pack_bf16(f[0], f[1]), tc::pack_bf16(f[2], f[3]), tc::pack_bf16(f[4], f[5]), tc::pack_bf16(f[6], f[7]));
             }
         }
-        // ---- next tile's row: the load flies while the tensor cores work on this tile
-        const TcRaw nxt = tc_fetch_row(sched, rb, tile + gridDim.x, threadIdx.x, n_crit);
-        float l[NO];
-        Net::run(img, a1, tmem_base, &bar, phase, l);
-        fetch_snap(nxt, sn);                              // consumed at the top of the next iteration
-        // ---- epilogue of row `ri`: logits in registers
-        if (ok) {
-            if (EXEC) {
-                const uint32_t n = N3;
-                float value = 0.0f;
-#pragma unroll
-                for (int i = 0; i < NO; i++) if ((uint32_t)i == n) value = l[i];
-                if (ri.critic) {
-                    P.val[(size_t)trow * P.E + ri.env] = value;
-                } else {
-                    if (P.exec.logits) {
-#pragma unroll
-                        for (int i = 0; i < NO; i++) if ((uint32_t)i <= n) P.exec.logits[(size_t)ri.gidx * P.exec.n_out + i] = l[i];
-                    }
-                    const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
-                    const int32_t t = t0 + (int32_t)(ri.a >> 19);
-                    const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
-                    float logp;
-                    const uint32_t act = sample_reg<48, NO>(l, 0, n, u24(d.x), logp);
-                    exec_commit(P, ri, d, act, logp, value, t);
-                }
-            } else {
-                if (P.plan.logits) {
-#pragma unroll
-                    for (int i = 0; i < 24; i++) P.plan.logits[(size_t)ri.gidx * 24 + i] = l[i];
-                }
-                const uint32_t q = ri.a & 0x3FFu;
-                const int32_t t = t0 + (int32_t)(ri.a >> 19);
-                const uint32_t gid = P.env_id_base + ri.env;
-                const Ph4 d0 = draw(P, STREAM_PLAN, gid, t, q, 0), d1 = draw(P, STREAM_PLAN, gid, t, q, 1);
-                float lp_t, lp_c, lp_r[4];
-                const uint32_t topo = sample_reg<4, NO>(l, 0, 4, u24(d0.x), lp_t);
-                const uint32_t cnt = sample_reg<4, NO>(l, 4, 4, u24(d0.y), lp_c);
-                const uint32_t ur[4] = {d1.x, d1.y, d1.z, d1.w};
-                uint32_t roles = 0;
-#pragma unroll
-                for (int a = 0; a < 4; a++) roles |= sample_reg<4, NO>(l, 8 + 4 * a, 4, u24(ur[a]), lp_r[a]) << (2 * a);
-                const uint32_t keff = keff_of(topo, cnt + 1);
-                float lp = __fadd_rn(lp_t, lp_c);
-#pragma unroll
-                for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
-                plan_commit(P, ri, topo, cnt, roles, lp);
-            }
+    };
+    // ---- prologue: warpgroup 1 gathers the first tile and starts its layer 1
+    TcRaw nxt;
+    float4 sn[12];
+    if (wg == 1) {
+        nxt = tc_fetch_row(sched, rb, blockIdx.x, r, n_crit);
+        fetch_snap(nxt, sn);
+        if (blockIdx.x < total) {
+            build_a1(nxt, sn, rowbuf);
+            tc::fence_proxy_async_smem();
+            tc::bar_sync(2, 128);
+            if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
+            nxt = tc_fetch_row(sched, rb, blockIdx.x + gridDim.x, r, n_crit);
+            fetch_snap(nxt, sn);
         }
-        cur = nxt;
+    }
+    uint32_t phase = 0, it = 0;
+    for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
+        // ---- hidden layer 1: warpgroup w takes columns [128 w, 128 w + 128) as soon as its half is ready
+        tc::mbar_wait(&bars[wg], phase);
+        tc::tc_fence_after();
+        Net::half_epilogue(tlane, 128 * wg, Net::kColA2 + 64 * wg, bias + 128 * wg);
+        tc::tc_fence_before();
+        __syncthreads();
+        if (threadIdx.x == 0) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
+        // ---- hidden layer 2
+        tc::mbar_wait(&bars[2 + wg], phase);
+        tc::tc_fence_after();
+        Net::half_epilogue(tlane, 128 * wg, Net::kColA3 + 64 * wg, bias + kTcH + 128 * wg);
+        tc::tc_fence_before();
+        __syncthreads();
+        if (threadIdx.x == 0) Net::issue_l3(img, tmem_base, &bars[4]);
+        if (wg == 1) {
+            // ---- warpgroup 1: features of the next tile, its layer 1, then the row loads of the tile after it
+            if (tile + gridDim.x < total) {
+                build_a1(nxt, sn, rowbuf + 128 * ((it + 1) & 1u));
+                tc::fence_proxy_async_smem();
+                tc::bar_sync(2, 128);
+                if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
+                nxt = tc_fetch_row(sched, rb, tile + 2 * gridDim.x, r, n_crit);
+                fetch_snap(nxt, sn);
+            }
+            continue;
+        }
+        // ---- warpgroup 0: sampling epilogue of row r, logits in registers
+        const TcRowSlot sl = rowbuf[128 * (it & 1u) + r];
+        tc::mbar_wait(&bars[4], phase);
+        tc::tc_fence_after();
+        float l[NO];
+        Net::load_logits(img, tlane, l);
+        tc::tc_fence_before();
+        if (!(sl.flags & 1u)) continue;
+        TcRaw cur;
+        cur.row = sl.row; cur.env = sl.env; cur.gidx = sl.gidx; cur.ok = true; cur.critic = (sl.flags & 2u) != 0;
+        const RowInfo ri = tc_decode_row<EXEC>(P, cur, t0);
+        if (EXEC) {
+            const uint32_t n = N3;
+            float value = 0.0f;
+#pragma unroll
+            for (int i = 0; i < NO; i++) if ((uint32_t)i == n) value = l[i];
+            if (ri.critic) {
+                P.val[(size_t)trow * P.E + ri.env] = value;
+            } else {
+                if (P.exec.logits) {
+#pragma unroll
+                    for (int i = 0; i < NO; i++) if ((uint32_t)i <= n) P.exec.logits[(size_t)ri.gidx * P.exec.n_out + i] = l[i];
+                }
+                const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
+                const int32_t t = t0 + (int32_t)(ri.a >> 19);
+                const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
+                float logp;
+                const uint32_t act = sample_reg<48, NO>(l, 0, n, u24(d.x), logp);
+                exec_commit(P, ri, d, act, logp, value, t);
+            }
+        } else {
+            if (P.plan.logits) {
+#pragma unroll
+                for (int i = 0; i < 24; i++) P.plan.logits[(size_t)ri.gidx * 24 + i] = l[i];
+            }
+            const uint32_t q = ri.a & 0x3FFu;
+            const int32_t t = t0 + (int32_t)(ri.a >> 19);
+            const uint32_t gid = P.env_id_base + ri.env;
+            const Ph4 d0 = draw(P, STREAM_PLAN, gid, t, q, 0), d1 = draw(P, STREAM_PLAN, gid, t, q, 1);
+            float lp_t, lp_c, lp_r[4];
+            const uint32_t topo = sample_reg<4, NO>(l, 0, 4, u24(d0.x), lp_t);
+            const uint32_t cnt = sample_reg<4, NO>(l, 4, 4, u24(d0.y), lp_c);
+            const uint32_t ur[4] = {d1.x, d1.y, d1.z, d1.w};
+            uint32_t roles = 0;
+#pragma unroll
+            for (int a = 0; a < 4; a++) roles |= sample_reg<4, NO>(l, 8 + 4 * a, 4, u24(ur[a]), lp_r[a]) << (2 * a);
+            const uint32_t keff = keff_of(topo, cnt + 1);
+            float lp = __fadd_rn(lp_t, lp_c);
+#pragma unroll
+            for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
+            plan_commit(P, ri, topo, cnt, roles, lp);
+        }
     }
     tc::tc_fence_before();
     __syncthreads();
@@ -690,7 +743,7 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
         return 0;
     }
     if (W.tc_img) {
-        const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes;
+        const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot);
         if (exec) {
             cudaFuncSetAttribute(k_policy_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             k_policy_tc<true><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);

@@ -7,14 +7,8 @@
 // A core matrix (8 rows x 16 bytes) is then 128 contiguous bytes; in the UMMA shared-memory descriptor the stride
 // between 8-row groups (SBO) is 128 B and the stride between k-chunks (LBO) is rows * 16 B.
 //
-// Tile data flow (M = 128 rows = 128 TMEM lanes, one thread per row in the epilogues):
-//   A1 (features, smem) x W1 -> D1 (TMEM cols [0,H))        SS-mode UMMA, K1 / 16 instructions of N = H
-//   tanh(D1 + b1) -> bf16, packed two per column in place    TMEM cols [0,H/2)        (tcgen05.ld / tcgen05.st)
-//   A2 (TMEM) x W2 -> D2 (TMEM cols [H,2H))                  TS-mode UMMA, H / 16 instructions
-//   tanh(D2 + b2) -> bf16 in place                           TMEM cols [H,H+H/2)
-//   A3 (TMEM) x W3 -> D3 (TMEM cols [0,NO))                  TS-mode UMMA, N = NO
-//   logits = D3 + b3 -> registers of the row's thread
-// The hidden activations never touch shared memory: all three weight matrices stay resident in it instead.
+// Tile data flow: see TcMlp below.  The hidden activations never touch shared memory: all three weight matrices
+// stay resident in it instead.
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -159,104 +153,95 @@ __host__ __device__ constexpr uint32_t canon_off(uint32_t rows, uint32_t r, uint
 // ---------------------------------------------------------------------------------------------- the MLP of one tile
 // Shared-memory image of one net (built once by k_pack_tc, copied verbatim by every CTA):
 //   [ W1 canon [H][K1] | W2 canon [H][H] | W3 canon [NO][H] | b1[H] b2[H] b3[NO] fp32 ]
+//
+// Two warpgroups (256 threads) work on one 128-row tile; every hidden layer is computed as two N-halves of 128
+// columns with their own mbarrier, so that warpgroup 0 runs the tanh epilogue of half a while the tensor core still
+// computes half b (which warpgroup 1 then takes).  TMEM map (512 columns, H = 256):
+//   D1 = [0,256)  ->  A2 = [256,384)  ;  D2 = [0,256)  ->  A3 = [384,512)  ;  D3 = [256,256+NO)
+// Nothing is packed in place, and the next tile's layer 1 (D1) touches no column the sampling epilogue (D3) reads.
 template <int K1, int H, int NO>
 struct TcMlp {
-    static_assert(K1 % 16 == 0 && H % 32 == 0 && NO % 16 == 0 && NO <= 64 && H <= 256, "shape");
+    static_assert(K1 % 16 == 0 && H == 256 && NO % 16 == 0 && NO <= 64, "shape");
     static constexpr uint32_t kW1 = 0, kW2 = kW1 + H * K1 * 2, kW3 = kW2 + H * H * 2, kBias = kW3 + NO * H * 2;
     static constexpr uint32_t kImageBytes = kBias + (2 * H + NO) * 4;
     static constexpr uint32_t kA1Bytes = 128 * K1 * 2;
-    static constexpr uint32_t kTmemCols = 2 * H;                 // 512 for H = 256, 256 for H = 128 (powers of two)
+    static constexpr uint32_t kTmemCols = 512;
+    static constexpr uint32_t kColA2 = 256, kColA3 = 384, kColD3 = 256;
+    static constexpr uint32_t kIdescHalf = instr_desc_bf16(128, 128), kIdescOut = instr_desc_bf16(128, NO);
 
-    // tanh(D + bias) of TMEM columns [col0, col0+H) -> bf16 pairs packed in place into [col0, col0+H/2).
+    // tanh(D + bias) of the 128 TMEM columns [src, src+128) -> bf16 pairs in [dst, dst+64); bias points at the half's first column.
     // `tlane` = TMEM address of this warp's lane quarter at column 0 of the allocation.
-    static __device__ __forceinline__ void hidden_epilogue(uint32_t tlane, uint32_t col0, const float *bias)
+    static __device__ __forceinline__ void half_epilogue(uint32_t tlane, uint32_t src, uint32_t dst, const float *bias)
     {
 #pragma unroll 1
-        for (int j = 0; j < H / 32; j++) {
+        for (int j = 0; j < 4; j++) {
             uint32_t v[32], o[16];
-            tmem_ld32(tlane + col0 + 32 * j, v);
+            tmem_ld32(tlane + src + 32 * j, v);
             tc_wait_ld();
 #pragma unroll
             for (int i = 0; i < 16; i++) {
                 const float2 b = *reinterpret_cast<const float2 *>(bias + 32 * j + 2 * i);
                 o[i] = pack_bf16(tanh_approx(__uint_as_float(v[2 * i]) + b.x), tanh_approx(__uint_as_float(v[2 * i + 1]) + b.y));
             }
-            tmem_st16(tlane + col0 + 16 * j, o);   // in place: columns [16j,16j+16) lie below every column still to be read
+            tmem_st16(tlane + dst + 16 * j, o);
         }
         tc_wait_st();
     }
 
-    // Runs the three layers for the 128 rows whose features sit in `a1` (canonical [128][K1], written by the generic
-    // proxy).  All 128 threads call it; on return `logit[i]` = D3[row = threadIdx.x][i] + b3[i].  `phase` is the mbarrier
-    // parity, flipped three times.
-    static __device__ __forceinline__ void run(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar,
-                                               uint32_t &phase, float (&logit)[NO], long long *ts = nullptr)
+    // ---- UMMA issue, ONE thread each.  Layer 1 (SS): A1 in shared memory (canonical [128][K1]) x W1 -> D1, two halves.
+    static __device__ __forceinline__ void issue_l1(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
     {
-        const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
-        const float *bias = reinterpret_cast<const float *>(image + kBias);
-        constexpr uint32_t idescH = instr_desc_bf16(128, H), idescO = instr_desc_bf16(128, NO);
-#define IM_TS(i) do { if (ts && threadIdx.x == 0) ts[i] = clock64(); } while (0)
-        IM_TS(0);
-        // ---- layer 1 (SS)
-        fence_proxy_async_smem();
-        tc_fence_before();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            tc_fence_after();
-            const uint32_t sa = smem_u32(a1), sb = smem_u32(image + kW1);
+        tc_fence_after();
+        const uint32_t sa = smem_u32(a1), sb = smem_u32(image + kW1);
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
 #pragma unroll
             for (int k = 0; k < K1 / 16; k++)
-                umma_ss(tmem_base, smem_desc(sa + k * 2 * 128 * 16, 128 * 16, 128), smem_desc(sb + k * 2 * H * 16, H * 16, 128), idescH, k > 0);
-            umma_commit(bar);
+                umma_ss(tmem_base + 128 * h, smem_desc(sa + k * 2 * 128 * 16, 128 * 16, 128),
+                        smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
+            umma_commit(h ? bar_b : bar_a);
         }
-        mbar_wait(bar, phase); phase ^= 1u;
+    }
+    // Layer 2 (TS): A2 (TMEM) x W2 -> D2, two halves
+    static __device__ __forceinline__ void issue_l2(const uint8_t *image, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
+    {
         tc_fence_after();
-        IM_TS(1);
-        hidden_epilogue(tlane, 0, bias);
-        IM_TS(2);
-        // ---- layer 2 (TS): A2 = TMEM cols [0, H/2), D2 = cols [H, 2H)
-        tc_fence_before();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            tc_fence_after();
-            const uint32_t sb = smem_u32(image + kW2);
+        const uint32_t sb = smem_u32(image + kW2);
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
 #pragma unroll
             for (int k = 0; k < H / 16; k++)
-                umma_ts(tmem_base + H, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16, H * 16, 128), idescH, k > 0);
-            umma_commit(bar);
+                umma_ts(tmem_base + 128 * h, tmem_base + kColA2 + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
+            umma_commit(h ? bar_b : bar_a);
         }
-        mbar_wait(bar, phase); phase ^= 1u;
+    }
+    // Layer 3 (TS): A3 (TMEM) x W3 -> D3
+    static __device__ __forceinline__ void issue_l3(const uint8_t *image, uint32_t tmem_base, uint64_t *bar)
+    {
         tc_fence_after();
-        IM_TS(3);
-        hidden_epilogue(tlane, H, bias + H);
-        IM_TS(4);
-        // ---- layer 3 (TS): A3 = TMEM cols [H, H + H/2), D3 = cols [0, NO)
-        tc_fence_before();
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            tc_fence_after();
-            const uint32_t sb = smem_u32(image + kW3);
+        const uint32_t sb = smem_u32(image + kW3);
 #pragma unroll
-            for (int k = 0; k < H / 16; k++)
-                umma_ts(tmem_base, tmem_base + H + 8 * k, smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), idescO, k > 0);
-            umma_commit(bar);
-        }
-        mbar_wait(bar, phase); phase ^= 1u;
-        tc_fence_after();
-        IM_TS(5);
+        for (int k = 0; k < H / 16; k++)
+            umma_ts(tmem_base + kColD3, tmem_base + kColA3 + 8 * k, smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
+        umma_commit(bar);
+    }
+    // logits of this thread's row: D3 + b3
+    static __device__ __forceinline__ void load_logits(const uint8_t *image, uint32_t tlane, float (&logit)[NO])
+    {
+        const float *bias = reinterpret_cast<const float *>(image + kBias);
 #pragma unroll
         for (int j = 0; j < NO / 16; j++) {
             uint32_t v[16];
-            tmem_ld16(tlane + 16 * j, v);
+            tmem_ld16(tlane + kColD3 + 16 * j, v);
             tc_wait_ld();
 #pragma unroll
             for (int i = 0; i < 16; i++) logit[16 * j + i] = __uint_as_float(v[i]) + bias[2 * H + 16 * j + i];
         }
-        IM_TS(6);
-#undef IM_TS
-        tc_fence_before();       // the next tile's layer-1 UMMA overwrites D3's columns: order these loads before it
     }
 };
+
+// named barrier over `n` threads (ids 1.. ; 0 is __syncthreads)
+__device__ __forceinline__ void bar_sync(uint32_t id, uint32_t n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 }  // namespace tc
 }  // namespace im
