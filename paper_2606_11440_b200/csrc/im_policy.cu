@@ -141,7 +141,9 @@ __device__ __forceinline__ void exec_epilogue(const Params &P, const RowInfo &ri
 }
 
 // planner decision -> log row, plan word of the query and the stage-0 executor rows (R17)
-__device__ __forceinline__ void plan_commit(const Params &P, const RowInfo &ri, uint32_t topo, uint32_t cnt, uint32_t roles, float lp)
+// claimed_idx0 != ~0u: ring position (reduced modulo regcap) of the row's stage-0 executor rows, claimed by the caller
+__device__ __forceinline__ void plan_commit(const Params &P, const RowInfo &ri, uint32_t topo, uint32_t cnt, uint32_t roles, float lp,
+                                            uint32_t claimed_idx0 = ~0u)
 {
     const uint32_t q = ri.a & 0x3FFu, t_rel = ri.a >> 19;
     const uint32_t keff = keff_of(topo, cnt + 1), nst = nstages_of(topo, keff);
@@ -155,7 +157,7 @@ __device__ __forceinline__ void plan_commit(const Params &P, const RowInfo &ri, 
     const uint32_t pw = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
     env_q(P, ri.env)[q].x = pw | (1u << 9) | (nc << QP_PEND_SHIFT);
     const uint32_t region = ri.env % kRegions;
-    const uint32_t idx0 = rows_claim(P, P.exec, region, nc) % P.exec.regcap;
+    const uint32_t idx0 = claimed_idx0 != ~0u ? claimed_idx0 : rows_claim(P, P.exec, region, nc) % P.exec.regcap;
     write_exec_rows(P, region, idx0, ri.env, q, pw, ri.c & 0xFFFFu, ri.dl, t_rel, a0, nc);
 }
 
@@ -677,9 +679,10 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         float l[NO];
         Net::load_logits(img, tlane, l);
         tc::tc_fence_before();
-        if (!(sl.flags & 1u)) continue;
+        const bool ok = (sl.flags & 1u) != 0;
+        if (EXEC && !ok) continue;
         TcRaw cur;
-        cur.row = sl.row; cur.env = sl.env; cur.gidx = sl.gidx; cur.ok = true; cur.critic = (sl.flags & 2u) != 0;
+        cur.row = sl.row; cur.env = sl.env; cur.gidx = sl.gidx; cur.ok = ok; cur.critic = (sl.flags & 2u) != 0;
         const RowInfo ri = tc_decode_row<EXEC>(P, cur, t0);
         if (EXEC) {
             const uint32_t n = N3;
@@ -701,26 +704,44 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
                 exec_commit(P, ri, d, act, logp, value, t);
             }
         } else {
-            if (P.plan.logits) {
+            uint32_t topo = 0, cnt = 0, roles = 0, nc = 0;
+            float lp = 0.0f;
+            if (ok) {
+                if (P.plan.logits) {
 #pragma unroll
-                for (int i = 0; i < 24; i++) P.plan.logits[(size_t)ri.gidx * 24 + i] = l[i];
+                    for (int i = 0; i < 24; i++) P.plan.logits[(size_t)ri.gidx * 24 + i] = l[i];
+                }
+                const uint32_t q = ri.a & 0x3FFu;
+                const int32_t t = t0 + (int32_t)(ri.a >> 19);
+                const uint32_t gid = P.env_id_base + ri.env;
+                const Ph4 d0 = draw(P, STREAM_PLAN, gid, t, q, 0), d1 = draw(P, STREAM_PLAN, gid, t, q, 1);
+                float lp_t, lp_c, lp_r[4];
+                topo = sample_reg<4, NO>(l, 0, 4, u24(d0.x), lp_t);
+                cnt = sample_reg<4, NO>(l, 4, 4, u24(d0.y), lp_c);
+                const uint32_t ur[4] = {d1.x, d1.y, d1.z, d1.w};
+#pragma unroll
+                for (int a = 0; a < 4; a++) roles |= sample_reg<4, NO>(l, 8 + 4 * a, 4, u24(ur[a]), lp_r[a]) << (2 * a);
+                const uint32_t keff = keff_of(topo, cnt + 1);
+                lp = __fadd_rn(lp_t, lp_c);
+#pragma unroll
+                for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
+                uint32_t a0;
+                stage_calls(topo, keff, 0, a0, nc);
             }
-            const uint32_t q = ri.a & 0x3FFu;
-            const int32_t t = t0 + (int32_t)(ri.a >> 19);
-            const uint32_t gid = P.env_id_base + ri.env;
-            const Ph4 d0 = draw(P, STREAM_PLAN, gid, t, q, 0), d1 = draw(P, STREAM_PLAN, gid, t, q, 1);
-            float lp_t, lp_c, lp_r[4];
-            const uint32_t topo = sample_reg<4, NO>(l, 0, 4, u24(d0.x), lp_t);
-            const uint32_t cnt = sample_reg<4, NO>(l, 4, 4, u24(d0.y), lp_c);
-            const uint32_t ur[4] = {d1.x, d1.y, d1.z, d1.w};
-            uint32_t roles = 0;
+            // one claim per warp: the rows of a tile belong to one region (the tile schedule is per region)
+            const uint32_t lane = threadIdx.x & 31u;
+            uint32_t inc = nc;
 #pragma unroll
-            for (int a = 0; a < 4; a++) roles |= sample_reg<4, NO>(l, 8 + 4 * a, 4, u24(ur[a]), lp_r[a]) << (2 * a);
-            const uint32_t keff = keff_of(topo, cnt + 1);
-            float lp = __fadd_rn(lp_t, lp_c);
-#pragma unroll
-            for (uint32_t a = 0; a < 4; a++) if (a < keff) lp = __fadd_rn(lp, lp_r[a]);
-            plan_commit(P, ri, topo, cnt, roles, lp);
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += v; }
+            const uint32_t tot = __shfl_sync(0xffffffffu, inc, 31), okm = __ballot_sync(0xffffffffu, ok);
+            if (tot) {
+                const uint32_t region = __shfl_sync(0xffffffffu, ri.env % kRegions, __ffs(okm) - 1);
+                uint32_t base = 0;
+                if (lane == 0) base = rows_claim(P, P.exec, region, tot) % P.exec.regcap;
+                uint32_t idx0 = __shfl_sync(0xffffffffu, base, 0) + inc - nc;
+                if (idx0 >= P.exec.regcap) idx0 -= P.exec.regcap;
+                if (ok) plan_commit(P, ri, topo, cnt, roles, lp, idx0);
+            }
         }
     }
     tc::tc_fence_before();
