@@ -101,7 +101,9 @@ __device__ __forceinline__ uint32_t sample_seq(const float *l, float *e, uint32_
 
 // executor decision -> log row + one issue record of its env (R18): {waiting-list key, static word} (im_device.cuh);
 // phase D of the simulation kernel appends it to the env's waiting list.
-__device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, const Ph4 &d, uint32_t act, float logp, float value, int32_t t)
+// `slot_in` != ~0u: issue-list slot of the env already claimed by the caller (claimed early to hide the atomic's latency)
+__device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, const Ph4 &d, uint32_t act, float logp, float value, int32_t t,
+                                            uint32_t slot_in = ~0u)
 {
     const uint32_t q = ri.a & 0x3FFu, agent = (ri.a >> 10) & 3u;
     if (P.log_mode) {
@@ -114,7 +116,7 @@ __device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, 
     out_total = out_total < 1u ? 1u : out_total;
     const uint32_t succ = d.z < P.model[model].succ[depth] ? 1u : 0u;
     uint8_t *rec = env_rec(P, ri.env);
-    const uint32_t slot = atomicAdd(reinterpret_cast<uint32_t *>(rec) + P.hw_misc + 1, 1u);
+    const uint32_t slot = slot_in != ~0u ? slot_in : atomicAdd(reinterpret_cast<uint32_t *>(rec) + P.hw_misc + 1, 1u);
     const uint32_t tm = (uint32_t)(P.sched_mode ? ri.dl : t) & 0xFFFFu;             // R20: deadline (EDF) or issue tick (FCFS)
     if (slot < kIssueCap)
         reinterpret_cast<uint2 *>(rec + P.off_iss)[slot] =
@@ -674,6 +676,8 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         }
         // ---- warpgroup 0: sampling epilogue of row r, logits in registers
         const TcRowSlot sl = rowbuf[128 * (it & 1u) + r];
+        uint32_t islot = ~0u;                              // executor rows: the env's issue-list slot, claimed before the wait
+        if (EXEC && (sl.flags & 3u) == 1u) islot = atomicAdd(reinterpret_cast<uint32_t *>(env_rec(P, sl.row.x)) + P.hw_misc + 1, 1u);
         tc::mbar_wait(&bars[4], phase);
         tc::tc_fence_after();
         float l[NO];
@@ -701,7 +705,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
                 const Ph4 d = draw(P, STREAM_EXEC, P.env_id_base + ri.env, t, q * 4u + agent, 0);
                 float logp;
                 const uint32_t act = sample_reg<48, NO>(l, 0, n, u24(d.x), logp);
-                exec_commit(P, ri, d, act, logp, value, t);
+                exec_commit(P, ri, d, act, logp, value, t, islot);
             }
         } else {
             uint32_t topo = 0, cnt = 0, roles = 0, nc = 0;
