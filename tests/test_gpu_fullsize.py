@@ -1,0 +1,90 @@
+"""Parity at BASELINE.json's full size, in the launch configuration bench.py times (configs[4]: E = 262144, T = 512).
+
+The oracle cannot replay 262144 envs, and a full decision / logit log of 3.2e8 decisions does not fit a test.  So:
+  (1) sampled env ranges are re-run as small contexts with the same global env ids (R2: every draw is keyed by the
+      global env id) AND replayed by the oracle in lock-step (teacher-forced, R25); the small contexts must agree
+      bit for bit with the same columns of the full-size run (trajectory rows, counters, model telemetry);
+  (2) the invariants that hold at any size (P8) are evaluated for every one of the 262144 envs from the counters.
+"""
+import numpy as np
+import pytest
+
+from im_workload import make_policy_blob, make_pool_spec
+from parity import compare_chunk, compare_returns, finish_stats
+
+pytestmark = pytest.mark.gpu
+
+CN = {n: i for i, n in enumerate(("arrivals", "dropped", "finished", "solved", "missed", "calls_issued", "calls_done", "preemptions",
+                                  "sum_sojourn", "sum_live_mid", "plans", "exec_decisions", "sum_running", "sum_waiting",
+                                  "near_boundary", "abandoned"))}
+
+
+def test_cfg5_full_size_sampled_envs_and_invariants():
+    import torch
+    from oracle import oracle as O
+    from paper_2606_11440_b200 import InfraMind, IM_TEL_REW, IM_TEL_COST, IM_TEL_VAL, IM_TEL_MISS, IM_TEL_ADV, IM_TEL_RET
+
+    full = make_pool_spec(5)
+    E, T, N = full.n_envs, full.n_ticks, full.n_models
+    assert (E, T) == (262144, 512)
+    blob = make_policy_blob(full, seed=0)
+    gpu = InfraMind(full, seed=0, debug_flags=1)          # bench.py's configuration
+    gpu.rollout(blob, T)
+    gpu.returns(0.99, 0.95, 0.5)
+    ctr = gpu.counters().astype(np.int64)
+    snap = gpu.snapshot().astype(np.int64)                # [E][N]{n_wait, n_run, kv_used, ewma_q8}
+
+    # ---- (2) invariants for every env (P8)
+    assert np.array_equal(ctr[:, CN["calls_issued"]], ctr[:, CN["calls_done"]] + snap[:, :, 0].sum(1) + snap[:, :, 1].sum(1))
+    assert np.array_equal(ctr[:, CN["calls_issued"]], ctr[:, CN["exec_decisions"]])
+    assert np.all(snap[:, :, 1] <= np.asarray(full.slots, dtype=np.int64)[None, :])
+    assert np.all(snap[:, :, 2] <= np.asarray(full.kv_cap, dtype=np.int64)[None, :])      # kv_preempt = 1
+    assert np.all(ctr[:, CN["finished"]] + ctr[:, CN["dropped"]] <= ctr[:, CN["arrivals"]])
+    assert np.all(ctr[:, CN["arrivals"]] - ctr[:, CN["finished"]] - ctr[:, CN["dropped"]] <= full.qcap)   # live queries
+    assert np.all(ctr[:, CN["solved"]] <= ctr[:, CN["finished"]]) and np.all(ctr[:, CN["missed"]] <= ctr[:, CN["finished"]] + ctr[:, CN["dropped"]])
+    assert np.all(ctr[:, CN["plans"]] == ctr[:, CN["arrivals"]] - ctr[:, CN["dropped"]])
+    assert ctr[:, CN["preemptions"]].sum() > 0 and ctr[:, CN["dropped"]].sum() >= 0
+    # utilisation sweep across env blocks (configs[3]-[4]): the mean running count grows with the level
+    run_lo, run_hi = ctr[: E // 8, CN["sum_running"]].mean(), ctr[-E // 8:, CN["sum_running"]].mean()
+    assert run_hi > 2.0 * run_lo
+
+    # columns of the sampled ranges, gathered on the device (zero-copy views of the arena)
+    bases = [0, 65536 + 37, 200003, E - 40]
+    width = 40
+    cols = torch.cat([torch.arange(b, b + width) for b in bases]).to("cuda")
+    views = {}
+    for name, what, dt in (("rew", IM_TEL_REW, torch.float32), ("cost", IM_TEL_COST, torch.float32), ("val", IM_TEL_VAL, torch.float32),
+                           ("miss", IM_TEL_MISS, torch.uint8), ("adv", IM_TEL_ADV, torch.float32), ("ret", IM_TEL_RET, torch.float32)):
+        gpu.sync()
+        v = gpu.device_tensor(what, dt).view(-1, E)
+        views[name] = v[:, cols].cpu().numpy()
+    gpu.close()
+    del gpu
+    torch.cuda.empty_cache()
+
+    # ---- (1) the same envs as small contexts, against the oracle and against the full-size run
+    for i, b in enumerate(bases):
+        sl = slice(i * width, (i + 1) * width)
+        small = full.with_(n_envs=width, env_id_base=b, env_level=full.env_level[b:b + width].copy(),
+                           log_cap_exec=width * T * 40 + 1024, log_cap_plan=width * T * 32 + 1024, log_cap_query=width * T * 32 + 1024)
+        env_ids = np.arange(b, b + width, dtype=np.uint32)
+        g = InfraMind(small, seed=0, debug_flags=3)
+        o = O.Oracle(small, seed=0, env_ids=env_ids, keep_logits=False)
+        stats = {}
+        for ci, n in enumerate((256, 256)):
+            compare_chunk(g, o, env_ids, n, blob, True, stats, check_state=True)
+            row0 = 256 * ci
+            # the second chunk's rows sit at 256.. in the full-size run (one rollout of 512 ticks)
+            assert np.array_equal(g.rew(), views["rew"][row0:row0 + 256, sl])
+            assert np.array_equal(g.cost(), views["cost"][row0:row0 + 256, sl])
+            assert np.array_equal(g.miss(), views["miss"][row0:row0 + 256, sl])
+            assert np.array_equal(g.val()[:256], views["val"][row0:row0 + 256, sl])
+        finish_stats(o, stats, True)
+        assert np.array_equal(g.counters().astype(np.int64), ctr[b:b + width])
+        assert np.array_equal(g.snapshot().astype(np.int64), snap[b:b + width])
+        # returns of the full-size run on these columns (GAE over 512 ticks) vs the oracle recurrence on the same arrays
+        o_adv, o_ret = O.gae(views["rew"][:T, sl], views["cost"][:T, sl], views["val"][:T + 1, sl], np.zeros((T, width), np.uint8), 0.99, 0.95, 0.5)
+        for gg, oo in ((views["adv"][:T, sl], o_adv), (views["ret"][:T, sl], o_ret)):
+            err = np.abs(gg.astype(np.float64) - oo) / np.maximum(1.0, np.abs(oo))
+            assert err.max() <= 1e-5, err.max()
+        g.close()
