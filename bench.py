@@ -260,9 +260,9 @@ def main():
         tms = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tms, op=dist.ReduceOp.MAX)
         ms = float(tms.item())
-        # the step's one collective: sums behind C-bar over all ranks
-        sums = torch.tensor([sc["sum_cost"], float(sc["n_final"])], device=dev, dtype=torch.float64)
-        dist.all_reduce(sums)
+        # the step's one collective: the four sums behind C-bar / U-bar / sigma_U over all ranks
+        from paper_2606_11440_b200.sharding import allreduce_scalars
+        sc.update(allreduce_scalars(sc, device=dev))
     ms_per_step = ms / args.steps
     env_ticks_per_s = world * E * T / (ms_per_step * 1e-3)
     model = algorithmic_model(spec, csum, T, E)
@@ -297,6 +297,15 @@ def main():
         else:
             pk = 148 * 128 * 2 * 1.965e9 / 1e12       # fp32 FFMA: 148 SMs x 128 lanes x 2 flop x max clock
             roof = {"bound": "alu", "kernel": f"k_policy_f32<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None}
+    # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this command, if any
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            tr = json.load(f).get(f"cfg{cfg}", {}).get(roof["kernel"].split("<")[0])
+        roof["traffic"] = tr["dram_bytes_per_launch"] / 1e9 if tr and E == CONFIGS[cfg]["E"] else None
+        if tr:
+            roof["traffic_source"] = tr["source"]
+    except (OSError, ValueError, KeyError):
+        pass
     roof["peak_source"] = f"MEASURED_PEAKS.json ({peaks['src']})"
     roof["kernel_share_of_step"] = share
     roof["kernel_ms_per_launch"] = per_launch_ms
