@@ -287,16 +287,16 @@ def main():
     bf16 = spec.policy_dtype == 1
     if dominant == "sim":
         achieved = model["sim_bytes"] / n_l["sim"] / (per_launch_ms["sim"] * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k_sim", "achieved": achieved, "peak": peaks["hbm"], "unit": "GB/s", "frac": achieved / peaks["hbm"], "traffic": None}
+        roof = {"bound": "hbm", "kernel": "k_sim", "achieved": achieved, "peak": peaks["hbm"], "unit": "GB/s", "frac": achieved / peaks["hbm"], "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
     else:
         fl = model["exec_flops"] if dominant == "exec" else model["plan_flops"]
         achieved = fl / n_l[dominant] / (per_launch_ms[dominant] * 1e-3) / 1e12
         if bf16:
             pk = peaks["bf16_sustained"]
-            roof = {"bound": "tensor", "kernel": f"k_policy_bf16<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None}
+            roof = {"bound": "tensor", "kernel": f"k_policy_bf16<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
         else:
             pk = 148 * 128 * 2 * 1.965e9 / 1e12       # fp32 FFMA: 148 SMs x 128 lanes x 2 flop x max clock
-            roof = {"bound": "alu", "kernel": f"k_policy_f32<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None}
+            roof = {"bound": "alu", "kernel": f"k_policy_f32<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
     # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this command, if any
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
