@@ -25,7 +25,7 @@ constexpr int kSimThreads = 256;
 
 // ---- per-group shared memory layout (bytes)
 struct SimLayout {
-    uint32_t o_hdr, o_pref, o_small, o_clist, total;
+    uint32_t o_hdr, o_pref, o_small, o_clist, o_glist, total;
 };
 // small per-env arrays (u32 words): 16 per model-indexed array
 enum : uint32_t { SM_LATSUM = 0, SM_LATN = 16, SM_RELKV = 32, SM_RELNRUN = 48, SM_KVADD = 64, SM_OCCCLR = 80, SM_AMIN = 112,
@@ -39,6 +39,7 @@ __host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW,
     L.o_pref = o; o += up((QW + 1) * 4);
     L.o_small = o; o += up(kSmallWords * 4);
     L.o_clist = o; o += up(SP * 2);              // every slot may complete in one tick
+    L.o_glist = o; o += 128;                     // non-empty slot groups of the tick (u8 each)
     L.total = o;
     return L;
 }
@@ -155,6 +156,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     uint32_t *s_sc = s_small + SM_SC;                 // [0] ccnt, [1] rew, [2] miss, [3] removals, [4..5] cost (u64)
     unsigned long long *s_cost = (unsigned long long *)(s_sc + 4);
     uint16_t *s_clist = (uint16_t *)(sm + L.o_clist); // completed requests: global slot index
+    uint8_t *s_glist = (uint8_t *)(sm + L.o_glist);
 
     uint8_t *rec = env_rec(P, e);
     uint32_t *hot = (uint32_t *)(rec + P.off_hot), *wkey = (uint32_t *)(rec + P.off_wkey);
@@ -302,15 +304,28 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 const uint32_t k = s_gmodel[gi], sl0 = gi * 8 - s_sbase[k];       // first slot of the group within its model
                 return (s_occ[2 * k + (sl0 >> 5)] >> (sl0 & 31)) & 0xFFu;
             };
-            uint4 na = make_uint4(0, 0, 0, 0), nb = na;
-            uint32_t nocc = 0;
-            if (gl < n_grp) { nocc = occ8_of(gl); na = pre_a; nb = pre_b; }
-            for (uint32_t g0 = 0; g0 < n_grp; g0 += G) {
+            // Lane gl takes group gl first (its words came with the header); the non-empty groups beyond the first G are
+            // compacted into a list, so that later iterations keep all lanes busy whatever the load of the pool.
+            uint32_t n_list = 0;
+#pragma unroll 1
+            for (uint32_t g0 = G; g0 < n_grp; g0 += G) {
                 const uint32_t gi = g0 + gl;
+                const bool ne = gi < n_grp && occ8_of(gi) != 0;
+                const uint32_t m = g.ballot(ne);
+                if (ne) s_glist[n_list + __popc(m & lt_mask)] = (uint8_t)gi;
+                n_list += __popc(m);
+            }
+            g.sync();
+            const uint32_t n_it = 1 + (n_list + G - 1) / G;
+            uint4 na = pre_a, nb = pre_b;
+            uint32_t ngi = gl, nocc = gl < n_grp ? occ8_of(gl) : 0u;
+#pragma unroll 1
+            for (uint32_t it = 0; it < n_it; it++) {
+                const uint32_t gi = ngi;
                 const uint4 ha = na, hb = nb;
                 const uint32_t occ8 = nocc;
                 nocc = 0;
-                if (gi + G < n_grp) { nocc = occ8_of(gi + G); if (nocc) { na = hot4[2 * (gi + G)]; nb = hot4[2 * (gi + G) + 1]; } }
+                if (it * G + gl < n_list) { ngi = s_glist[it * G + gl]; nocc = occ8_of(ngi); na = hot4[2 * ngi]; nb = hot4[2 * ngi + 1]; }
                 if (occ8) {
                     const uint32_t k = s_gmodel[gi], base = s_base[k], thr = s_thr[k];
                     const Ph4 u4 = draw(P, STREAM_SVC, gid, t, gi, 0);
