@@ -648,14 +648,22 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     }
     uint32_t phase = 0, it = 0;
     for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
-        // ---- hidden layer 1: warpgroup w takes columns [128 w, 128 w + 128) as soon as its half is ready
-        tc::mbar_wait(&bars[wg], phase);
-        tc::tc_fence_after();
-        Net::half_epilogue(tlane, 128 * wg, Net::kColA2 + 64 * wg, bias + 128 * wg);
-        tc::tc_fence_before();
-        __syncthreads();
-        if (threadIdx.x == 0) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
-        // ---- hidden layer 2
+        if (wg == 1) {
+            // ---- warpgroup 1 owns hidden layer 1: half a while the tensor core computes half b, then layer 2's issue.
+            // Its packed output A2 overlaps the columns of the previous tile's D3: wait until warpgroup 0 has the logits.
+            if (it > 0) tc::bar_sync(3, 256);
+            tc::mbar_wait(&bars[0], phase);
+            tc::tc_fence_after();
+            Net::half_epilogue(tlane, 0, Net::kColA2, bias);
+            tc::mbar_wait(&bars[1], phase);
+            tc::tc_fence_after();
+            Net::half_epilogue(tlane, 128, Net::kColA2 + 64, bias + 128);
+            tc::tc_fence_before();
+            tc::bar_sync(2, 128);
+            if (r == 0) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
+        }
+        // ---- hidden layer 2: warpgroup w takes columns [128 w, 128 w + 128) as soon as its half is ready
+        // (warpgroup 0 arrives here from the sampling epilogue of the previous tile)
         tc::mbar_wait(&bars[2 + wg], phase);
         tc::tc_fence_after();
         Net::half_epilogue(tlane, 128 * wg, Net::kColA3 + 64 * wg, bias + kTcH + 128 * wg);
@@ -683,6 +691,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         float l[NO];
         Net::load_logits(img, tlane, l);
         tc::tc_fence_before();
+        if (tile + gridDim.x < total) tc::bar_arrive(3, 256);   // warpgroup 1 may now overwrite D3's columns
         const bool ok = (sl.flags & 1u) != 0;
         if (EXEC && !ok) continue;
         TcRaw cur;

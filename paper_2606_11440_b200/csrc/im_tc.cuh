@@ -155,8 +155,9 @@ __host__ __device__ constexpr uint32_t canon_off(uint32_t rows, uint32_t r, uint
 //   [ W1 canon [H][K1] | W2 canon [H][H] | W3 canon [NO][H] | b1[H] b2[H] b3[NO] fp32 ]
 //
 // Two warpgroups (256 threads) work on one 128-row tile; every hidden layer is computed as two N-halves of 128
-// columns with their own mbarrier, so that warpgroup 0 runs the tanh epilogue of half a while the tensor core still
-// computes half b (which warpgroup 1 then takes).  TMEM map (512 columns, H = 256):
+// columns with their own mbarrier, so that the tanh epilogue of half a runs while the tensor core still computes
+// half b.  Warpgroup 1 owns layer 1 (gather, both epilogue halves, issue of layer 2) and half b of layer 2;
+// warpgroup 0 owns half a of layer 2 and the sampling epilogue, which thus overlaps the next tile's layer 1.  TMEM map (512 columns, H = 256):
 //   D1 = [0,256)  ->  A2 = [256,384)  ;  D2 = [0,256)  ->  A3 = [384,512)  ;  D3 = [256,256+NO)
 // Nothing is packed in place, and the next tile's layer 1 (D1) touches no column the sampling epilogue (D3) reads.
 template <int K1, int H, int NO>
@@ -242,6 +243,7 @@ struct TcMlp {
 
 // named barrier over `n` threads (ids 1.. ; 0 is __syncthreads)
 __device__ __forceinline__ void bar_sync(uint32_t id, uint32_t n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(uint32_t id, uint32_t n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 }  // namespace tc
 }  // namespace im
