@@ -515,6 +515,21 @@ __device__ __forceinline__ uint32_t sample_reg(const float (&l)[NO], int off, ui
 
 struct TcRaw { uint4 row; uint32_t env, gidx; bool ok, critic; };
 
+// Loads of the NEXT tile's inputs are issued one tile ahead of their use; `asm volatile` keeps ptxas from sinking them
+// to the point of use (measured: the feature build then waits two dependent round trips, 1.5 us per tile).
+__device__ __forceinline__ uint4 ld_early_u4(const uint4 *p)
+{
+    uint4 v;
+    asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ float4 ld_early_f4(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+    return v;
+}
+
 // row `r` of tile `tile`: issues the row load, decodes nothing (the consumer decodes after the latency has passed)
 __device__ __forceinline__ TcRaw tc_fetch_row(const TileSched &S, const RowBuf &rb, uint32_t tile, uint32_t r, uint32_t n_crit)
 {
@@ -532,7 +547,7 @@ __device__ __forceinline__ TcRaw tc_fetch_row(const TileSched &S, const RowBuf &
     const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * 128u + r;
     if (idx >= rb.cnt[lo]) return x;
     x.gidx = row_gid(rb, lo, idx);
-    x.row = rb.row[x.gidx];
+    x.row = ld_early_u4(rb.row + x.gidx);
     x.ok = true;
     return x;
 }
@@ -589,13 +604,14 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
     const float *bias = reinterpret_cast<const float *>(img + Net::kBias);
     const uint32_t total = sched.total;
+    uint32_t phase = 0, it = 0;                           // mbarrier parity and tile counter of this CTA
 
     // snapshot floats of a row's env (R14): up to 12 float4 per thread, issued early, consumed one tile later
     auto fetch_snap = [&](const TcRaw &x, float4 (&sn)[12]) {
         const uint32_t env = x.critic ? x.env : x.row.x;
         const float4 *src = reinterpret_cast<const float4 *>(P.snap + (size_t)env * N3);
 #pragma unroll
-        for (int j = 0; j < 12; j++) sn[j] = (x.ok && vec && (uint32_t)(4 * j) < N3) ? __ldg(src + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int j = 0; j < 12; j++) sn[j] = (x.ok && vec && (uint32_t)(4 * j) < N3) ? ld_early_f4(src + j) : make_float4(0.f, 0.f, 0.f, 0.f);
     };
     // features of row `cur` -> A1 (bf16 RNE), canonical layout: chunk c of row r at c * 2048 + r * 16; row -> rowbuf
     auto build_a1 = [&](const TcRaw &cur, const float4 (&sn)[12], TcRowSlot *slot) {
@@ -603,9 +619,22 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         const bool ok = cur.ok;
         slot[r].row = cur.row; slot[r].env = cur.env; slot[r].gidx = cur.gidx; slot[r].flags = (ok ? 1u : 0u) | (cur.critic ? 2u : 0u);
         if (vec) {
-            float tl[16];                                 // the 12 features behind the snapshot block, then zeros
+            float tl[16];                                 // the 12 features behind the snapshot block (R15), then zeros
 #pragma unroll
-            for (int j = 0; j < 16; j++) tl[j] = (ok && j < 12) ? feature(P, EXEC, ri, j == 0 ? 0u : N3 + (uint32_t)j) : 0.0f;
+            for (int j = 0; j < 16; j++) tl[j] = 0.0f;
+            if (ok) {
+                tl[0] = ri.b;
+                if (!ri.critic) {
+                    tl[1] = __uint2float_rn(ri.c & 0xFFFFu) * 0x1p-13f;
+                    if (EXEC) {
+                        const uint32_t topo = (ri.a >> 12) & 3u, role = (ri.a >> 14) & 3u;
+#pragma unroll
+                        for (int j = 0; j < 4; j++) { tl[2 + j] = (uint32_t)j == topo ? 1.0f : 0.0f; tl[6 + j] = (uint32_t)j == role ? 1.0f : 0.0f; }
+                        tl[10] = __uint2float_rn((ri.a >> 10) & 3u) * 0.25f;
+                        tl[11] = __uint2float_rn((ri.a >> 16) & 7u) * 0.25f;
+                    }
+                }
+            }
             const uint32_t c0 = N3 / 8;
 #pragma unroll
             for (int c = 0; c < kTcK1 / 8; c++) {
@@ -646,7 +675,6 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             fetch_snap(nxt, sn);
         }
     }
-    uint32_t phase = 0, it = 0;
     for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
         if (wg == 1) {
             // ---- warpgroup 1 owns hidden layer 1: half a while the tensor core computes half b, then layer 2's issue.
@@ -661,6 +689,11 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             tc::tc_fence_before();
             tc::bar_sync(2, 128);
             if (r == 0) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
+            // while the tensor core runs layer 2: the next tile's features (layer 1 of this tile is done with a1)
+            if (tile + gridDim.x < total) {
+                build_a1(nxt, sn, rowbuf + 128 * ((it + 1) & 1u));
+                tc::fence_proxy_async_smem();
+            }
         }
         // ---- hidden layer 2: warpgroup w takes columns [128 w, 128 w + 128) as soon as its half is ready
         // (warpgroup 0 arrives here from the sampling epilogue of the previous tile)
@@ -671,11 +704,8 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         __syncthreads();
         if (threadIdx.x == 0) Net::issue_l3(img, tmem_base, &bars[4]);
         if (wg == 1) {
-            // ---- warpgroup 1: features of the next tile, its layer 1, then the row loads of the tile after it
-            if (tile + gridDim.x < total) {
-                build_a1(nxt, sn, rowbuf + 128 * ((it + 1) & 1u));
-                tc::fence_proxy_async_smem();
-                tc::bar_sync(2, 128);
+            // ---- warpgroup 1: layer 1 of the next tile, then the row loads of the tile after it
+            if (tile + gridDim.x < total) {     // a1 was written before the __syncthreads above
                 if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
                 nxt = tc_fetch_row(sched, rb, tile + 2 * gridDim.x, r, n_crit);
                 fetch_snap(nxt, sn);

@@ -174,15 +174,17 @@ struct TcMlp {
     // `tlane` = TMEM address of this warp's lane quarter at column 0 of the allocation.
     static __device__ __forceinline__ void half_epilogue(uint32_t tlane, uint32_t src, uint32_t dst, const float *bias)
     {
-#pragma unroll 1
+        uint32_t v[2][32];
+        tmem_ld32(tlane + src, v[0]);
+#pragma unroll
         for (int j = 0; j < 4; j++) {
-            uint32_t v[32], o[16];
-            tmem_ld32(tlane + src + 32 * j, v);
+            uint32_t o[16];
             tc_wait_ld();
+            if (j + 1 < 4) tmem_ld32(tlane + src + 32 * (j + 1), v[(j + 1) & 1]);   // flies while chunk j is processed
 #pragma unroll
             for (int i = 0; i < 16; i++) {
                 const float2 b = *reinterpret_cast<const float2 *>(bias + 32 * j + 2 * i);
-                o[i] = pack_bf16(tanh_approx(__uint_as_float(v[2 * i]) + b.x), tanh_approx(__uint_as_float(v[2 * i + 1]) + b.y));
+                o[i] = pack_bf16(tanh_approx(__uint_as_float(v[j & 1][2 * i]) + b.x), tanh_approx(__uint_as_float(v[j & 1][2 * i + 1]) + b.y));
             }
             tmem_st16(tlane + dst + 16 * j, o);
         }
