@@ -301,6 +301,10 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
         P.flags = s.debug_flags; P.has_intok = c->tab_intok.empty() ? 0 : 1;
         P.seed_lo = (uint32_t)c->seed; P.seed_hi = (uint32_t)(c->seed >> 32);
         P.f_in = F; P.hidden = H; P.log_mode = log ? 1 : 0;
+        for (uint32_t r = 0; r < 10; r++) {      // R2: key = (seed_lo, seed_hi ^ stream), Weyl increments per round
+            P.svc_rk[2 * r] = P.seed_lo + r * 0x9E3779B9u;
+            P.svc_rk[2 * r + 1] = (P.seed_hi ^ (uint32_t)STREAM_SVC) + r * 0xBB67AE85u;
+        }
         for (uint32_t k = 0; k < N; k++) {
             const im_model_spec &m = s.model[k];
             P.model[k] = ModelTab{m.rate_tok_s, m.slots, m.kv_cap, m.prefill_us_per_ktok, {m.succ_thresh[0], m.succ_thresh[1], m.succ_thresh[2]}, m.kv_inv};

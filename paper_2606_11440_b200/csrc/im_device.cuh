@@ -77,6 +77,7 @@ struct Params {
     uint32_t f_in, hidden, log_mode, pad0;
     ModelTab model[kMaxModels];
     uint32_t slot_base[kMaxModels + 1];      // first global slot of each model (multiples of 8)
+    uint32_t svc_rk[20];                     // Philox round keys of the service stream (k0, k1 per round): constant-bank operands
     // per-env record
     uint8_t *env_base;
     unsigned long long env_stride;           // bytes, multiple of 128
@@ -115,6 +116,19 @@ __device__ __forceinline__ Ph4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t 
         c0 = hi1 ^ c1 ^ k0; c1 = lo1;
         c2 = hi0 ^ c3 ^ k1; c3 = lo0;
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return Ph4{c0, c1, c2, c3};
+}
+
+// the same with the 10 round keys precomputed (k_r = k + r * Weyl): saves the two key additions of every round
+__device__ __forceinline__ Ph4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20])
+{
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ rk[2 * r]; c1 = lo1;
+        c2 = hi0 ^ c3 ^ rk[2 * r + 1]; c3 = lo0;
     }
     return Ph4{c0, c1, c2, c3};
 }

@@ -328,7 +328,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 if (it * G + gl < n_list) { ngi = s_glist[it * G + gl]; nocc = occ8_of(ngi); na = hot4[2 * ngi]; nb = hot4[2 * ngi + 1]; }
                 if (occ8) {
                     const uint32_t k = s_gmodel[gi], base = s_base[k], thr = s_thr[k];
-                    const Ph4 u4 = draw(P, STREAM_SVC, gid, t, gi, 0);
+                    const Ph4 u4 = philox4x32_10_rk(gid, (uint32_t)t, gi, 0u, P.svc_rk);
                     const uint32_t uw[4] = {u4.x, u4.y, u4.z, u4.w};
                     uint32_t hh[8] = {ha.x, ha.y, ha.z, ha.w, hb.x, hb.y, hb.z, hb.w};
                     uint32_t tot = 0;
