@@ -1,0 +1,64 @@
+"""GPU parity on the degenerate and extreme cases of the path (through the C ABI, vs the oracle, element by element)."""
+import numpy as np
+import pytest
+
+from helpers import tiny_spec
+from im_workload import make_policy_blob
+from test_gpu_parity import _run
+
+pytestmark = pytest.mark.gpu
+
+
+def test_no_arrivals_everything_stays_zero():
+    """Empty input: arrival rate 0 => no query, no decision, all-zero trajectories; V[t] is the critic on a zero snapshot."""
+    from paper_2606_11440_b200 import InfraMind
+    spec = tiny_spec(n_envs=19, N=3, n_ticks=40, qcap=32, rcap=128, rate_tick=0.0, slots=4, f_in=32, hidden=32)
+    _run(spec, seed=1, chunks=[1, 39])
+    g = InfraMind(spec, seed=1, debug_flags=1)
+    g.rollout(make_policy_blob(spec), 40)
+    assert not g.rew().any() and not g.cost().any() and not g.miss().any() and not g.counters().any()
+    assert np.all(g.val() == g.val()[0, 0])
+    g.close()
+
+
+def test_full_query_table_drops_and_long_waiting_list():
+    """Overload far beyond capacity: the query table fills (tail drops, R9: miss + cost 1.0 per drop), the waiting list
+    reaches its bound of 3 calls per live query, admission scans a long list every tick."""
+    spec = tiny_spec(n_envs=21, N=2, n_ticks=160, qcap=32, rcap=128, rate_tick=3.0, slots=2, rates=[60, 45], budget=(20, 90),
+                     medians=(200, 400, 800), f_in=32, hidden=32, seed=8)
+    st = _run(spec, seed=2, chunks=[1] * 30 + [130])
+    assert st["decisions"] > 500 and st["dropped"] > 1000 and st["finished"] > 5
+
+
+def test_sixteen_models_extreme_slot_counts_and_largest_tables():
+    """N = 16 with slot counts 1 .. 64 (a lane's 8 slots never straddle two models), qcap = 1024 (12-bit request ids),
+    KV pressure with preemption on a few models, prefill, fp32 policy (decisions bit-exact)."""
+    slots = [1, 64, 8, 3, 17, 64, 2, 40, 9, 1, 33, 5, 64, 12, 7, 24]
+    kv = [4000, 30000, 6000, 5000, 9000, 25000, 4000, 20000, 6000, 4000, 15000, 5000, 28000, 8000, 5000, 12000]
+    spec = tiny_spec(n_envs=9, N=16, n_ticks=150, qcap=1024, rcap=3072, rate_tick=2.2, slots=slots, kv_cap=kv, kv_preempt=1,
+                     budget=(30, 400), medians=(150, 500, 1200), in_tok=600, prefill=900, f_in=64, hidden=32, seed=12)
+    st = _run(spec, seed=3, chunks=[1] * 10 + [140])
+    assert st["decisions"] > 500 and st["preemptions"] > 0
+
+
+def test_single_model_single_slot():
+    """N = 1, S = 1: the M/M/1 shape of pin P6 on the GPU path (every admission waits for the one slot)."""
+    spec = tiny_spec(n_envs=17, N=1, n_ticks=300, qcap=64, rcap=256, rate_tick=0.06, slots=1, rates=[80], budget=(100, 900),
+                     medians=(40, 80, 160), f_in=32, hidden=16, seed=4)
+    _run(spec, seed=4, chunks=[300])
+
+
+def test_clock_limit_is_an_error_not_a_wraparound():
+    """Device state keeps absolute ticks in 16 bits: im_rollout refuses to run past tick + budget >= 65536."""
+    from paper_2606_11440_b200 import InfraMind, IMError
+    spec = tiny_spec(n_envs=4, N=1, n_ticks=8000, qcap=32, rcap=128, rate_tick=0.01, slots=2, f_in=32, hidden=16, budget=(10, 1000))
+    g = InfraMind(spec, seed=0, debug_flags=0)
+    blob = make_policy_blob(spec)
+    for _ in range(8):
+        g.rollout(blob, 8000)
+    with pytest.raises(IMError) as ei:
+        g.rollout(blob, 8000)           # 64000 + 8000 + 1000 >= 65536
+    assert ei.value.code == -6
+    g.reset()
+    g.rollout(blob, 100)                # the clock restarts with im_reset
+    g.close()

@@ -26,6 +26,8 @@ def _run(spec, seed, chunks, blob=None, env_ids=None, gamma=0.99, lam=0.95, mu=0
         compare_chunk(gpu, orc, env_ids, n, blob, bf16, stats)
     finish_stats(orc, stats, bf16)
     compare_returns(gpu, orc, env_ids, gamma, lam, mu, bf16, whole_batch=(len(env_ids) == spec.n_envs))
+    csum = gpu.counters().sum(axis=0)
+    stats.update(arrivals=int(csum[0]), dropped=int(csum[1]), finished=int(csum[2]), preemptions=int(csum[7]))
     gpu.close()
     return stats
 
