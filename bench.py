@@ -299,11 +299,12 @@ def main():
             roof = {"bound": "alu", "kernel": f"k_policy_f32<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
     # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this command, if any
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            tr = json.load(f).get(f"cfg{cfg}", {}).get(roof["kernel"].split("<")[0])
-        roof["traffic"] = tr["dram_bytes_per_launch"] / 1e9 if tr and E == CONFIGS[cfg]["E"] else None
-        if tr:
-            roof["traffic_source"] = tr["source"]
+        import csv
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["config"] == f"cfg{cfg}" and row["kernel"] == roof["kernel"].split("<")[0] and E == CONFIGS[cfg]["E"]:
+                    roof["traffic"] = float(row["dram_bytes_per_launch"]) / 1e9
+                    roof["traffic_source"] = row["source"]
     except (OSError, ValueError, KeyError):
         pass
     roof["peak_source"] = f"MEASURED_PEAKS.json ({peaks['src']})"

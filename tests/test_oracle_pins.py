@@ -279,7 +279,7 @@ def test_p9_queue_order_and_admission_brute_force(orc, sched_mode):
             for k in range(2):
                 w = np.nonzero((st["r_state"][e] == ST_WAIT) & (st["r_model"][e] == k))[0]
                 base = st["r_deadline"][e][w] if sched_mode else st["r_issue"][e][w]
-                ref = w[np.lexsort((w, base))]     # repeated arg-min over (base, ridx)
+                ref = w[np.lexsort((w, base))]     # repeated arg-min over (base, request id = 4 q + agent)
                 got = o.queue_order(e, k, tnow)
                 assert np.array_equal(got, ref)
                 checked += len(w)
@@ -546,7 +546,7 @@ def test_p19_preemption_victim_and_token_conservation(orc):
                                        & (prev["r_issue"][e] == st["r_issue"][e])))[0]
                 running = np.nonzero(st["r_state"][e] == ST_RUN)[0]
                 if len(evicted) and len(running):
-                    # every victim has a larger (deadline, ridx) than every survivor
+                    # every victim has a larger (deadline, request id) than every survivor
                     vmin = min((int(st["r_deadline"][e][i]), int(i)) for i in evicted)
                     smax = max((int(st["r_deadline"][e][i]), int(i)) for i in running)
                     assert vmin > smax
