@@ -88,3 +88,22 @@ def test_cfg5_full_size_sampled_envs_and_invariants():
             err = np.abs(gg.astype(np.float64) - oo) / np.maximum(1.0, np.abs(oo))
             assert err.max() <= 1e-5, err.max()
         g.close()
+
+
+def test_cfg5_many_ctas_run_to_run_determinism():
+    """A race between lanes, groups or CTAs would show as run-to-run differences once every SM is busy: 32768 envs of
+    configs[4] (2048 CTAs of k_sim, persistent policy kernels on all SMs), 160 ticks, twice, bit for bit."""
+    from paper_2606_11440_b200 import InfraMind
+    spec = make_pool_spec(5, n_envs=32768, n_ticks=160)
+    blob = make_policy_blob(spec, seed=0)
+    g = InfraMind(spec, seed=3, debug_flags=1)
+    outs = []
+    for _ in range(2):
+        g.reset()
+        g.rollout(blob, 160)
+        g.returns(0.99, 0.95, 0.5)
+        outs.append((g.rew(), g.cost(), g.val(), g.miss(), g.counters(), g.snapshot(), g.adv()))
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+    assert outs[0][4][:, CN["exec_decisions"]].sum() > 1_000_000
+    g.close()
