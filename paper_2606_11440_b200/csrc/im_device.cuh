@@ -146,7 +146,11 @@ __device__ __forceinline__ float im_exp(float x)
 {
     // branch-free (the x < -80 case is a select at the end): 48 of these per executor decision must interleave, and an
     // early return keeps the compiler from overlapping their dependent chains (measured: 8600 -> cycles per tile)
-    const float n = rintf(__fmul_rn(x, 0x1.715476p+0f));
+    // n = rintf(x log2e) without the conversion unit: adding 1.5 * 2^23 rounds to an integer (RNE, |x log2e| < 2^22) and
+    // leaves that integer in the low bits of the sum; 2^n is then an add into the exponent field of p (exact: the
+    // result is normal for n >= -116).  Same values as rintf / ldexpf, two FADDs and two integer ops.
+    const float t = __fadd_rn(__fmul_rn(x, 0x1.715476p+0f), 12582912.0f);
+    const float n = __fsub_rn(t, 12582912.0f);
     float r = __fmaf_rn(n, -0x1.62e400p-1f, x);
     r = __fmaf_rn(n, -0x1.7f7d1cp-20f, r);
     float p = 0x1.6c16c2p-10f;
@@ -156,7 +160,7 @@ __device__ __forceinline__ float im_exp(float x)
     p = __fmaf_rn(p, r, 0.5f);
     p = __fmaf_rn(p, r, 1.0f);
     p = __fmaf_rn(p, r, 1.0f);
-    const float y = __fmul_rn(p, __int_as_float(((int)n + 127) << 23));   // exact scaling by 2^n, n in [-116, 0]
+    const float y = __int_as_float(__float_as_int(p) + (__float_as_int(t) << 23));   // p * 2^n (the low 9 bits of the magic are 0)
     return x < -80.0f ? 0.0f : y;
 }
 

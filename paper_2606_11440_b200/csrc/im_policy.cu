@@ -483,32 +483,35 @@ void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t
     else k_pack_tc<false><<<64, 256, 0, st>>>(W, 3 * n_models);
 }
 
-// R24 sampler on logits held in registers: l[off .. off+n), n <= NMAX.  Same operation sequence as sample_seq.
+// R24 sampler on logits held in registers: l[off .. off+n), n <= NMAX.  Same VALUES as sample_seq, arranged for a lone
+// warp, which pays ~5 cycles per instruction here (profiles/r1_ncu_final_cfg5.md): logits beyond n become -inf (their
+// exponential is exactly 0, so the running sums simply stop growing); the max is a tree (exact); the sums
+// c_i = c_{i-1} + e_i are computed once in ascending order (Z is the last); since they never decrease, the first i
+// with c_i > u Z is the NUMBER of i with c_i <= u Z (capped at n - 1).
 template <int NMAX, int NO>
 __device__ __forceinline__ uint32_t sample_reg(const float (&l)[NO], int off, uint32_t n, float u, float &logp)
 {
-    float m = l[off];
+    float c[NMAX], mx[NMAX];
 #pragma unroll
-    for (int i = 1; i < NMAX; i++) if ((uint32_t)i < n) m = fmaxf(m, l[off + i]);
-    float e[NMAX];
+    for (int i = 0; i < NMAX; i++) { c[i] = (uint32_t)i < n ? l[off + i] : -INFINITY; mx[i] = c[i]; }
 #pragma unroll
-    for (int i = 0; i < NMAX; i++) e[i] = im_exp(__fsub_rn(l[off + i], m));
-    float Z = 0.0f;
+    for (int s = 1; s < NMAX; s <<= 1)
 #pragma unroll
-    for (int i = 0; i < NMAX; i++) if ((uint32_t)i < n) Z = __fadd_rn(Z, e[i]);
+        for (int i = 0; i + s < NMAX; i += 2 * s) mx[i] = fmaxf(mx[i], mx[i + s]);
+    const float m = mx[0];
+#pragma unroll
+    for (int i = 0; i < NMAX; i++) c[i] = im_exp(__fsub_rn(c[i], m));
+#pragma unroll
+    for (int i = 1; i < NMAX; i++) c[i] = __fadd_rn(c[i - 1], c[i]);          // c_0 = 0 + e_0 = e_0
+    const float Z = c[NMAX - 1];
     const float th = __fmul_rn(u, Z);
-    uint32_t a = n - 1;
-    float la = l[off], c = 0.0f;
-    bool found = false;
+    uint32_t cnt = 0;
 #pragma unroll
-    for (int i = 0; i < NMAX; i++) {
-        if ((uint32_t)i < n) {
-            c = __fadd_rn(c, e[i]);
-            const bool hit = !found && c > th;
-            if (hit || (!found && (uint32_t)i == n - 1)) { a = (uint32_t)i; la = l[off + i]; }
-            found = found || hit;
-        }
-    }
+    for (int i = 0; i < NMAX; i++) cnt += c[i] <= th ? 1u : 0u;
+    const uint32_t a = min(cnt, n - 1u);
+    float la = l[off];
+#pragma unroll
+    for (int i = 1; i < NMAX; i++) la = (uint32_t)i == a ? l[off + i] : la;
     logp = __fsub_rn(__fsub_rn(la, m), logf(Z));
     return a;
 }
