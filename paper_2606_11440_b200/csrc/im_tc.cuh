@@ -140,6 +140,17 @@ __device__ __forceinline__ float tanh_approx(float x)
     asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// (a.x + b.x, a.y + b.y) in one instruction (sm_100 packed fp32 add; each half rounds like a scalar add.rn)
+__device__ __forceinline__ float2 fadd2(uint32_t ax, uint32_t ay, float2 b)
+{
+    unsigned long long ra, rb, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "r"(ax), "r"(ay));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
     const __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
@@ -184,7 +195,8 @@ struct TcMlp {
 #pragma unroll
             for (int i = 0; i < 16; i++) {
                 const float2 b = *reinterpret_cast<const float2 *>(bias + 32 * j + 2 * i);
-                o[i] = pack_bf16(tanh_approx(__uint_as_float(v[j & 1][2 * i]) + b.x), tanh_approx(__uint_as_float(v[j & 1][2 * i + 1]) + b.y));
+                const float2 y = fadd2(v[j & 1][2 * i], v[j & 1][2 * i + 1], b);
+                o[i] = pack_bf16(tanh_approx(y.x), tanh_approx(y.y));
             }
             tmem_st16(tlane + dst + 16 * j, o);
         }
