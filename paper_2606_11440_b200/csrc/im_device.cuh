@@ -164,6 +164,36 @@ __device__ __forceinline__ float im_exp(float x)
     return x < -80.0f ? 0.0f : y;
 }
 
+// Two im_exp at once with the packed fp32 instructions of sm_100 (mul / add / fma .f32x2: each half rounds exactly like
+// the scalar operation, so the values are those of im_exp bit for bit); 19 instructions per pair instead of 32.
+struct F2 { unsigned long long v; };
+__device__ __forceinline__ F2 f2_pack(float a, float b) { F2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void f2_unpack(F2 p, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(p.v)); }
+__device__ __forceinline__ F2 f2_mul(F2 a, F2 b) { F2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ F2 f2_add(F2 a, F2 b) { F2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ F2 f2_fma(F2 a, F2 b, F2 c) { F2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
+__device__ __forceinline__ void im_exp_x2(float x0, float x1, float &y0, float &y1)
+{
+    const F2 x = f2_pack(x0, x1), magic = f2_pack(12582912.0f, 12582912.0f), nmagic = f2_pack(-12582912.0f, -12582912.0f);
+    const F2 t = f2_add(f2_mul(x, f2_pack(0x1.715476p+0f, 0x1.715476p+0f)), magic);
+    const F2 n = f2_add(t, nmagic);                                   // t - magic == t + (-magic), exactly
+    F2 r = f2_fma(n, f2_pack(-0x1.62e400p-1f, -0x1.62e400p-1f), x);
+    r = f2_fma(n, f2_pack(-0x1.7f7d1cp-20f, -0x1.7f7d1cp-20f), r);
+    F2 p = f2_pack(0x1.6c16c2p-10f, 0x1.6c16c2p-10f);
+    p = f2_fma(p, r, f2_pack(0x1.111112p-7f, 0x1.111112p-7f));
+    p = f2_fma(p, r, f2_pack(0x1.555556p-5f, 0x1.555556p-5f));
+    p = f2_fma(p, r, f2_pack(0x1.555556p-3f, 0x1.555556p-3f));
+    p = f2_fma(p, r, f2_pack(0.5f, 0.5f));
+    p = f2_fma(p, r, f2_pack(1.0f, 1.0f));
+    p = f2_fma(p, r, f2_pack(1.0f, 1.0f));
+    float p0, p1, t0, t1;
+    f2_unpack(p, p0, p1); f2_unpack(t, t0, t1);
+    const float z0 = __int_as_float(__float_as_int(p0) + (__float_as_int(t0) << 23));
+    const float z1 = __int_as_float(__float_as_int(p1) + (__float_as_int(t1) << 23));
+    y0 = x0 < -80.0f ? 0.0f : z0;
+    y1 = x1 < -80.0f ? 0.0f : z1;
+}
+
 __device__ __forceinline__ float im_tanh(float x)
 {
     const float e = im_exp(__fmul_rn(-2.0f, fabsf(x)));

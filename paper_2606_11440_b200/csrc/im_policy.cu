@@ -499,8 +499,9 @@ __device__ __forceinline__ uint32_t sample_reg(const float (&l)[NO], int off, ui
 #pragma unroll
         for (int i = 0; i + s < NMAX; i += 2 * s) mx[i] = fmaxf(mx[i], mx[i + s]);
     const float m = mx[0];
+    static_assert(NMAX % 2 == 0, "pairs");
 #pragma unroll
-    for (int i = 0; i < NMAX; i++) c[i] = im_exp(__fsub_rn(c[i], m));
+    for (int i = 0; i < NMAX; i += 2) im_exp_x2(__fsub_rn(c[i], m), __fsub_rn(c[i + 1], m), c[i], c[i + 1]);
 #pragma unroll
     for (int i = 1; i < NMAX; i++) c[i] = __fadd_rn(c[i - 1], c[i]);          // c_0 = 0 + e_0 = e_0
     const float Z = c[NMAX - 1];
