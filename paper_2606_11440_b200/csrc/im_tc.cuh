@@ -250,7 +250,10 @@ struct TcMlp {
             tmem_ld16(tlane + kColD3 + 16 * j, v);
             tc_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 16; i++) logit[16 * j + i] = __uint_as_float(v[i]) + bias[2 * H + 16 * j + i];
+            for (int i = 0; i < 16; i += 2) {
+                const float2 y = fadd2(v[i], v[i + 1], *reinterpret_cast<const float2 *>(bias + 2 * H + 16 * j + i));
+                logit[16 * j + i] = y.x; logit[16 * j + i + 1] = y.y;
+            }
         }
     }
 };
