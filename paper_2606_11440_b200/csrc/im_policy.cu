@@ -724,6 +724,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         tc::tc_fence_after();
         float l[NO];
         Net::load_logits(img, tlane, l);
+        const float value = EXEC ? Net::load_output(img, tlane, N3) : 0.0f;     // critic / value head (R26: row 3N)
         tc::tc_fence_before();
         if (tile + gridDim.x < total) tc::bar_arrive(3, 256);   // warpgroup 1 may now overwrite D3's columns
         const bool ok = (sl.flags & 1u) != 0;
@@ -733,9 +734,6 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         const RowInfo ri = tc_decode_row<EXEC>(P, cur, t0);
         if (EXEC) {
             const uint32_t n = N3;
-            float value = 0.0f;
-#pragma unroll
-            for (int i = 0; i < NO; i++) if ((uint32_t)i == n) value = l[i];
             if (ri.critic) {
                 P.val[(size_t)trow * P.E + ri.env] = value;
             } else {

@@ -124,6 +124,12 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
         : "r"(taddr)
         : "memory");
 }
+__device__ __forceinline__ uint32_t tmem_ld1(uint32_t taddr)
+{
+    uint32_t v;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(taddr) : "memory");
+    return v;
+}
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16])
 {
     asm volatile(
@@ -239,6 +245,14 @@ struct TcMlp {
         for (int k = 0; k < H / 16; k++)
             umma_ts(tmem_base + kColD3, tmem_base + kColA3 + 8 * k, smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
         umma_commit(bar);
+    }
+    // one output of this thread's row, column `o` chosen at run time (the value head sits at 3N): D3[o] + b3[o]
+    static __device__ __forceinline__ float load_output(const uint8_t *image, uint32_t tlane, uint32_t o)
+    {
+        const float *bias = reinterpret_cast<const float *>(image + kBias);
+        const uint32_t v = tmem_ld1(tlane + kColD3 + o);
+        tc_wait_ld();
+        return __uint_as_float(v) + bias[2 * H + o];
     }
     // logits of this thread's row: D3 + b3
     static __device__ __forceinline__ void load_logits(const uint8_t *image, uint32_t tlane, float (&logit)[NO])
