@@ -673,7 +673,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         if (blockIdx.x < total) {
             build_a1(nxt, sn, rowbuf);
             tc::fence_proxy_async_smem();
-            tc::bar_sync(2, 128);
+            tc::bar_sync(4, 128);
             if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
             nxt = tc_fetch_row(sched, rb, blockIdx.x + gridDim.x, r, n_crit);
             fetch_snap(nxt, sn);
@@ -681,41 +681,40 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     }
     for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
         if (wg == 1) {
-            // ---- warpgroup 1 owns hidden layer 1: half a while the tensor core computes half b, then layer 2's issue.
-            // Its packed output A2 overlaps the columns of the previous tile's D3: wait until warpgroup 0 has the logits.
-            if (it > 0) tc::bar_sync(3, 256);
+            // ---- warpgroup 1: tanh of layer 1, packed in place (half a while the tensor core computes half b)
             tc::mbar_wait(&bars[0], phase);
             tc::tc_fence_after();
-            Net::half_epilogue(tlane, 0, Net::kColA2, bias);
+            Net::half_epilogue(tlane, 0, 0, bias);
             tc::mbar_wait(&bars[1], phase);
             tc::tc_fence_after();
-            Net::half_epilogue(tlane, 128, Net::kColA2 + 64, bias + 128);
+            Net::half_epilogue(tlane, 128, 64, bias + 128);
             tc::tc_fence_before();
             tc::bar_sync(2, 128);
+            // layer 2 overwrites D3 / A3 of the previous tile: wait until warpgroup 0 has its logits in registers
+            if (it > 0) tc::bar_sync(3, 256);
             if (r == 0) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
-            // while the tensor core runs layer 2: the next tile's features (layer 1 of this tile is done with a1)
+            // the next tile: features (layer 1 of this tile is done with a1), layer 1 behind layer 2 in the tensor pipe
+            // (UMMAs of one thread execute in order, so A2 is consumed by then), row loads of the tile after it
             if (tile + gridDim.x < total) {
                 build_a1(nxt, sn, rowbuf + 128 * ((it + 1) & 1u));
                 tc::fence_proxy_async_smem();
-            }
-        }
-        // ---- hidden layer 2: warpgroup w takes columns [128 w, 128 w + 128) as soon as its half is ready
-        // (warpgroup 0 arrives here from the sampling epilogue of the previous tile)
-        tc::mbar_wait(&bars[2 + wg], phase);
-        tc::tc_fence_after();
-        Net::half_epilogue(tlane, 128 * wg, Net::kColA3 + 64 * wg, bias + kTcH + 128 * wg);
-        tc::tc_fence_before();
-        __syncthreads();
-        if (threadIdx.x == 0) Net::issue_l3(img, tmem_base, &bars[4]);
-        if (wg == 1) {
-            // ---- warpgroup 1: layer 1 of the next tile, then the row loads of the tile after it
-            if (tile + gridDim.x < total) {     // a1 was written before the __syncthreads above
+                tc::bar_sync(4, 128);
                 if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
                 nxt = tc_fetch_row(sched, rb, tile + 2 * gridDim.x, r, n_crit);
                 fetch_snap(nxt, sn);
             }
             continue;
         }
+        // ---- warpgroup 0: tanh of layer 2, packed in place (half a while the tensor core computes half b), layer 3
+        tc::mbar_wait(&bars[2], phase);
+        tc::tc_fence_after();
+        Net::half_epilogue(tlane, Net::kColD2, Net::kColD2, bias + kTcH);
+        tc::mbar_wait(&bars[3], phase);
+        tc::tc_fence_after();
+        Net::half_epilogue(tlane, Net::kColD2 + 128, Net::kColD2 + 128, bias + kTcH + 128);
+        tc::tc_fence_before();
+        tc::bar_sync(5, 128);
+        if (threadIdx.x == 0) Net::issue_l3(img, tmem_base, &bars[4]);
         // ---- warpgroup 0: sampling epilogue of row r, logits in registers
         const TcRowSlot sl = rowbuf[128 * (it & 1u) + r];
         uint32_t islot = ~0u;                              // executor rows: the env's issue-list slot, claimed before the wait
@@ -726,7 +725,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         Net::load_logits(img, tlane, l);
         const float value = EXEC ? Net::load_output(img, tlane, N3) : 0.0f;     // critic / value head (R26: row 3N)
         tc::tc_fence_before();
-        if (tile + gridDim.x < total) tc::bar_arrive(3, 256);   // warpgroup 1 may now overwrite D3's columns
+        if (tile + gridDim.x < total) tc::bar_arrive(3, 256);   // warpgroup 1 may now issue the next tile's layer 2
         const bool ok = (sl.flags & 1u) != 0;
         if (EXEC && !ok) continue;
         TcRaw cur;

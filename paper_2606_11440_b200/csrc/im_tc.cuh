@@ -171,12 +171,12 @@ __host__ __device__ constexpr uint32_t canon_off(uint32_t rows, uint32_t r, uint
 // Shared-memory image of one net (built once by k_pack_tc, copied verbatim by every CTA):
 //   [ W1 canon [H][K1] | W2 canon [H][H] | W3 canon [NO][H] | b1[H] b2[H] b3[NO] fp32 ]
 //
-// Two warpgroups (256 threads) work on one 128-row tile; every hidden layer is computed as two N-halves of 128
-// columns with their own mbarrier, so that the tanh epilogue of half a runs while the tensor core still computes
-// half b.  Warpgroup 1 owns layer 1 (gather, both epilogue halves, issue of layer 2) and half b of layer 2;
-// warpgroup 0 owns half a of layer 2 and the sampling epilogue, which thus overlaps the next tile's layer 1.  TMEM map (512 columns, H = 256):
-//   D1 = [0,256)  ->  A2 = [256,384)  ;  D2 = [0,256)  ->  A3 = [384,512)  ;  D3 = [256,256+NO)
-// Nothing is packed in place, and the next tile's layer 1 (D1) touches no column the sampling epilogue (D3) reads.
+// Two warpgroups (256 threads) share a tile as a two-stage pipeline.  Warpgroup 1 owns layer 1: features into shared
+// memory, issue of layer 1, both tanh halves (half a while the tensor core computes half b), issue of layer 2, and -
+// behind layer 2 in the tensor pipe - layer 1 of the NEXT tile.  Warpgroup 0 owns layer 2's tanh, layer 3 and the
+// sampling epilogue.  So the hidden phases of consecutive tiles overlap.  Everything is packed in place:
+//   D1 = [0,256) -> A2 = [0,128) ; D2 = [256,512) -> A3 = [256,320) u [384,448) ; D3 = [448,512)
+// and the only cross-tile hazard is layer 2 of tile i+1 (D2) over D3 / A3 of tile i: its issue waits for the logits.
 template <int K1, int H, int NO>
 struct TcMlp {
     static_assert(K1 % 16 == 0 && H == 256 && NO % 16 == 0 && NO <= 64, "shape");
@@ -184,7 +184,7 @@ struct TcMlp {
     static constexpr uint32_t kImageBytes = kBias + (2 * H + NO) * 4;
     static constexpr uint32_t kA1Bytes = 128 * K1 * 2;
     static constexpr uint32_t kTmemCols = 512;
-    static constexpr uint32_t kColA2 = 256, kColA3 = 384, kColD3 = 256;
+    static constexpr uint32_t kColD2 = 256, kColD3 = 448;
     static constexpr uint32_t kIdescHalf = instr_desc_bf16(128, 128), kIdescOut = instr_desc_bf16(128, NO);
 
     // tanh(D + bias) of the 128 TMEM columns [src, src+128) -> bf16 pairs in [dst, dst+64); bias points at the half's first column.
@@ -223,7 +223,7 @@ struct TcMlp {
             umma_commit(h ? bar_b : bar_a);
         }
     }
-    // Layer 2 (TS): A2 (TMEM) x W2 -> D2, two halves
+    // Layer 2 (TS): A2 (TMEM cols [0,128), 8 columns per K-chunk) x W2 -> D2 = [256,512), two N-halves
     static __device__ __forceinline__ void issue_l2(const uint8_t *image, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
     {
         tc_fence_after();
@@ -232,18 +232,18 @@ struct TcMlp {
         for (int h = 0; h < 2; h++) {
 #pragma unroll
             for (int k = 0; k < H / 16; k++)
-                umma_ts(tmem_base + 128 * h, tmem_base + kColA2 + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
+                umma_ts(tmem_base + kColD2 + 128 * h, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
             umma_commit(h ? bar_b : bar_a);
         }
     }
-    // Layer 3 (TS): A3 (TMEM) x W3 -> D3
+    // Layer 3 (TS): A3 (K-chunks 0-7 at [256,320), 8-15 at [384,448)) x W3 -> D3 = [448,448+NO)
     static __device__ __forceinline__ void issue_l3(const uint8_t *image, uint32_t tmem_base, uint64_t *bar)
     {
         tc_fence_after();
         const uint32_t sb = smem_u32(image + kW3);
 #pragma unroll
         for (int k = 0; k < H / 16; k++)
-            umma_ts(tmem_base + kColD3, tmem_base + kColA3 + 8 * k, smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
+            umma_ts(tmem_base + kColD3, tmem_base + kColD2 + (k < 8 ? 8 * k : 128 + 8 * (k - 8)), smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
         umma_commit(bar);
     }
     // one output of this thread's row, column `o` chosen at run time (the value head sits at 3N): D3[o] + b3[o]
