@@ -17,6 +17,7 @@ struct RowInfo { uint32_t env, a, c; int32_t dl; float b; uint32_t gidx; bool cr
 struct TileSched {
     uint32_t pref[kRegions + 1];
     uint32_t base[kRegions];
+    uint32_t cnt[kRegions];      // append counters at kernel start (the kernel's own list does not grow while it runs)
     uint32_t crit_tiles, total;
 };
 
@@ -25,6 +26,7 @@ __device__ __forceinline__ void sched_init(TileSched &S, const RowBuf &rb, uint3
     if (threadIdx.x < kRegions) {
         const uint32_t b = rb.base[parity * kRegions + threadIdx.x], c = rb.cnt[threadIdx.x];
         S.base[threadIdx.x] = b;
+        S.cnt[threadIdx.x] = c;
         S.pref[threadIdx.x + 1] = (c - b + rows_per_tile - 1) / rows_per_tile;
         if (blockIdx.x == 0) rb.base[(parity ^ 1u) * kRegions + threadIdx.x] = c;   // next tick starts here
     }
@@ -549,7 +551,7 @@ __device__ __forceinline__ TcRaw tc_fetch_row(const TileSched &S, const RowBuf &
     uint32_t lo = 0, hi = kRegions;
     while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
     const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * 128u + r;
-    if (idx >= rb.cnt[lo]) return x;
+    if (idx >= S.cnt[lo]) return x;
     x.gidx = row_gid(rb, lo, idx);
     x.row = ld_early_u4(rb.row + x.gidx);
     x.ok = true;
