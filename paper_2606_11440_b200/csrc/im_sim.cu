@@ -39,7 +39,7 @@ __host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW,
     L.o_pref = o; o += up((QW + 1) * 4);
     L.o_small = o; o += up(kSmallWords * 4);
     L.o_clist = o; o += up(SP * 2);              // every slot may complete in one tick
-    L.o_glist = o; o += 128;                     // non-empty slot groups of the tick (u8 each)
+    L.o_glist = o; o += 256;                     // non-empty slot groups of the tick: group | occupancy byte << 8
     L.total = o;
     return L;
 }
@@ -156,7 +156,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     uint32_t *s_sc = s_small + SM_SC;                 // [0] ccnt, [1] rew, [2] miss, [3] removals, [4..5] cost (u64)
     unsigned long long *s_cost = (unsigned long long *)(s_sc + 4);
     uint16_t *s_clist = (uint16_t *)(sm + L.o_clist); // completed requests: global slot index
-    uint8_t *s_glist = (uint8_t *)(sm + L.o_glist);
+    uint16_t *s_glist = (uint16_t *)(sm + L.o_glist);
 
     uint8_t *rec = env_rec(P, e);
     uint32_t *hot = (uint32_t *)(rec + P.off_hot), *wkey = (uint32_t *)(rec + P.off_wkey);
@@ -310,9 +310,10 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
 #pragma unroll 1
             for (uint32_t g0 = G; g0 < n_grp; g0 += G) {
                 const uint32_t gi = g0 + gl;
-                const bool ne = gi < n_grp && occ8_of(gi) != 0;
+                const uint32_t o8 = gi < n_grp ? occ8_of(gi) : 0u;
+                const bool ne = o8 != 0;
                 const uint32_t m = g.ballot(ne);
-                if (ne) s_glist[n_list + __popc(m & lt_mask)] = (uint8_t)gi;
+                if (ne) s_glist[n_list + __popc(m & lt_mask)] = (uint16_t)(gi | (o8 << 8));
                 n_list += __popc(m);
             }
             g.sync();
@@ -325,7 +326,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
                 const uint4 ha = na, hb = nb;
                 const uint32_t occ8 = nocc;
                 nocc = 0;
-                if (it * G + gl < n_list) { ngi = s_glist[it * G + gl]; nocc = occ8_of(ngi); na = hot4[2 * ngi]; nb = hot4[2 * ngi + 1]; }
+                if (it * G + gl < n_list) { const uint32_t ent = s_glist[it * G + gl]; ngi = ent & 0xFFu; nocc = ent >> 8; na = hot4[2 * ngi]; nb = hot4[2 * ngi + 1]; }
                 if (occ8) {
                     const uint32_t k = s_gmodel[gi], base = s_base[k], thr = s_thr[k];
                     const Ph4 u4 = philox4x32_10_rk(gid, (uint32_t)t, gi, 0u, P.svc_rk);
