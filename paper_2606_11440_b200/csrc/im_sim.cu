@@ -134,8 +134,8 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     const uint32_t e = blockIdx.x * GPB + threadIdx.x / G;
     if (e >= P.E) return;
     // The kernel is ~58 KB of code against a 32 KB instruction cache, and every group walks through all of it once per
-    // tick.  Before the phases whose control flow does not depend on the env (the service pass, record, arrivals,
-    // write-back) the groups of a CTA wait for each other, so that the CTA's warps fetch the same lines at the same time
+    // tick.  Before the phases whose control flow does not depend on the env (the service pass, record, arrivals)
+    // the groups of a CTA wait for each other, so that the CTA's warps fetch the same lines at the same time
     // (measured on configs[4]: 0.81 -> 0.71 ms per tick with 256-thread CTAs; more barriers or 512 threads lose again).
     const uint32_t cmask = (G == 32 || (e ^ 1u) >= P.E) ? g.gmask : 0xffffffffu;
     const bool cta_full = (blockIdx.x + 1) * GPB <= P.E;
@@ -647,7 +647,6 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
         sn[2 * N + gl] = __fmul_rn(__uint2float_rn(M_KV(gl)), s_model[gl].kv_inv);
     }
     // ---- counters, then write the header back
-    IM_CONVERGE();
     if (gl < 16 && s_ctr[gl]) {
         unsigned long long *c64 = (unsigned long long *)(s_hdr + P.hw_ctr);
         c64[gl] += s_ctr[gl];
