@@ -134,9 +134,10 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     const uint32_t e = blockIdx.x * GPB + threadIdx.x / G;
     if (e >= P.E) return;
     // The kernel is ~58 KB of code against a 32 KB instruction cache, and every group walks through all of it once per
-    // tick.  Before the phases whose control flow does not depend on the env (the service pass, record, arrivals)
-    // the groups of a CTA wait for each other, so that the CTA's warps fetch the same lines at the same time
-    // (measured on configs[4]: 0.81 -> 0.71 ms per tick with 256-thread CTAs; more barriers or 512 threads lose again).
+    // tick.  Before the service pass and before the record / arrival phases (control flow there does not depend on the
+    // env) the groups of a CTA wait for each other, so that the CTA's warps fetch the same lines at the same time
+    // (measured on configs[4]: 0.81 -> 0.71 ms per tick with 256-thread CTAs; more barriers, barriers before the
+    // arrival phase or the write-back, and 512 threads all lose again).
     const uint32_t cmask = (G == 32 || (e ^ 1u) >= P.E) ? g.gmask : 0xffffffffu;
     const bool cta_full = (blockIdx.x + 1) * GPB <= P.E;
 #define IM_CONVERGE() do { if (cta_full) __syncthreads(); else __syncwarp(cmask); } while (0)
@@ -583,7 +584,6 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
             g.sync();
         }
         // ---- A arrive (R5, R7, R8, R9)
-        IM_CONVERGE();
         {
             const uint32_t xr = draw(P, STREAM_ARR, gid, t, 0, 0).x;
             const uint32_t *cdf = P.tab_cdf + 32u * P.env_level[e];
