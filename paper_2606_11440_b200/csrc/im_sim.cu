@@ -1,4 +1,4 @@
-// im_sim.cu — the fixed-tick simulation kernel: one group of G lanes (a half-warp) per environment, 16 envs per CTA.
+// im_sim.cu — the fixed-tick simulation kernel: one group of G lanes (a half-warp) per environment, 24 envs per CTA.
 //
 // One launch runs, for every env, the environment half of the canonical tick:
 //   post(t):  D-issue (the calls the executor kernel decided for tick t join the waiting list), E admit
@@ -21,7 +21,8 @@
 
 namespace im {
 
-constexpr int kSimThreads = 256;
+constexpr int kSimThreads = 384;   // 3 CTAs per SM; measured on configs[4], ms per tick: (192,6) 0.714, (256,4) 0.686,
+                                   // (320,4) 0.756, (384,3) 0.650, (448,2) 0.751
 
 // ---- per-group shared memory layout (bytes)
 struct SimLayout {
@@ -105,7 +106,7 @@ __device__ __forceinline__ uint32_t u16_field(const Ph4 &u, uint32_t f)
 
 // tick arguments: t_post < 0 => no post phases; pre_mode 0 none, 1 full (A, B, rows), 2 snapshot only
 template <int G>
-__global__ void __launch_bounds__(kSimThreads, 4)
+__global__ void __launch_bounds__(kSimThreads, 3)
 k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -137,7 +138,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     // tick.  Before the service pass and before the record / arrival phases (control flow there does not depend on the
     // env) the groups of a CTA wait for each other, so that the CTA's warps fetch the same lines at the same time
     // (measured on configs[4]: 0.81 -> 0.71 ms per tick with 256-thread CTAs; more barriers, barriers before the
-    // arrival phase or the write-back, and 512 threads all lose again).
+    // arrival phase or the write-back, and 512 threads all lose again; 384 threads x 3 CTAs is the best shape).
     const uint32_t cmask = (G == 32 || (e ^ 1u) >= P.E) ? g.gmask : 0xffffffffu;
     const bool cta_full = (blockIdx.x + 1) * GPB <= P.E;
 #define IM_CONVERGE() do { if (cta_full) __syncthreads(); else __syncwarp(cmask); } while (0)
