@@ -314,6 +314,8 @@ def main():
     roof["sim_hbm_frac"] = hbm_frac_sim
     roof["step_hbm_frac"] = (model["sim_bytes"] + model["exec_bytes"] + model["plan_bytes"] + model["ret_bytes"]) / (ms_per_step * 1e-3) / 1e9 / peaks["hbm"]
     roof["step_tensor_frac"] = (model["exec_flops"] + model["plan_flops"]) / (ms_per_step * 1e-3) / 1e12 / peaks["bf16_sustained"] if bf16 else None
+    # t_lb / t, t_lb = the larger of the two bound times of the whole step
+    roof["step_lb_frac"] = max(roof["step_hbm_frac"], roof["step_tensor_frac"] or 0.0)
     roof["returns_hbm_frac"] = model["ret_bytes"] / max(per_launch_ms["returns"] * 1e-3, 1e-12) / 1e9 / peaks["hbm"]
 
     # ---- end to end through the C ABI with HOST buffers: host blob in, ADV / RET / scalars out to pinned host memory
