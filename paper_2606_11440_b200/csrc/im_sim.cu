@@ -139,13 +139,14 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     const uint32_t e = bid * GPB + threadIdx.x / G;
     if (e >= P.E) return;
     // The kernel is ~58 KB of code against a 32 KB instruction cache, and every group walks through all of it once per
-    // tick.  Before the service pass and before the record / arrival phases (control flow there does not depend on the
-    // env) the groups of a CTA wait for each other, so that the CTA's warps fetch the same lines at the same time
-    // (measured on configs[4]: 0.81 -> 0.71 ms per tick with 256-thread CTAs; more barriers, barriers before the
-    // arrival phase or the write-back, and 512 threads all lose again; 384 threads x 3 CTAs is the best shape).
+    // tick.  Before the record / arrival phases (control flow there does not depend on the env) the groups of a CTA
+    // wait for each other, so that the CTA's warps fetch the same lines at the same time (measured on configs[4] with
+    // 384-thread CTAs, ms per tick: no barrier 0.721, before the service pass only 0.728, before the record only
+    // 0.639, both 0.643; a second barrier before admission, completion or preemption: 0.649 / 0.654 / 0.647).
     const uint32_t cmask = (G == 32 || (e ^ 1u) >= P.E) ? g.gmask : 0xffffffffu;
     const bool cta_full = (bid + 1) * GPB <= P.E;
 #define IM_CONVERGE() do { if (cta_full) __syncthreads(); else __syncwarp(cmask); } while (0)
+#define IM_WCONV() __syncwarp(cmask)
     const uint32_t gid = P.env_id_base + e;
     const uint32_t N = P.N, QW = P.QW, QCAP = P.QCAP;
     const uint32_t region = e % kRegions;
@@ -302,7 +303,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
         const uint32_t madm = g.ballot(gl < N && M_NWAIT(gl) > 0 && M_NRUN(gl) < s_model[gl].slots && M_KV(gl) <= s_model[gl].kv_cap);
 
         // =============================================================== F serve (R11): one streaming pass over the slots
-        IM_CONVERGE();
+        g.sync();
         {
             uint4 *hot4 = (uint4 *)hot;
             const uint32_t n_grp = P.SP >> 3;
@@ -664,6 +665,7 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
         for (uint32_t i = gl; i < P.hdr_words / 4; i += G) dst[i] = src[i];
     }
 #undef IM_CONVERGE
+#undef IM_WCONV
 #undef M_NWAIT
 #undef M_NRUN
 #undef M_KV
