@@ -22,7 +22,7 @@
 namespace im {
 
 constexpr int kSimThreads = 384;   // 3 CTAs per SM; measured on configs[4], ms per tick: (192,6) 0.714, (256,4) 0.686,
-                                   // (320,4) 0.756, (384,3) 0.650, (448,2) 0.751
+                                   // (320,4) 0.756, (352,3) 0.669, (384,3) 0.650, (416,3) 0.690, (448,2) 0.751
 
 // ---- per-group shared memory layout (bytes)
 struct SimLayout {
@@ -31,7 +31,7 @@ struct SimLayout {
 // small per-env arrays (u32 words): 16 per model-indexed array
 enum : uint32_t { SM_LATSUM = 0, SM_LATN = 16, SM_RELKV = 32, SM_RELNRUN = 48, SM_KVADD = 64, SM_OCCCLR = 80, SM_AMIN = 112,
                   SM_AIDX = 128, SM_ALAST = 144, SM_CTR = 160, SM_SC = 176, SM_RM = 184, SM_MV = 200, kSmallWords = 216 };
-__host__ __device__ inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW, uint32_t SP)
+inline SimLayout sim_layout(uint32_t hdr_words, uint32_t QW, uint32_t SP)
 {
     auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
     SimLayout L;
@@ -107,7 +107,7 @@ __device__ __forceinline__ uint32_t u16_field(const Ph4 &u, uint32_t f)
 // tick arguments: t_post < 0 => no post phases; pre_mode 0 none, 1 full (A, B, rows), 2 snapshot only
 template <int G>
 __global__ void __launch_bounds__(kSimThreads, 3)
-k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0)
+k_sim(const Params P, const SimLayout L, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ ModelTab s_model[kMaxModels];
@@ -151,7 +151,6 @@ k_sim(const Params P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_
     const uint32_t N = P.N, QW = P.QW, QCAP = P.QCAP;
     const uint32_t region = e % kRegions;
 
-    const SimLayout L = sim_layout(P.hdr_words, QW, P.SP);
     unsigned char *sm = smem_raw + (size_t)(threadIdx.x / G) * L.total;
     uint32_t *s_hdr = (uint32_t *)(sm + L.o_hdr);
     uint32_t *s_occ = s_hdr + P.hw_occ, *s_qfree = s_hdr + P.hw_qfree, *s_qready = s_hdr + P.hw_qready, *s_misc = s_hdr + P.hw_misc;
@@ -687,8 +686,8 @@ void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_p
     const uint32_t gpb = kSimThreads / G;
     const size_t smem = (size_t)gpb * L.total;
     const uint32_t blocks = (P.E + gpb - 1) / gpb;
-    if (G == 16) k_sim<16><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
-    else k_sim<32><<<blocks, kSimThreads, smem, st>>>(P, t_post, trow_post, t_pre, pre_mode, t0);
+    if (G == 16) k_sim<16><<<blocks, kSimThreads, smem, st>>>(P, L, t_post, trow_post, t_pre, pre_mode, t0);
+    else k_sim<32><<<blocks, kSimThreads, smem, st>>>(P, L, t_post, trow_post, t_pre, pre_mode, t0);
 }
 
 }  // namespace im
