@@ -3,6 +3,8 @@
 episodes, prefill and input tokens, budgets, depth medians, the three policy kernels, ragged env counts, chunking).
 The named cases of test_gpu_parity.py / test_gpu_edges.py pin what each of them is about; this sweep is there for the
 combinations nobody thought of.  Seeds are fixed: a failure reproduces."""
+import os
+
 import numpy as np
 import pytest
 
@@ -43,7 +45,7 @@ def _random_spec(case: int):
     return spec, chunks, int(rng.integers(0, 1000))
 
 
-@pytest.mark.parametrize("case", range(48))
+@pytest.mark.parametrize("case", range(int(os.environ.get("IM_RANDOM_CASES", "48"))))   # more cases: a bug hunt, not the suite
 def test_random_spec_parity(case):
     spec, chunks, seed = _random_spec(case)
     st = _run(spec, seed=seed, chunks=chunks)
