@@ -590,7 +590,11 @@ k_sim(const Params P, const SimLayout L, int32_t t_post, uint32_t trow_post, int
         }
         // ---- A arrive (R5, R7, R8, R9)
         {
-            const uint32_t xr = draw(P, STREAM_ARR, gid, t, 0, 0).x;
+            // one Philox pass for the whole group: the last lane draws the arrival count, lane j < G - 1 draws, ahead of
+            // need, the budget / input tokens of arrival j (same streams and counters as two separate passes, R2)
+            const bool cnt_lane = gl == G - 1;
+            const Ph4 dsp = draw(P, cnt_lane ? STREAM_ARR : STREAM_QRY, gid, t, cnt_lane ? 0u : gl, 0);
+            const uint32_t xr = g.shfl(dsp.x, G - 1);
             const uint32_t *cdf = P.tab_cdf + 32u * P.env_level[e];
             uint32_t n = 0;
 #pragma unroll 1
@@ -605,7 +609,7 @@ k_sim(const Params P, const SimLayout L, int32_t t_post, uint32_t trow_post, int
 #pragma unroll 1
                 for (uint32_t j = gl; j < n_ok; j += G) {
                     const uint32_t q = find_nth(s_qfree, QW, prefB, j);
-                    const Ph4 d = draw(P, STREAM_QRY, gid, t, j, 0);
+                    const Ph4 d = j < G - 1 ? dsp : draw(P, STREAM_QRY, gid, t, j, 0);
                     const uint32_t comp = d.z < P.mix_thresh ? 0u : 1u;
                     const uint32_t budget = P.mix_lo[comp] + __umulhi(d.x, P.mix_hi[comp] - P.mix_lo[comp] + 1u);
                     const uint32_t in_tok = P.has_intok ? __ldg(&P.tab_intok[d.y >> 22]) : P.in_tok_const;

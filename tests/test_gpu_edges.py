@@ -62,3 +62,27 @@ def test_clock_limit_is_an_error_not_a_wraparound():
     g.reset()
     g.rollout(blob, 100)                # the clock restarts with im_reset
     g.close()
+
+
+def test_arrival_bursts_of_sixteen_and_more():
+    """Poisson(14) arrivals per tick with short calls and a large table: bursts of 16..31 queries in one tick are common,
+    i.e. more arrivals than a group has lanes (the second iteration of the arrival loop and its separately drawn
+    budgets, R7/R8)."""
+    from paper_2606_11440_b200 import InfraMind
+    spec = tiny_spec(n_envs=11, N=2, n_ticks=50, qcap=256, rcap=1024, rate_tick=14.0, slots=64, rates=[200, 200], budget=(5, 30),
+                     medians=(4, 8, 12), f_in=32, hidden=32, seed=4)
+    cap = (64 + spec.n_envs) * spec.n_ticks * 80
+    spec = spec.with_(log_cap_exec=cap, log_cap_plan=cap, log_cap_query=cap)
+    st = _run(spec, seed=9, chunks=[1] * 10 + [40])
+    assert st["arrivals"] > 11 * 50 * 12
+    # some tick of some env took sixteen or more queries at once: the planner log holds one row per accepted arrival
+    g = InfraMind(spec, seed=9, debug_flags=1)
+    before = g.counters()[:, 10].astype(np.int64)
+    burst = 0
+    for _ in range(50):
+        g.rollout(make_policy_blob(spec), 1)
+        now = g.counters()[:, 10].astype(np.int64)
+        burst = max(burst, int((now - before).max()))
+        before = now
+    g.close()
+    assert burst >= 16
