@@ -27,7 +27,7 @@ def _run(spec, seed, chunks, blob=None, env_ids=None, gamma=0.99, lam=0.95, mu=0
     finish_stats(orc, stats, bf16)
     compare_returns(gpu, orc, env_ids, gamma, lam, mu, bf16, whole_batch=(len(env_ids) == spec.n_envs))
     csum = gpu.counters().sum(axis=0)
-    stats.update(arrivals=int(csum[0]), dropped=int(csum[1]), finished=int(csum[2]), preemptions=int(csum[7]))
+    stats.update(arrivals=int(csum[0]), dropped=int(csum[1]), finished=int(csum[2]), preemptions=int(csum[7]), missed=int(csum[4]))
     gpu.close()
     return stats
 
@@ -73,6 +73,23 @@ def test_fcfs_and_episodes_and_miss_cost():
     spec = tiny_spec(n_envs=37, N=3, n_ticks=240, qcap=32, rcap=128, rate_tick=0.35, slots=2, sched_mode=0,
                      episode_ticks=60, cost_mode=1, f_in=32, hidden=64, budget=(20, 120))
     _run(spec, seed=5, chunks=[60, 1, 59, 120])
+
+
+def test_t9_bimodal_budgets_edf_vs_fcfs_single_server():
+    """PAPER.md:179 (Table 3, "w/o EDF"), qualitative: one stable single-slot server, budgets 100 / 1000 ticks.
+    Both orders are bit-exact against the oracle, and the CUDA path's own counters show fewer misses under EDF."""
+    from helpers import forced_single_blob
+    kw = dict(n_envs=35, N=1, n_ticks=1500, qcap=64, rcap=256, rate_tick=0.025, slots=1, budget=(100, 100), seed=3,
+              rates=[40], f_in=32, hidden=64)
+    missed = []
+    for mode in (0, 1):
+        spec = tiny_spec(sched_mode=mode, **kw).with_(
+            mix_thresh=0x80000000, mix_lo=np.array([100, 1000], dtype=np.uint32),
+            mix_hi=np.array([100, 1000], dtype=np.uint32), budget_norm_ticks=1000)
+        st = _run(spec, seed=5, chunks=[700, 800], blob=forced_single_blob(spec))
+        assert st["dropped"] == 0
+        missed.append(st["missed"])
+    assert missed[1] < 0.75 * missed[0]
 
 
 def test_tiny_queue_preemption_fp32():

@@ -308,6 +308,28 @@ def test_p9_equal_budgets_edf_equals_fcfs(orc):
     assert a.counters()[:, CN["sum_waiting"]].sum() > 0
 
 
+def test_t9_bimodal_budgets_edf_misses_fewer_deadlines_than_fcfs(orc):
+    """PAPER.md:179, 191 (Table 3, "w/o EDF"): with mixed budgets, deadline order protects the tight queries.
+    Qualitative echo on one stable single-slot server (load ~0.75) with budgets 100 / 1000 ticks, half each:
+    same arrivals and job sizes under both orders (the draws do not depend on sched_mode), EDF misses far fewer
+    deadlines and does not finish fewer queries. Not a numeric target of the paper."""
+    kw = dict(n_envs=32, N=1, n_ticks=3000, qcap=64, rcap=192, rate_tick=0.025, slots=1, budget=(100, 100), seed=3,
+              rates=[40])
+    res = []
+    for mode in (0, 1):                             # 0 = FCFS, 1 = EDF
+        s = tiny_spec(sched_mode=mode, **kw).with_(
+            mix_thresh=0x80000000, mix_lo=np.array([100, 1000], dtype=np.uint32),
+            mix_hi=np.array([100, 1000], dtype=np.uint32), budget_norm_ticks=1000)
+        o = orc.Oracle(s, seed=5)
+        o.rollout(forced_single_blob(s), 3000)
+        res.append(o.counters().astype(np.int64))
+    fcfs, edf = res
+    assert np.array_equal(fcfs[:, CN["arrivals"]], edf[:, CN["arrivals"]]) and fcfs[:, CN["dropped"]].sum() == 0
+    assert fcfs[:, CN["sum_waiting"]].sum() > 0     # there is a queue to reorder
+    assert abs(int(edf[:, CN["finished"]].sum()) - int(fcfs[:, CN["finished"]].sum())) <= 0.01 * fcfs[:, CN["finished"]].sum()
+    assert edf[:, CN["missed"]].sum() < 0.6 * fcfs[:, CN["missed"]].sum()
+
+
 def test_p10_action_decode(orc):
     """model = a div 3, strategy = a mod 3, a in [0, 3N)."""
     spec = make_pool_spec(1, n_envs=4, n_ticks=1)
