@@ -15,6 +15,8 @@
 
 namespace im {
 void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st);
+int sim_prepare_device();
+int policy_prepare_device(const Params &P);
 int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm, bool bf16, cudaStream_t st);
 int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st);
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st);
@@ -23,15 +25,31 @@ bool tc_supported(uint32_t F, uint32_t H);
 size_t tc_image_bytes(bool exec);
 void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t st);
 
-// empty pools: zero the header of every env record (no slot taken, empty waiting list), query bitmap all free
+// empty pools: per 32-env block, zero the SoA-32 parts (header, counters, slot groups: a free slot holds 0, issue list,
+// ready bitmap), query bitmap all free for the envs that exist (the padding lanes of the last block have no free slot
+// and therefore never admit a query)
 __global__ void k_reset(const Params P)
 {
-    const size_t n = (size_t)P.E * P.hdr_words;
+    const uint32_t words = P.off_wkey / 4;                       // hdr | ctr | hot
+    const size_t n = (size_t)P.NB * words;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const uint32_t e = (uint32_t)(i / P.hdr_words), w = (uint32_t)(i % P.hdr_words);
+        const uint32_t b = (uint32_t)(i / words), w = (uint32_t)(i % words);
         uint32_t v = 0;
-        if (w >= P.hw_qfree && w < P.hw_qfree + P.QW) v = 0xFFFFFFFFu;
-        reinterpret_cast<uint32_t *>(env_rec(P, e))[w] = v;
+        if (w >= P.hw_qfree * 32u && w < (P.hw_qfree + P.QW) * 32u && b * 32u + (w & 31u) < P.E) v = 0xFFFFFFFFu;
+        reinterpret_cast<uint32_t *>(P.env_base + (size_t)b * P.blk_stride)[w] = v;
+    }
+    const uint32_t qw = P.QW * 32u;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)P.NB * qw; i += (size_t)gridDim.x * blockDim.x)
+        reinterpret_cast<uint32_t *>(P.env_base + (size_t)(i / qw) * P.blk_stride + P.off_qready)[i % qw] = 0;
+}
+
+// de-interleave `nw` header / counter words starting at unit `w0` of part `off` into dst[e][nw] (telemetry read-back)
+__global__ void k_gather_words(const Params P, uint32_t off, uint32_t w0, uint32_t nw, uint32_t *__restrict__ dst)
+{
+    const size_t n = (size_t)P.E * nw;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const uint32_t e = (uint32_t)(i / nw), w = (uint32_t)(i % nw);
+        dst[i] = reinterpret_cast<const uint32_t *>(P.env_base + (size_t)(e >> 5) * P.blk_stride + off)[(w0 + w) * 32u + (e & 31u)];
     }
 }
 
@@ -210,14 +228,27 @@ struct Carver {
     }
 };
 
+// Row capacities of the three lists (whole job).  With IM_FLAG_LOG_DECISIONS the executor / planner lists are linear
+// logs of one im_rollout and log_cap_* sizes them (0 = a default from max_ticks).  Without it they are rings that only
+// hold one tick's work rows: log_cap_exec / log_cap_plan are ignored and the ring gets a fixed per-tick bound (a tick that
+// produces more rows than that is flagged, IM_ERR_CAPACITY at the next read).
 static void default_caps(const im_pool_spec &s, uint32_t E, uint64_t &ce, uint64_t &cp, uint64_t &cq)
 {
     const bool log = s.debug_flags & IM_FLAG_LOG_DECISIONS;
-    const uint64_t per_tick_e = (uint64_t)E * 16 + 4096, per_tick_p = (uint64_t)E * 8 + 4096;
-    ce = s.log_cap_exec ? s.log_cap_exec : (log ? per_tick_e * s.max_ticks / 4 : per_tick_e);
-    cp = s.log_cap_plan ? s.log_cap_plan : (log ? per_tick_p * s.max_ticks / 4 : per_tick_p);
-    cq = s.log_cap_query ? s.log_cap_query : per_tick_p * s.max_ticks / 4;
-    if (!log) { ce = ce < per_tick_e ? ce : per_tick_e; cp = cp < per_tick_p ? cp : per_tick_p; }
+    const uint64_t per_tick_e = (uint64_t)E * 32 + 4096, per_tick_p = (uint64_t)E * 16 + 4096;
+    ce = !log ? per_tick_e : (s.log_cap_exec ? s.log_cap_exec : per_tick_e * s.max_ticks / 8);
+    cp = !log ? per_tick_p : (s.log_cap_plan ? s.log_cap_plan : per_tick_p * s.max_ticks / 8);
+    cq = s.log_cap_query ? s.log_cap_query : per_tick_p * s.max_ticks / 8;
+}
+
+// rows of ONE region: the whole-job capacity scaled by the largest share of envs a region can hold (regions are whole
+// 32-env blocks, so small jobs are uneven)
+static uint32_t region_cap(uint64_t cap, uint32_t E, uint32_t NB, uint32_t n_regions)
+{
+    const uint64_t blocks = (NB + n_regions - 1) / n_regions;
+    uint64_t envs = blocks * 32;
+    if (envs > E) envs = E;
+    return (uint32_t)((cap * envs + E - 1) / E) + 64u;
 }
 
 static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
@@ -227,23 +258,28 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     memset(&P, 0, sizeof P);
     const uint32_t N = s.n_models, Q = s.qcap, R = s.rcap;
     const size_t T1 = (size_t)s.max_ticks + 1;
-    auto up4 = [](uint32_t w) { return (w + 3u) & ~3u; };
-    // ---- per-env record (im_device.cuh): header words, then the arrays
+    // ---- one record per block of 32 envs (im_device.cuh): SoA-32 parts, then the per-env arrays
     P.QW = Q / 32;
+    P.NB = (E + 31u) / 32u;
+    P.n_regions = P.NB < kRegions ? P.NB : kRegions;
     P.slot_base[0] = 0;
     for (uint32_t k = 0; k < kMaxModels; k++) P.slot_base[k + 1] = P.slot_base[k] + (k < N ? ((s.model[k].slots + 7u) & ~7u) : 0u);
     P.SP = P.slot_base[N];
-    P.hw_occ = 4 * N; P.hw_qfree = P.hw_occ + up4(2 * N); P.hw_qready = P.hw_qfree + up4(P.QW);
-    P.hw_misc = P.hw_qready + up4(P.QW); P.hw_ctr = P.hw_misc + 4; P.hdr_words = P.hw_ctr + 32;
-    uint32_t off = (P.hdr_words * 4 + 127u) & ~127u;
-    P.off_iss = off; off += kIssueCap * 8;
-    P.off_hot = off; off += ((P.SP * 4 + 127u) & ~127u);
-    P.off_cold = off; off += ((P.SP * 8 + 127u) & ~127u);
-    P.off_wkey = off; off += R * 4;
-    P.off_waux = off; off += R * 8;
-    P.off_q = off; off += Q * 16;
-    P.env_stride = (off + 127u) & ~127u;
-    P.env_base = cv.take<uint8_t>((size_t)E * P.env_stride);
+    P.n_grp = P.SP / 8; P.cm_words = (P.n_grp + 3u) / 4u;
+    P.hw_occ = 3 * N; P.hw_qfree = P.hw_occ + 2 * N; P.hw_misc = P.hw_qfree + P.QW; P.hdr_words = P.hw_misc + 2;
+    auto up128 = [](uint32_t x) { return (x + 127u) & ~127u; };
+    uint32_t off = P.hdr_words * 128u;
+    P.off_ctr = off; off += (uint32_t)C_N * 128u;
+    P.off_hot = off; off += P.n_grp * 512u;
+    P.off_wkey = off; off += R * 128u;                        // (R / 4) units of 16 B x 32 lanes
+    P.off_iss = off; off += kIssueCap * 256u;
+    P.off_qready = off; off += P.QW * 128u;
+    P.cold_stride = up128(P.SP * 16u); P.waux_stride = R * 8u; P.q_stride = Q * 16u;
+    P.off_cold = off; off += 32u * P.cold_stride;
+    P.off_waux = off; off += 32u * P.waux_stride;
+    P.off_q = off; off += 32u * P.q_stride;
+    P.blk_stride = up128(off);
+    P.env_base = cv.take<uint8_t>((size_t)P.NB * P.blk_stride);
     // ---- control block (zeroed by im_reset)
     cv.off = (cv.off + 255) & ~(size_t)255;
     const size_t ctl_off = cv.off;
@@ -264,9 +300,9 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     // ---- row lists / logs
     uint64_t ce, cp, cq;
     default_caps(s, E, ce, cp, cq);
-    const uint32_t rce = (uint32_t)((ce + kRegions - 1) / kRegions), rcp = (uint32_t)((cp + kRegions - 1) / kRegions), rcq = (uint32_t)((cq + kRegions - 1) / kRegions);
+    const uint32_t rce = region_cap(ce, E, P.NB, P.n_regions), rcp = region_cap(cp, E, P.NB, P.n_regions), rcq = region_cap(cq, E, P.NB, P.n_regions);
     P.exec.regcap = rce; P.plan.regcap = rcp; P.qlog.regcap = rcq;
-    const size_t ne = (size_t)rce * kRegions, np = (size_t)rcp * kRegions, nq = (size_t)rcq * kRegions;
+    const size_t ne = (size_t)rce * P.n_regions, np = (size_t)rcp * P.n_regions, nq = (size_t)rcq * P.n_regions;
     const bool log = s.debug_flags & IM_FLAG_LOG_DECISIONS;
     P.exec.row = cv.take<uint4>(ne); P.plan.row = cv.take<uint4>(np);
     if (log) { P.exec.logp = cv.take<float>(ne); P.exec.val = cv.take<float>(ne); P.plan.logp = cv.take<float>(np); }
@@ -332,18 +368,6 @@ static int copy_out(im_ctx *c, const void *src, size_t bytes, void *dst, size_t 
     return IM_OK;
 }
 
-// E rows of `width` bytes, `pitch` apart on the device, packed densely into dst
-static int copy_out_2d(im_ctx *c, const void *src, size_t pitch, size_t width, size_t rows, void *dst, size_t cap, size_t *written)
-{
-    const size_t bytes = width * rows;
-    if (written) *written = bytes;
-    if (!dst) return IM_OK;
-    if (cap < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", cap, bytes);
-    CUDA_TRY(c, cudaMemcpy2DAsync(dst, width, src, pitch, width, rows, cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    return IM_OK;
-}
-
 template <typename T>
 static int fetch(im_ctx *c, std::vector<T> &h, const T *d, size_t n)
 {
@@ -404,6 +428,8 @@ int im_bind(im_ctx *c, void *dev_arena, size_t bytes, void *cuda_stream)
     if (bytes < need) return fail(c, IM_ERR_NOMEM, "arena too small: %zu < %zu", bytes, need);
     c->arena = (uint8_t *)dev_arena; c->arena_bytes = bytes; c->stream = (cudaStream_t)cuda_stream;
     carve(c, c->spec, c->E, c->arena);
+    // shared-memory opt-ins are per device: set them for the device this ctx is bound on
+    if (sim_prepare_device() || policy_prepare_device(c->P)) return fail(c, IM_ERR_CUDA, "cudaFuncSetAttribute failed on device %d", dev);
     CUDA_TRY(c, cudaMemcpyAsync((void *)c->P.tab_mult, c->tab_mult.data(), 4096, cudaMemcpyHostToDevice, c->stream));
     if (!c->tab_intok.empty()) CUDA_TRY(c, cudaMemcpyAsync((void *)c->P.tab_intok, c->tab_intok.data(), 4096, cudaMemcpyHostToDevice, c->stream));
     else CUDA_TRY(c, cudaMemsetAsync((void *)c->P.tab_intok, 0, 4096, c->stream));
@@ -532,8 +558,35 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
     case IM_TEL_RET:
         if (!c->have_returns) return fail(c, IM_ERR_STATE, "ADV/RET read before im_returns");
         return copy_out(c, what == IM_TEL_ADV ? c->adv : c->ret, 4 * T * E, dst, dst_bytes, written);
-    case IM_TEL_COUNTERS: return copy_out_2d(c, P.env_base + 4 * (size_t)P.hw_ctr, P.env_stride, 128, E, dst, dst_bytes, written);
-    case IM_TEL_SNAPSHOT: return copy_out_2d(c, P.env_base, P.env_stride, 16 * N, E, dst, dst_bytes, written);
+    case IM_TEL_COUNTERS:
+    case IM_TEL_SNAPSHOT: {
+        // the device keeps these struct-of-arrays across the 32 envs of a block: gather them per env, then widen / unpack
+        const bool ctr = what == IM_TEL_COUNTERS;
+        const size_t nw = ctr ? (size_t)C_N : 3 * N, bytes = ctr ? 128 * E : 16 * N * E;
+        if (written) *written = bytes;
+        if (!dst) return IM_OK;
+        if (dst_bytes < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, bytes);
+        k_gather_words<<<c->n_sm * 4, 256, 0, c->stream>>>(P, ctr ? P.off_ctr : 0u, 0u, (uint32_t)nw, c->qorder);
+        c->launches++;
+        CUDA_TRY(c, cudaGetLastError());
+        std::vector<uint32_t> h;
+        int rc = fetch(c, h, c->qorder, E * nw);
+        if (rc) return rc;
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (ctr) {
+            uint64_t *o = (uint64_t *)dst;
+            for (size_t i = 0; i < E * nw; i++) o[i] = h[i];
+        } else {
+            uint32_t *o = (uint32_t *)dst;
+            for (size_t e = 0; e < E; e++)
+                for (size_t k = 0; k < N; k++) {
+                    const uint32_t *m = &h[e * nw + 3 * k];
+                    uint32_t *r = o + (e * N + k) * 4;
+                    r[0] = m[0] & 0xFFFFu; r[1] = m[0] >> 16; r[2] = m[1]; r[3] = m[2];
+                }
+        }
+        return IM_OK;
+    }
     case IM_TEL_TABLES: {
         const size_t bytes = 4096 + 4096 + c->tab_cdf.size() * 4;
         if (written) *written = bytes;
@@ -636,21 +689,24 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         if (!dst) return IM_OK;
         if (dst_bytes < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", dst_bytes, bytes);
         std::vector<uint8_t> buf;
-        const size_t batch = 256;
+        const size_t batch = 8;                                   // blocks of 32 envs per copy
         uint32_t *w = (uint32_t *)dst;
-        for (size_t e0 = 0; e0 < E; e0 += batch) {
-            const size_t ne = E - e0 < batch ? E - e0 : batch;
-            buf.resize(ne * P.env_stride);
-            CUDA_TRY(c, cudaMemcpy(buf.data(), P.env_base + e0 * P.env_stride, ne * P.env_stride, cudaMemcpyDeviceToHost));
-            for (size_t e = 0; e < ne; e++) {
-                const uint8_t *rec = buf.data() + e * P.env_stride;
-                const uint32_t *hdr = (const uint32_t *)rec, *occ = hdr + P.hw_occ, *qfree = hdr + P.hw_qfree;
-                const uint32_t *hot = (const uint32_t *)(rec + P.off_hot), *wkey = (const uint32_t *)(rec + P.off_wkey);
-                const uint2 *cold = (const uint2 *)(rec + P.off_cold), *waux = (const uint2 *)(rec + P.off_waux);
-                const uint4 *qt = (const uint4 *)(rec + P.off_q);
-                memcpy(w, hdr, 16 * N); w += 4 * N;
+        for (size_t b0 = 0; b0 < P.NB; b0 += batch) {
+            const size_t nb = P.NB - b0 < batch ? P.NB - b0 : batch;
+            buf.resize(nb * P.blk_stride);
+            CUDA_TRY(c, cudaMemcpy(buf.data(), P.env_base + b0 * P.blk_stride, nb * P.blk_stride, cudaMemcpyDeviceToHost));
+            for (size_t e = b0 * 32; e < (b0 + nb) * 32 && e < E; e++) {
+                const uint8_t *blk = buf.data() + (e / 32 - b0) * P.blk_stride;
+                const size_t l = e & 31;
+                const uint32_t *hdr = (const uint32_t *)blk;
+                auto H = [&](uint32_t wd) { return hdr[wd * 32 + l]; };
+                const uint16_t *hot = (const uint16_t *)(blk + P.off_hot);
+                const uint32_t *wkey = (const uint32_t *)(blk + P.off_wkey);
+                const uint4 *cold = (const uint4 *)(blk + P.off_cold + l * P.cold_stride), *qt = (const uint4 *)(blk + P.off_q + l * P.q_stride);
+                const uint2 *waux = (const uint2 *)(blk + P.off_waux + l * P.waux_stride);
+                for (uint32_t k = 0; k < N; k++, w += 4) { w[0] = H(3 * k) & 0xFFFFu; w[1] = H(3 * k) >> 16; w[2] = H(3 * k + 1); w[3] = H(3 * k + 2); }
                 for (size_t i = 0; i < Q; i++, w += 4) {
-                    if ((qfree[i >> 5] >> (i & 31)) & 1u) { w[0] = w[1] = w[2] = w[3] = 0; continue; }
+                    if ((H(P.hw_qfree + (uint32_t)(i >> 5)) >> (i & 31)) & 1u) { w[0] = w[1] = w[2] = w[3] = 0; continue; }
                     w[0] = qt[i].x; w[1] = qt[i].z; w[2] = qt[i].w; w[3] = qt[i].y;
                 }
                 memset(w, 0, 4 * 5 * RD);
@@ -662,14 +718,16 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
                 };
                 for (uint32_t k = 0; k < N; k++)
                     for (uint32_t sl = 0; sl < c->spec.model[k].slots; sl++) {
-                        if (!((occ[2 * k + (sl >> 5)] >> (sl & 31)) & 1u)) continue;
+                        if (!((H(P.hw_occ + 2 * k + (sl >> 5)) >> (sl & 31)) & 1u)) continue;
                         const uint32_t gs = P.slot_base[k] + sl;
-                        put((hot[gs] >> 16) & 0xFFFu, ST_RUN, k, cold[gs].y, cold[gs].x >> 16, cold[gs].x & 0xFFFFu, hot[gs] & 0xFFFFu, sl + 1);
+                        const uint32_t rem = hot[((gs >> 3) * 32 + l) * 8 + (gs & 7)];
+                        put(cold[gs].z & 0xFFFu, ST_RUN, k, cold[gs].y, cold[gs].x >> 16, cold[gs].x & 0xFFFFu, rem, sl + 1);
                     }
-                const uint32_t nw = hdr[P.hw_misc + 2];
-                for (uint32_t j = 0; j < nw && j < R; j++) {
-                    const uint32_t id = wkey[j] & 0xFFFu, tm = (wkey[j] >> 12) & 0xFFFFu;
-                    put(id, ST_WAIT, wkey[j] >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
+                const uint32_t nwl = H(P.hw_misc) & 0xFFFFu;
+                for (uint32_t j = 0; j < nwl && j < R; j++) {
+                    const uint32_t key = wkey[((j >> 2) * 32 + l) * 4 + (j & 3)];
+                    const uint32_t id = key & 0xFFFu, tm = (key >> 12) & 0xFFFFu;
+                    put(id, ST_WAIT, key >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
                 }
                 w += 5 * RD;
             }

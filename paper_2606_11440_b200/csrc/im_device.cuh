@@ -2,22 +2,31 @@
 // im_tanh) of the CUDA path.  Written independently of oracle/ (no shared code); the definitions follow
 // DESIGN.md readings R2, R3, R23, R24.
 //
-// HBM layout of the environment state: one contiguous record per env,
-//   [ header | issue list | hot[SP] | cold[SP] (uint2) | wkey[RCAP] | waux[RCAP] (uint2) | q[QCAP] (uint4) ]
-// SP = sum over models of ceil8(S_k): the slots of all models, numbered consecutively (R10).  The group of lanes
-// that owns an env streams `header` and `hot` with 128-bit coalesced loads and touches the other arrays only for the
-// few requests that change state in a tick.
-//   header (u32 words): m[N] as uint4 {n_wait, n_run, kv_used, ewma_q8} | occ[N] (u64: bit s = slot s taken) |
-//                       qfree[QW] | qready[QW] | misc[4] {drops, icnt, nw, -} | counters u64[16]
-//   hot[gs]  = remaining(16) | id<<16, id = 4*query + agent   — the only per-request word the service phase touches
-//   cold[gs] = {issue(16) | deadline<<16, sw}      sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
-//   wkey[j]  = model<<28 | time(16)<<12 | id       time = deadline (EDF) or issue tick (FCFS): one u32 compare orders
-//                                                   the waiting list by (model, R20 key)
-//   waux[j]  = {issue(16) | remaining<<16, sw}
-//   issue[j] = {wkey, sw}                          written by the executor kernel, appended to the list in phase D
-//   q[i]     = {plan word, budget | in_tok<<16, deadline, arrive}
-// The waiting list wkey/waux[0..nw) is compact and unordered; free query slots are defined by the qfree bitmap and
-// free service slots by occ (their words hold stale data).  Absolute ticks are < 65536 on the device.
+// HBM layout of the environment state.  Environments are grouped in BLOCKS of 32: block b
+// holds envs 32b .. 32b+31 and is owned by ONE WARP of the simulation kernel, lane = env & 31 (one thread per env).
+// A block is one contiguous record (stride multiple of 128 B):
+//   [ hdr | ctr | hot | wkey | iss | qready |  cold[32] | waux[32] | q[32] ]
+// The first six parts are struct-of-arrays ACROSS the 32 envs of the block ("SoA-32"): unit u of lane l sits at
+// part + (u * 32 + l) * unit_bytes, so that a warp whose lanes walk their own envs in step reads and writes whole
+// 128 .. 512-byte lines, and the header lands in shared memory as [word][lane] (bank = lane: conflict-free for any
+// word index) with ONE bulk copy (cp.async.bulk) per block.  The last three parts are per-env arrays (lane l at
+// part + l * stride): they are touched only at data-dependent positions by the few requests that change state.
+//   hdr   u32 units (hdr_words): m[3k] = n_wait | n_run << 16, m[3k+1] = kv_used, m[3k+2] = ewma_q8 |
+//         occ[2k], occ[2k+1] (bit s = slot s of model k taken) | qfree[QW] | misc0 = nw | drops << 16 | misc1 = icnt
+//   ctr   u32 units (16): the counters of enum Counter (absolute ticks < 65536 keep every sum below 2^32)
+//   hot   uint4 units (SP / 8): remaining tokens of the 8 slots of a group as 8 x u16 (slot 2j = low half of word j);
+//         a FREE slot holds 0, so the service pass needs no occupancy bits.  SP = sum_k ceil8(S_k): the slots of all
+//         models numbered consecutively (R10); a group belongs to ONE model and to ONE Philox call (R2)
+//   wkey  uint4 units (RCAP / 4): the waiting list, compact and unordered; key = model<<28 | time(16)<<12 | id, time =
+//         deadline (EDF) or issue tick (FCFS): one u32 compare orders by (model, R20 key); id = 4*query + agent.
+//         Entries of the last partly filled unit beyond the list length hold 0xFFFFFFFF (never a valid key)
+//   iss   uint2 units (kIssueCap): {key, static word} written by the executor kernel for this tick (phase D)
+//   qready u32 units (QW): queries whose next stage is due, kept only ACROSS im_rollout calls
+//   cold[gs] uint4 = {issue(16) | deadline<<16, sw, id, 0}    sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
+//   waux[j]  uint2 = {issue(16) | remaining<<16, sw}
+//   q[i]     uint4 = {plan word, budget | in_tok<<16, deadline, arrive}
+// Free query slots are defined by the qfree bitmap and free service slots by occ (their cold words hold stale data).
+// Absolute ticks are < 65536 on the device.
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
@@ -26,7 +35,7 @@
 namespace im {
 
 constexpr uint32_t kMaxModels = 16;
-constexpr uint32_t kRegions = 64;        // row-list / log regions (one atomic counter each), region = env % 64
+constexpr uint32_t kRegions = 64;        // row-list / log regions (one atomic counter each), region = (env / 32) % n_regions
 constexpr uint32_t kDtUs = 50000;
 constexpr uint32_t kIssueCap = 128;      // issue records per env per tick (31 arrivals x 3 calls + continuing stages)
 
@@ -71,6 +80,7 @@ struct QLog {
 
 struct Params {
     uint32_t E, N, QCAP, RCAP, QW, SP;                 // SP = padded slot count of the pool
+    uint32_t NB, n_regions;                            // 32-env blocks; row-list regions in use = min(kRegions, NB)
     uint32_t sched_mode, kv_preempt, cost_mode, episode_ticks, budget_norm, in_tok_const, mix_thresh, env_id_base;
     uint32_t mix_lo[2], mix_hi[2], depth_median[3];
     uint32_t flags, has_intok, seed_lo, seed_hi;
@@ -78,11 +88,13 @@ struct Params {
     ModelTab model[kMaxModels];
     uint32_t slot_base[kMaxModels + 1];      // first global slot of each model (multiples of 8)
     uint32_t svc_rk[20];                     // Philox round keys of the service stream (k0, k1 per round): constant-bank operands
-    // per-env record
+    // env state: one record per block of 32 envs (layout at the top of this file)
     uint8_t *env_base;
-    unsigned long long env_stride;           // bytes, multiple of 128
-    uint32_t hw_occ, hw_qfree, hw_qready, hw_misc, hw_ctr, hdr_words;     // header word offsets (m at word 0)
-    uint32_t off_iss, off_hot, off_cold, off_wkey, off_waux, off_q;       // byte offsets inside the record
+    unsigned long long blk_stride;           // bytes, multiple of 128
+    uint32_t hw_occ, hw_qfree, hw_misc, hdr_words;                        // header word indices (m at word 0)
+    uint32_t off_ctr, off_hot, off_wkey, off_iss, off_qready;             // SoA-32 parts: byte offsets inside the block (hdr at 0)
+    uint32_t off_cold, off_waux, off_q, cold_stride, waux_stride, q_stride;   // per-env parts: offset of lane 0 and lane stride
+    uint32_t n_grp, cm_words;                // SP / 8 slot groups; completion-mask words per env = ceil(n_grp / 4)
     float *snap;                             // [E][3N] telemetry features of the current tick (R14)
     const uint32_t *tab_mult, *tab_intok, *tab_cdf;
     const uint8_t *env_level;
@@ -101,8 +113,22 @@ struct Weights {          // device copies of one net, prepared by k_repack (im_
     uint8_t *tc_img;                     // tcgen05 path (F=128, H=256): shared-memory image of the net (im_tc.cuh), else null
 };
 
-__device__ __forceinline__ uint8_t *env_rec(const Params &P, uint32_t e) { return P.env_base + (size_t)e * P.env_stride; }
-__device__ __forceinline__ uint4 *env_q(const Params &P, uint32_t e) { return reinterpret_cast<uint4 *>(env_rec(P, e) + P.off_q); }
+__device__ __forceinline__ uint8_t *blk_rec(const Params &P, uint32_t e) { return P.env_base + (size_t)(e >> 5) * P.blk_stride; }
+// word w of env e's header (SoA-32: [word][lane])
+__device__ __forceinline__ uint32_t *hdr_word(const Params &P, uint32_t e, uint32_t w)
+{
+    return reinterpret_cast<uint32_t *>(blk_rec(P, e)) + w * 32u + (e & 31u);
+}
+__device__ __forceinline__ uint2 *iss_rec(const Params &P, uint32_t e, uint32_t slot)
+{
+    return reinterpret_cast<uint2 *>(blk_rec(P, e) + P.off_iss) + slot * 32u + (e & 31u);
+}
+__device__ __forceinline__ uint4 *env_q(const Params &P, uint32_t e)
+{
+    return reinterpret_cast<uint4 *>(blk_rec(P, e) + P.off_q + (size_t)(e & 31u) * P.q_stride);
+}
+// row-list / log region of an env: the 32 envs of a block share one, so that a warp claims rows with one atomic
+__device__ __forceinline__ uint32_t region_of(const Params &P, uint32_t e) { return (e >> 5) % P.n_regions; }
 
 // ------------------------------------------------------------------------------------------------ R2
 struct Ph4 { uint32_t x, y, z, w; };
@@ -111,10 +137,9 @@ __device__ __forceinline__ Ph4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t 
 {
 #pragma unroll
     for (int r = 0; r < 10; r++) {
-        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        c0 = hi1 ^ c1 ^ k0; c1 = lo1;
-        c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0, p1 = (unsigned long long)0xCD9E8D57u * c2;   // IMAD.WIDE
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0; c1 = (uint32_t)p1;
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1; c3 = (uint32_t)p0;
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     return Ph4{c0, c1, c2, c3};
@@ -125,10 +150,9 @@ __device__ __forceinline__ Ph4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32
 {
 #pragma unroll
     for (int r = 0; r < 10; r++) {
-        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        c0 = hi1 ^ c1 ^ rk[2 * r]; c1 = lo1;
-        c2 = hi0 ^ c3 ^ rk[2 * r + 1]; c3 = lo0;
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0, p1 = (unsigned long long)0xCD9E8D57u * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r]; c1 = (uint32_t)p1;
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1]; c3 = (uint32_t)p0;
     }
     return Ph4{c0, c1, c2, c3};
 }
@@ -221,7 +245,9 @@ __device__ __forceinline__ uint32_t row_gid_wrapped(const RowBuf &rb, uint32_t r
     return region * rb.regcap + r;
 }
 
-// claim n consecutive rows of region `region`; flags overflow in log mode
+// claim n consecutive rows of region `region`.  In log mode the region is a linear log of the rollout and an overflow is
+// flagged here; without the log it is a ring that only has to hold one tick's rows, and the consumer (sched_init of
+// im_policy.cu) flags a tick that produced more rows than the ring holds.
 __device__ __forceinline__ uint32_t rows_claim(const Params &P, const RowBuf &rb, uint32_t region, uint32_t n)
 {
     const uint32_t idx = atomicAdd(&rb.cnt[region], n);
@@ -242,5 +268,47 @@ __device__ __forceinline__ void write_exec_rows(const Params &P, uint32_t region
         P.exec.row[row_gid_wrapped(P.exec, region, idx0, j)] = make_uint4(e, a, (uint32_t)dl, in_tok);
     }
 }
+
+// ------------------------------------------------------------------------------------ bulk async copies (TMA, 1-D)
+// One elected lane moves a whole header block between HBM and shared memory; completion of a load is signalled on an
+// mbarrier (complete_tx), completion of a store through the bulk async-group.  Sizes and addresses are multiples of 16 B.
+namespace bulk {
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "BULK_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra BULK_DONE;\n\t"
+        "bra BULK_WAIT;\n\t"
+        "BULK_DONE:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void s2g(void *dst_gmem, const void *src_smem, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+}  // namespace bulk
 
 }  // namespace im

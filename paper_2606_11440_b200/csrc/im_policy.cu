@@ -21,10 +21,12 @@ struct TileSched {
     uint32_t crit_tiles, total;
 };
 
-__device__ __forceinline__ void sched_init(TileSched &S, const RowBuf &rb, uint32_t parity, uint32_t rows_per_tile, uint32_t n_crit)
+__device__ __forceinline__ void sched_init(const Params &P, TileSched &S, const RowBuf &rb, uint32_t parity, uint32_t rows_per_tile, uint32_t n_crit)
 {
     if (threadIdx.x < kRegions) {
         const uint32_t b = rb.base[parity * kRegions + threadIdx.x], c = rb.cnt[threadIdx.x];
+        // a ring (no decision log) holds one tick's rows: more than regcap of them have overwritten each other
+        if (blockIdx.x == 0 && !P.log_mode && c - b > rb.regcap) atomicOr(P.err_flag, 1u);
         S.base[threadIdx.x] = b;
         S.cnt[threadIdx.x] = c;
         S.pref[threadIdx.x + 1] = (c - b + rows_per_tile - 1) / rows_per_tile;
@@ -117,11 +119,10 @@ __device__ __forceinline__ void exec_commit(const Params &P, const RowInfo &ri, 
     uint32_t out_total = (uint32_t)(((unsigned long long)P.depth_median[depth] * __ldg(&P.tab_mult[d.y >> 22])) >> 16);
     out_total = out_total < 1u ? 1u : out_total;
     const uint32_t succ = d.z < P.model[model].succ[depth] ? 1u : 0u;
-    uint8_t *rec = env_rec(P, ri.env);
-    const uint32_t slot = slot_in != ~0u ? slot_in : atomicAdd(reinterpret_cast<uint32_t *>(rec) + P.hw_misc + 1, 1u);
+    const uint32_t slot = slot_in != ~0u ? slot_in : atomicAdd(hdr_word(P, ri.env, P.hw_misc + 1u), 1u);
     const uint32_t tm = (uint32_t)(P.sched_mode ? ri.dl : t) & 0xFFFFu;             // R20: deadline (EDF) or issue tick (FCFS)
     if (slot < kIssueCap)
-        reinterpret_cast<uint2 *>(rec + P.off_iss)[slot] =
+        *iss_rec(P, ri.env, slot) =
             make_uint2((model << 28) | (tm << 12) | (q << 2) | agent,
                        out_total | ((ri.c & 0xFFFFu) << SW_IN_SHIFT) | (succ << SW_SUCC_SHIFT) | (depth << SW_DEPTH_SHIFT));
     else
@@ -160,7 +161,7 @@ __device__ __forceinline__ void plan_commit(const Params &P, const RowInfo &ri, 
     stage_calls(topo, keff, 0, a0, nc);
     const uint32_t pw = QP_LIVE | QP_PLANNED | (topo << 2) | (cnt << 4) | (keff << 6) | (nst << 12) | (roles << QP_ROLE_SHIFT);
     env_q(P, ri.env)[q].x = pw | (1u << 9) | (nc << QP_PEND_SHIFT);
-    const uint32_t region = ri.env % kRegions;
+    const uint32_t region = region_of(P, ri.env);
     const uint32_t idx0 = claimed_idx0 != ~0u ? claimed_idx0 : rows_claim(P, P.exec, region, nc) % P.exec.regcap;
     write_exec_rows(P, region, idx0, ri.env, q, pw, ri.c & 0xFFFFu, ri.dl, t_rel, a0, nc);
 }
@@ -206,7 +207,7 @@ k_policy_f32(const Params P, const Weights W, uint32_t parity, int32_t t0, uint3
     for (uint32_t i = threadIdx.x; i < NOP; i += blockDim.x) sb3[i] = W.b3[i];
     const RowBuf &rb = EXEC ? P.exec : P.plan;
     const uint32_t n_crit = EXEC ? P.E : 0u;
-    sched_init(sched, rb, parity, kF32Rows, n_crit);
+    sched_init(P, sched, rb, parity, kF32Rows, n_crit);
 
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const uint32_t per_warp = kF32RowsPerWarp * (F + 2 * H + 128);
@@ -351,7 +352,7 @@ k_policy_bf16(const Params P, const Weights W, uint32_t parity, int32_t t0, uint
     float *lg = reinterpret_cast<float *>(actA);   // logits [128][64] fp32 reuse actA after layer 2 consumed it
     const RowBuf &rb = EXEC ? P.exec : P.plan;
     const uint32_t n_crit = EXEC ? P.E : 0u;
-    sched_init(sched, rb, parity, kBfRows, n_crit);
+    sched_init(P, sched, rb, parity, kBfRows, n_crit);
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int g = lane >> 2, tq = lane & 3;
     const uint32_t n_tiles3 = W.n_out_pad / 8;
@@ -599,7 +600,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     if (threadIdx.x < 32) tc::tmem_alloc(&tmem_slot, Net::kTmemCols);
     const RowBuf &rb = EXEC ? P.exec : P.plan;
     const uint32_t n_crit = EXEC ? P.E : 0u;
-    sched_init(sched, rb, parity, 128, n_crit);
+    sched_init(P, sched, rb, parity, 128, n_crit);
     tc::tc_fence_before();
     __syncthreads();
     tc::tc_fence_after();
@@ -720,7 +721,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         // ---- warpgroup 0: sampling epilogue of row r, logits in registers
         const TcRowSlot sl = rowbuf[128 * (it & 1u) + r];
         uint32_t islot = ~0u;                              // executor rows: the env's issue-list slot, claimed before the wait
-        if (EXEC && (sl.flags & 3u) == 1u) islot = atomicAdd(reinterpret_cast<uint32_t *>(env_rec(P, sl.row.x)) + P.hw_misc + 1, 1u);
+        if (EXEC && (sl.flags & 3u) == 1u) islot = atomicAdd(hdr_word(P, sl.row.x, P.hw_misc + 1u), 1u);
         tc::mbar_wait(&bars[4], phase);
         tc::tc_fence_after();
         float l[NO];
@@ -781,7 +782,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (uint32_t)o) inc += v; }
             const uint32_t tot = __shfl_sync(0xffffffffu, inc, 31), okm = __ballot_sync(0xffffffffu, ok);
             if (tot) {
-                const uint32_t region = __shfl_sync(0xffffffffu, ri.env % kRegions, __ffs(okm) - 1);
+                const uint32_t region = __shfl_sync(0xffffffffu, region_of(P, ri.env), __ffs(okm) - 1);
                 uint32_t base = 0;
                 if (lane == 0) base = rows_claim(P, P.exec, region, tot) % P.exec.regcap;
                 uint32_t idx0 = __shfl_sync(0xffffffffu, base, 0) + inc - nc;
@@ -796,46 +797,45 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
+// opt-in to large dynamic shared memory on the CURRENT device (the attribute is per device: im_bind calls this once per ctx)
+int policy_prepare_device(const Params &P)
+{
+    const int big = 200 * 1024;
+    cudaError_t e = cudaSuccess;
+    auto set = [&](const void *f, int bytes) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); };
+    set((const void *)k_policy_f32<true>, big);
+    set((const void *)k_policy_f32<false>, big);
+    set((const void *)k_policy_bf16<64, 128, true>, (int)bf16_smem_bytes<64, 128>());
+    set((const void *)k_policy_bf16<64, 128, false>, (int)bf16_smem_bytes<64, 128>());
+    const int tc_smem = (int)(((tc_image_bytes(true) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot));
+    set((const void *)k_policy_tc<true>, tc_smem);
+    set((const void *)k_policy_tc<false>, tc_smem);
+    (void)P;
+    return e == cudaSuccess ? 0 : -1;
+}
+
 int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm,
                   bool bf16, cudaStream_t st)
 {
     if (!bf16) {
         const size_t smem = f32_smem_bytes(P.f_in, P.hidden, W.n_out_pad);
-        static size_t set_p = 0, set_e = 0;
-        if (exec) { if (set_e < smem) { cudaFuncSetAttribute(k_policy_f32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); set_e = smem; } }
-        else { if (set_p < smem) { cudaFuncSetAttribute(k_policy_f32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); set_p = smem; } }
         const uint32_t grid = (uint32_t)n_sm * 2;
         if (exec) k_policy_f32<true><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
         else k_policy_f32<false><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
         return 0;
     }
-    if (W.tc_img) {
+    if (W.tc_img) {      // F = 128, H = 256: tcgen05
         const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot);
-        if (exec) {
-            cudaFuncSetAttribute(k_policy_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            k_policy_tc<true><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
-        } else {
-            cudaFuncSetAttribute(k_policy_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            k_policy_tc<false><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
-        }
+        if (exec) k_policy_tc<true><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
+        else k_policy_tc<false><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
         return 0;
     }
-    const uint32_t grid = (uint32_t)n_sm;
-#define IM_BF16_CASE(FF, HH)                                                                                          \
-    if (P.f_in == FF && P.hidden == HH) {                                                                             \
-        const size_t smem = bf16_smem_bytes<FF, HH>();                                                                \
-        if (exec) {                                                                                                   \
-            cudaFuncSetAttribute(k_policy_bf16<FF, HH, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            k_policy_bf16<FF, HH, true><<<grid, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);                   \
-        } else {                                                                                                      \
-            cudaFuncSetAttribute(k_policy_bf16<FF, HH, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);\
-            k_policy_bf16<FF, HH, false><<<grid, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);                  \
-        }                                                                                                             \
-        return 0;                                                                                                     \
+    if (P.f_in == 64 && P.hidden == 128) {      // too narrow for a 128 x 256 UMMA tile to pay: mma.sync
+        const size_t smem = bf16_smem_bytes<64, 128>();
+        if (exec) k_policy_bf16<64, 128, true><<<(uint32_t)n_sm, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);
+        else k_policy_bf16<64, 128, false><<<(uint32_t)n_sm, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);
+        return 0;
     }
-    IM_BF16_CASE(64, 128)
-    IM_BF16_CASE(128, 256)
-#undef IM_BF16_CASE
     return -1;
 }
 

@@ -135,12 +135,12 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
     uint32_t n2cap = 32;
     while (n2cap < P.RCAP) n2cap <<= 1;
     uint32_t *keys = s_keys + (size_t)wib * n2cap;
-    const uint8_t *rec = env_rec(P, e);
-    const uint32_t *hdr = (const uint32_t *)rec, *wkey = (const uint32_t *)(rec + P.off_wkey);
-    const uint32_t n = min(hdr[P.hw_misc + 2], P.RCAP);
+    // the waiting list of env e: key j is component j & 3 of unit j >> 2 of the block's SoA-32 key array (im_device.cuh)
+    const uint32_t *wkey = reinterpret_cast<const uint32_t *>(blk_rec(P, e) + P.off_wkey) + (e & 31u) * 4u;
+    const uint32_t n = min(*hdr_word(P, e, P.hw_misc) & 0xFFFFu, P.RCAP);
     uint32_t n2 = 32;
     while (n2 < n) n2 <<= 1;
-    for (uint32_t i = lane; i < n2; i += 32) keys[i] = i < n ? wkey[i] : 0xFFFFFFFFu;
+    for (uint32_t i = lane; i < n2; i += 32) keys[i] = i < n ? wkey[(i >> 2) * 128u + (i & 3u)] : 0xFFFFFFFFu;
     __syncwarp();
     for (uint32_t k = 2; k <= n2; k <<= 1) {
         uint32_t j = k >> 1;
@@ -169,7 +169,7 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
         __syncwarp();
     }
     uint32_t *o = out + (size_t)e * (P.N + 1 + P.RCAP);
-    const uint32_t per_model = lane < P.N ? hdr[4 * lane] : 0u;               // n_wait of model `lane`
+    const uint32_t per_model = lane < P.N ? (*hdr_word(P, e, 3u * lane) & 0xFFFFu) : 0u;    // n_wait of model `lane`
     const uint32_t inc = [&] { uint32_t v = per_model; for (int s = 1; s < 32; s <<= 1) { const uint32_t u = __shfl_up_sync(0xffffffffu, v, s); if (lane >= (uint32_t)s) v += u; } return v; }();
     if (lane < P.N) o[lane + 1] = inc;
     if (lane == 0) o[0] = 0;
