@@ -22,10 +22,12 @@
  * tables (P2-P4), M/M/1 mean sojourn 1/(mu-lambda) (P6), Little's law (P7), conservation (P8), EDF
  * brute force (P9), action decode (P10), sampler closed forms (P11), MLP vs float64 numpy (P12), GAE
  * vs direct discounted sum (P13), Lagrangian linearity (P14), determinism / split / E-invariance (P15),
- * utility normalisation (P17), deterministic stamps (P18), preemption (P19), service rate (P20).
+ * utility normalisation (P17), deterministic stamps (P18), preemption (P19), service rate (P20); and
+ * (tests/test_oracle_pins2.py) the cost value l/beta per call, the success bit and its OR
+ * composition (R18/R19), the debate / review stage tables and K_eff (R17), the head-of-line stop under a KV
+ * misfit (R21), the episode hard reset (R33) and the near-boundary window (R25).
  * PARITY UNPINNED (definitional readings with no external truth): role semantics (R16),
- * OR-composition of call successes (R19), feature scale constants (R14-15), drop penalty (R9),
- * snapshot staleness (R14).
+ * feature scale constants (R14-15), drop penalty (R9), snapshot staleness (R14).
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/oracle.py).
  */
@@ -242,6 +244,9 @@ static int near_ok(const float *c, uint32_t n, float u, uint32_t a)
     double hi = (a == n - 1) ? 1.0 : (double)c[a] / Z;
     return ((double)u >= lo - 1e-6) && ((double)u <= hi + 1e-6);
 }
+
+/* exported for its pin (tests/test_oracle_pins2.py): the same function, callable */
+int orc_near_ok(const float *c, uint32_t n, float u, uint32_t a) { return near_ok(c, n, u, a); }
 
 /* --------------------------------------------------------------------------- R22 / R25: MLP */
 static float bf16_round(float x) /* RNE to bf16, returned as fp32 */

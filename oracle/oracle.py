@@ -94,6 +94,8 @@ def lib():
         L.orc_read_queries.argtypes = [C.c_void_p] * 5
         L.orc_queue_order.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_int32, C.c_void_p, C.c_uint32]
         L.orc_mlp_forward.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_near_ok.restype = C.c_int
+        L.orc_near_ok.argtypes = [C.c_void_p, C.c_uint32, C.c_float, C.c_uint32]
         L.orc_tick.restype = C.c_int32
         L.orc_tick.argtypes = [C.c_void_p]
         _lib = L
@@ -123,6 +125,12 @@ def sample(logits: np.ndarray, u: float):
     cdf = np.zeros(64, dtype=np.float32)
     a = lib().orc_sample(_p(l), l.size, C.c_float(u), C.byref(lp), _p(cdf))
     return int(a), float(lp.value), cdf[: l.size].copy()
+
+
+def near_ok(cdf: np.ndarray, u: float, a: int) -> bool:
+    """R25(3): is action `a` acceptable for uniform u, i.e. within 1e-6 of its CDF interval (cdf = running sums)."""
+    c = np.ascontiguousarray(cdf, dtype=np.float32)
+    return bool(lib().orc_near_ok(_p(c), c.size, C.c_float(u), a))
 
 
 def gae(rew, cost, val, done, gamma, lam, mu):
