@@ -15,6 +15,7 @@
 
 namespace im {
 void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st);
+void launch_serve(const Params &P, int32_t t, cudaStream_t st);
 int sim_prepare_device();
 int policy_prepare_device(const Params &P);
 int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm, bool bf16, cudaStream_t st);
@@ -30,12 +31,18 @@ void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t
 // and therefore never admit a query)
 __global__ void k_reset(const Params P)
 {
-    const uint32_t words = P.off_wkey / 4;                       // hdr | ctr | hot
+    const uint32_t words = P.off_iss / 4;                        // hdr | cm | kvt | ctr | hot
+    const uint32_t real_chunks = P.RCAP / 16 + P.N;
     const size_t n = (size_t)P.NB * words;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const uint32_t b = (uint32_t)(i / words), w = (uint32_t)(i % words);
+        const uint32_t b = (uint32_t)(i / words), w = (uint32_t)(i % words), hw = w >> 5;
         uint32_t v = 0;
-        if (w >= P.hw_qfree * 32u && w < (P.hw_qfree + P.QW) * 32u && b * 32u + (w & 31u) < P.E) v = 0xFFFFFFFFu;
+        if (hw >= P.hw_qfree && hw < P.hw_qfree + P.QW && b * 32u + (w & 31u) < P.E) v = 0xFFFFFFFFu;
+        if (hw >= P.hw_tail && hw < P.hw_tail + 4) v = 0xFFFFFFFFu;                       // no model has a tail chunk
+        if (hw >= P.hw_used && hw < P.hw_tail) {                                          // chunks that do not exist are "used"
+            const uint32_t c0 = (hw - P.hw_used) * 32u;
+            v = c0 >= real_chunks ? 0xFFFFFFFFu : (real_chunks - c0 >= 32u ? 0u : ~((1u << (real_chunks - c0)) - 1u));
+        }
         reinterpret_cast<uint32_t *>(P.env_base + (size_t)b * P.blk_stride)[w] = v;
     }
     const uint32_t qw = P.QW * 32u;
@@ -266,16 +273,20 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     for (uint32_t k = 0; k < kMaxModels; k++) P.slot_base[k + 1] = P.slot_base[k] + (k < N ? ((s.model[k].slots + 7u) & ~7u) : 0u);
     P.SP = P.slot_base[N];
     P.n_grp = P.SP / 8; P.cm_words = (P.n_grp + 3u) / 4u;
-    P.hw_occ = 3 * N; P.hw_qfree = P.hw_occ + 2 * N; P.hw_misc = P.hw_qfree + P.QW; P.hdr_words = P.hw_misc + 2;
+    P.n_chunks = (R / 16 + N + 31u) & ~31u;                    // usable: R / 16 + N (the rest is marked used by k_reset)
+    P.hw_occ = 3 * N; P.hw_qfree = P.hw_occ + 2 * N; P.hw_meta = P.hw_qfree + P.QW; P.hw_used = P.hw_meta + P.n_chunks / 8;
+    P.hw_tail = P.hw_used + P.n_chunks / 32; P.hw_misc = P.hw_tail + 4; P.hdr_words = P.hw_misc + 2;
     auto up128 = [](uint32_t x) { return (x + 127u) & ~127u; };
     uint32_t off = P.hdr_words * 128u;
+    P.off_cm = off; off += P.cm_words * 128u;                 // directly behind the header: one bulk copy brings both
+    P.off_kvt = off; off += N * 128u;
     P.off_ctr = off; off += (uint32_t)C_N * 128u;
     P.off_hot = off; off += P.n_grp * 512u;
-    P.off_wkey = off; off += R * 128u;                        // (R / 4) units of 16 B x 32 lanes
     P.off_iss = off; off += kIssueCap * 256u;
     P.off_qready = off; off += P.QW * 128u;
-    P.cold_stride = up128(P.SP * 16u); P.waux_stride = R * 8u; P.q_stride = Q * 16u;
+    P.cold_stride = up128(P.SP * 16u); P.wkey_stride = P.n_chunks * 64u; P.waux_stride = P.n_chunks * 128u; P.q_stride = Q * 16u;
     P.off_cold = off; off += 32u * P.cold_stride;
+    P.off_wkey = off; off += 32u * P.wkey_stride;
     P.off_waux = off; off += 32u * P.waux_stride;
     P.off_q = off; off += 32u * P.q_stride;
     P.blk_stride = up128(off);
@@ -512,9 +523,10 @@ int im_rollout(im_ctx *c, const void *policy_weights, uint32_t n_ticks)
         c->par_exec ^= 1;
         const bool last = (i + 1 == n_ticks);
         prof_begin(c, IM_KERNEL_SIM);
-        launch_sim(P, t, i, t + 1, last ? 2u : 1u, t0, st);                 // D-issue .. I of tick t, A, B of tick t+1
+        launch_serve(P, t, st);                                             // F of tick t
+        launch_sim(P, t, i, t + 1, last ? 2u : 1u, t0, st);                 // D-issue, E, G .. I of tick t, A, B of tick t+1
         prof_end(c);
-        c->launches += 3;
+        c->launches += 4;
     }
     prof_begin(c, IM_KERNEL_EXEC);
     launch_policy(P, c->We, true, c->par_exec, t0, n_ticks, c->n_sm, bf16, st);  // bootstrap V[n_ticks] (R30)
@@ -701,7 +713,7 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
                 const uint32_t *hdr = (const uint32_t *)blk;
                 auto H = [&](uint32_t wd) { return hdr[wd * 32 + l]; };
                 const uint16_t *hot = (const uint16_t *)(blk + P.off_hot);
-                const uint32_t *wkey = (const uint32_t *)(blk + P.off_wkey);
+                const uint32_t *wkey = (const uint32_t *)(blk + P.off_wkey + l * P.wkey_stride);
                 const uint4 *cold = (const uint4 *)(blk + P.off_cold + l * P.cold_stride), *qt = (const uint4 *)(blk + P.off_q + l * P.q_stride);
                 const uint2 *waux = (const uint2 *)(blk + P.off_waux + l * P.waux_stride);
                 for (uint32_t k = 0; k < N; k++, w += 4) { w[0] = H(3 * k) & 0xFFFFu; w[1] = H(3 * k) >> 16; w[2] = H(3 * k + 1); w[3] = H(3 * k + 2); }
@@ -723,11 +735,14 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
                         const uint32_t rem = hot[((gs >> 3) * 32 + l) * 8 + (gs & 7)];
                         put(cold[gs].z & 0xFFFu, ST_RUN, k, cold[gs].y, cold[gs].x >> 16, cold[gs].x & 0xFFFFu, rem, sl + 1);
                     }
-                const uint32_t nwl = H(P.hw_misc) & 0xFFFFu;
-                for (uint32_t j = 0; j < nwl && j < R; j++) {
-                    const uint32_t key = wkey[((j >> 2) * 32 + l) * 4 + (j & 3)];
-                    const uint32_t id = key & 0xFFFu, tm = (key >> 12) & 0xFFFFu;
-                    put(id, ST_WAIT, key >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
+                for (uint32_t ch = 0; ch < P.RCAP / 16 + P.N; ch++) {          // waiting lists: the chunks in use
+                    if (!((H(P.hw_used + (ch >> 5)) >> (ch & 31)) & 1u)) continue;
+                    for (uint32_t j = ch * 16; j < ch * 16 + 16; j++) {
+                        const uint32_t key = wkey[j];
+                        if (key == 0xFFFFFFFFu) continue;
+                        const uint32_t id = key & 0xFFFu, tm = (key >> 12) & 0xFFFFu;
+                        put(id, ST_WAIT, key >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
+                    }
                 }
                 w += 5 * RD;
             }

@@ -5,25 +5,31 @@
 // HBM layout of the environment state.  Environments are grouped in BLOCKS of 32: block b
 // holds envs 32b .. 32b+31 and is owned by ONE WARP of the simulation kernel, lane = env & 31 (one thread per env).
 // A block is one contiguous record (stride multiple of 128 B):
-//   [ hdr | ctr | hot | wkey | iss | qready |  cold[32] | waux[32] | q[32] ]
-// The first six parts are struct-of-arrays ACROSS the 32 envs of the block ("SoA-32"): unit u of lane l sits at
+//   [ hdr | cm | kvt | ctr | hot | iss | qready |  cold[32] | wkey[32] | waux[32] | q[32] ]
+// The first seven parts are struct-of-arrays ACROSS the 32 envs of the block ("SoA-32"): unit u of lane l sits at
 // part + (u * 32 + l) * unit_bytes, so that a warp whose lanes walk their own envs in step reads and writes whole
 // 128 .. 512-byte lines, and the header lands in shared memory as [word][lane] (bank = lane: conflict-free for any
-// word index) with ONE bulk copy (cp.async.bulk) per block.  The last three parts are per-env arrays (lane l at
+// word index) with ONE bulk copy (cp.async.bulk) per block.  The last four parts are per-env arrays (lane l at
 // part + l * stride): they are touched only at data-dependent positions by the few requests that change state.
 //   hdr   u32 units (hdr_words): m[3k] = n_wait | n_run << 16, m[3k+1] = kv_used, m[3k+2] = ewma_q8 |
-//         occ[2k], occ[2k+1] (bit s = slot s of model k taken) | qfree[QW] | misc0 = nw | drops << 16 | misc1 = icnt
+//         occ[2k], occ[2k+1] (bit s = slot s of model k taken) | qfree[QW] | the chunk directory of the waiting
+//         lists: owner nibbles (8 chunks per word) | used bitmap | tail chunk of every model (4 bytes per word,
+//         0xFF = none) | misc0 = drops | misc1 = icnt
+//   cm    u32 units (cm_words): completion bytes of the tick's service pass, one per slot group (k_serve -> k_sim)
+//   kvt   u32 units (N): tokens decoded per model by the tick's service pass (k_serve -> k_sim)
 //   ctr   u32 units (16): the counters of enum Counter (absolute ticks < 65536 keep every sum below 2^32)
 //   hot   uint4 units (SP / 8): remaining tokens of the 8 slots of a group as 8 x u16 (slot 2j = low half of word j);
 //         a FREE slot holds 0, so the service pass needs no occupancy bits.  SP = sum_k ceil8(S_k): the slots of all
 //         models numbered consecutively (R10); a group belongs to ONE model and to ONE Philox call (R2)
-//   wkey  uint4 units (RCAP / 4): the waiting list, compact and unordered; key = model<<28 | time(16)<<12 | id, time =
-//         deadline (EDF) or issue tick (FCFS): one u32 compare orders by (model, R20 key); id = 4*query + agent.
-//         Entries of the last partly filled unit beyond the list length hold 0xFFFFFFFF (never a valid key)
 //   iss   uint2 units (kIssueCap): {key, static word} written by the executor kernel for this tick (phase D)
 //   qready u32 units (QW): queries whose next stage is due, kept only ACROSS im_rollout calls
 //   cold[gs] uint4 = {issue(16) | deadline<<16, sw, id, 0}    sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
-//   waux[j]  uint2 = {issue(16) | remaining<<16, sw}
+//   wkey[c][16], waux[c][16]: the waiting lists, ONE UNORDERED LIST PER MODEL built from chunks of 16 entries out of a
+//         pool of n_chunks = RCAP/16 + N per env (a model has at most one partly filled chunk, its tail, so the pool
+//         always suffices): admission only reads the chunks of the model that admits.  key = model<<28 |
+//         time(16)<<12 | id, time = deadline (EDF) or issue tick (FCFS): one u32 compare is the R20 order; id =
+//         4*query + agent; an empty entry of a chunk in use holds 0xFFFFFFFF (never a valid key).
+//         waux = {issue(16) | remaining<<16, sw}
 //   q[i]     uint4 = {plan word, budget | in_tok<<16, deadline, arrive}
 // Free query slots are defined by the qfree bitmap and free service slots by occ (their cold words hold stale data).
 // Absolute ticks are < 65536 on the device.
@@ -91,10 +97,11 @@ struct Params {
     // env state: one record per block of 32 envs (layout at the top of this file)
     uint8_t *env_base;
     unsigned long long blk_stride;           // bytes, multiple of 128
-    uint32_t hw_occ, hw_qfree, hw_misc, hdr_words;                        // header word indices (m at word 0)
-    uint32_t off_ctr, off_hot, off_wkey, off_iss, off_qready;             // SoA-32 parts: byte offsets inside the block (hdr at 0)
-    uint32_t off_cold, off_waux, off_q, cold_stride, waux_stride, q_stride;   // per-env parts: offset of lane 0 and lane stride
+    uint32_t hw_occ, hw_qfree, hw_meta, hw_used, hw_tail, hw_misc, hdr_words;   // header word indices (m at word 0)
+    uint32_t off_cm, off_kvt, off_ctr, off_hot, off_iss, off_qready;      // SoA-32 parts: byte offsets inside the block (hdr at 0)
+    uint32_t off_cold, off_wkey, off_waux, off_q, cold_stride, wkey_stride, waux_stride, q_stride;   // per-env parts: lane 0 and lane stride
     uint32_t n_grp, cm_words;                // SP / 8 slot groups; completion-mask words per env = ceil(n_grp / 4)
+    uint32_t n_chunks;                       // waiting-list chunks per env (multiple of 32 for the bitmap; those beyond RCAP/16 + N are marked used)
     float *snap;                             // [E][3N] telemetry features of the current tick (R14)
     const uint32_t *tab_mult, *tab_intok, *tab_cdf;
     const uint8_t *env_level;

@@ -132,15 +132,21 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const uint32_t e = blockIdx.x * kQoWarps + wib;
     if (e >= P.E) return;
+    const uint32_t n_ent = P.n_chunks * 16u;
     uint32_t n2cap = 32;
-    while (n2cap < P.RCAP) n2cap <<= 1;
+    while (n2cap < n_ent) n2cap <<= 1;
     uint32_t *keys = s_keys + (size_t)wib * n2cap;
-    // the waiting list of env e: key j is component j & 3 of unit j >> 2 of the block's SoA-32 key array (im_device.cuh)
-    const uint32_t *wkey = reinterpret_cast<const uint32_t *>(blk_rec(P, e) + P.off_wkey) + (e & 31u) * 4u;
-    const uint32_t n = min(*hdr_word(P, e, P.hw_misc) & 0xFFFFu, P.RCAP);
-    uint32_t n2 = 32;
-    while (n2 < n) n2 <<= 1;
-    for (uint32_t i = lane; i < n2; i += 32) keys[i] = i < n ? wkey[(i >> 2) * 128u + (i & 3u)] : 0xFFFFFFFFu;
+    // the waiting lists of env e: the entries of its chunks in use (im_device.cuh); empty entries hold 0xFFFFFFFF and sort last
+    const uint32_t *wkey = reinterpret_cast<const uint32_t *>(blk_rec(P, e) + P.off_wkey + (size_t)(e & 31u) * P.wkey_stride);
+    uint32_t n = 0;
+    for (uint32_t k = 0; k < P.N; k++) n += *hdr_word(P, e, 3u * k) & 0xFFFFu;
+    n = min(n, P.RCAP);
+    const uint32_t n2 = n2cap;
+    for (uint32_t i = lane; i < n2; i += 32) {
+        const uint32_t ch = i >> 4;
+        const bool used = i < n_ent && ((*hdr_word(P, e, P.hw_used + (ch >> 5)) >> (ch & 31u)) & 1u) && ch < P.RCAP / 16 + P.N;
+        keys[i] = used ? wkey[i] : 0xFFFFFFFFu;
+    }
     __syncwarp();
     for (uint32_t k = 2; k <= n2; k <<= 1) {
         uint32_t j = k >> 1;
@@ -179,7 +185,7 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st)
 {
     uint32_t n2cap = 32;
-    while (n2cap < P.RCAP) n2cap <<= 1;
+    while (n2cap < P.n_chunks * 16u) n2cap <<= 1;
     const size_t smem = (size_t)kQoWarps * n2cap * 4;
     cudaFuncSetAttribute(k_queue_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_queue_order<<<(P.E + kQoWarps - 1) / kQoWarps, kQoWarps * 32, smem, st>>>(P, t, out);

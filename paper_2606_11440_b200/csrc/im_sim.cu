@@ -27,18 +27,18 @@
 
 namespace im {
 
-constexpr int kSimWarps = 4;            // 32-env blocks per CTA
+constexpr int kSimWarps = 2;            // 32-env blocks per CTA
+constexpr int kServeWarps = 8;
 constexpr uint32_t kFull = 0xffffffffu;
 
-// per-warp dynamic shared memory: header [hdr_words][32] | completion masks [cm_words][32] | service tokens [N][32]
-struct SimSmem { uint32_t hdr_bytes, o_cm, o_kv, per_warp; };
+// per-warp dynamic shared memory of k_sim: header [hdr_words][32] | completion masks [cm_words][32] (one bulk copy)
+struct SimSmem { uint32_t hdr_bytes, o_cm, per_warp; };
 static SimSmem sim_smem(const Params &P)
 {
     SimSmem L;
     L.hdr_bytes = P.hdr_words * 128u;
     L.o_cm = L.hdr_bytes;
-    L.o_kv = L.o_cm + P.cm_words * 128u;
-    L.per_warp = L.o_kv + P.N * 128u;
+    L.per_warp = L.o_cm + P.cm_words * 128u;
     return L;
 }
 
@@ -65,14 +65,63 @@ __device__ __forceinline__ uint32_t u16_field(const Ph4 &u, uint32_t f)
     return (f & 1u) ? (w >> 16) : (w & 0xFFFFu);
 }
 
+// =================================================================================================== F serve (R11)
+// The service pass of tick t: one streaming pass over the slots of every env.  It needs nothing but `hot` (a free slot
+// holds 0), so it is a kernel of its own with no shared memory and all its loads in flight at once: a warp takes the
+// (<= 8) slot groups of ONE model of one 32-env block, lane = env, so every load / store is 512 contiguous bytes and
+// the model's parameters are uniform.  Results for k_sim: the tokens decoded per (env, model) and one completion byte
+// per (env, group) (bits 0-3 = slots 0, 2, 4, 6; bits 4-7 = slots 1, 3, 5, 7), both SoA-32 behind the header.
+// The requests admitted in THIS tick are served by k_sim's admission phase (prefill, R11): they are not in `hot` yet.
+__global__ void __launch_bounds__(kServeWarps * 32)
+k_serve(const Params P, int32_t t)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t w = blockIdx.x * kServeWarps + (threadIdx.x >> 5);
+    if (w >= P.NB * P.N) return;
+    const uint32_t blk = P.NB - 1u - w / P.N, k = w % P.N;
+    const uint32_t g0 = P.slot_base[k] >> 3, ng = (P.slot_base[k + 1] - P.slot_base[k]) >> 3;    // 1 .. 8 groups
+    const uint32_t gid = P.env_id_base + blk * 32u + lane;
+    uint8_t *blkp = P.env_base + (size_t)blk * P.blk_stride;
+    uint4 *hot4 = reinterpret_cast<uint4 *>(blkp + P.off_hot) + lane;                   // group g at hot4[g * 32]
+    uint8_t *cmb = blkp + P.off_cm + lane * 4u;                                         // byte of group g at cmb[(g >> 2) * 128 + (g & 3)]
+    const uint32_t x = P.model[k].rate * kDtUs;                                         // rate <= 80000 => fits 32 bits
+    const uint32_t base2 = (x / 1000000u) * 0x00010001u;
+    const uint32_t thr2 = (uint32_t)(((unsigned long long)(x % 1000000u) << 16) / 1000000u) * 0x00010001u;   // R11: Bernoulli to 2^-16
+    uint4 h[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) if ((uint32_t)i < ng) h[i] = hot4[(g0 + i) * 32u];
+    uint32_t tot = 0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+        if ((uint32_t)i < ng) {
+            const uint32_t g = g0 + i;
+            const bool any = (h[i].x | h[i].y | h[i].z | h[i].w) != 0;
+            uint32_t cacc = 0;
+            if (__any_sync(kFull, any)) {
+                const Ph4 u = philox4x32_10_rk(gid, (uint32_t)t, g, 0u, P.svc_rk);
+                uint32_t totp = 0;
+                uint4 r;
+                r.x = serve_pair(h[i].x, u.x, base2, thr2, 0, totp, cacc);
+                r.y = serve_pair(h[i].y, u.y, base2, thr2, 1, totp, cacc);
+                r.z = serve_pair(h[i].z, u.z, base2, thr2, 2, totp, cacc);
+                r.w = serve_pair(h[i].w, u.w, base2, thr2, 3, totp, cacc);
+                tot += (totp & 0xFFFFu) + (totp >> 16);
+                if (any) hot4[g * 32u] = r;
+            }
+            cmb[(g >> 2) * 128u + (g & 3u)] = (uint8_t)((cacc & 0xFu) | ((cacc >> 12) & 0xF0u));
+        }
+    }
+    reinterpret_cast<uint32_t *>(blkp + P.off_kvt)[k * 32u + lane] = tot;
+}
+
 // tick arguments: t_post < 0 => no post phases; pre_mode 0 none, 1 full (A, B, rows), 2 snapshot only
-__global__ void __launch_bounds__(kSimWarps * 32)
+__global__ void __launch_bounds__(kSimWarps * 32, 5)
 k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint64_t s_bar[kSimWarps];
     __shared__ uint32_t s_rate[kMaxModels], s_slots[kMaxModels], s_kvcap[kMaxModels], s_prefill[kMaxModels];
-    __shared__ uint32_t s_base2[kMaxModels], s_thr2[kMaxModels], s_sbase[kMaxModels + 1];
+    __shared__ uint32_t s_sbase[kMaxModels + 1];
     __shared__ float s_kvinv[kMaxModels];
     __shared__ uint8_t s_gmodel[128];                                       // group of 8 slots -> model
     const uint32_t lane = threadIdx.x & 31u, wib = threadIdx.x >> 5;
@@ -80,15 +129,12 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         const ModelTab m = P.model[threadIdx.x];
         s_rate[threadIdx.x] = m.rate; s_slots[threadIdx.x] = m.slots; s_kvcap[threadIdx.x] = m.kv_cap; s_prefill[threadIdx.x] = m.prefill;
         s_kvinv[threadIdx.x] = m.kv_inv;
-        const uint32_t x = m.rate * kDtUs;                                  // rate <= 80000 => fits 32 bits
-        s_base2[threadIdx.x] = (x / 1000000u) * 0x00010001u;
-        s_thr2[threadIdx.x] = (uint32_t)(((unsigned long long)(x % 1000000u) << 16) / 1000000u) * 0x00010001u;   // R11: Bernoulli to 2^-16
     }
     if (threadIdx.x <= kMaxModels) s_sbase[threadIdx.x] = P.slot_base[threadIdx.x];
-    if (threadIdx.x < P.n_grp) {
+    for (uint32_t g = threadIdx.x; g < P.n_grp; g += blockDim.x) {
         uint32_t k = 0;
-        while (P.slot_base[k + 1] <= threadIdx.x * 8) k++;
-        s_gmodel[threadIdx.x] = (uint8_t)k;
+        while (P.slot_base[k + 1] <= g * 8) k++;
+        s_gmodel[g] = (uint8_t)k;
     }
     if (lane == 0) bulk::mbar_init(&s_bar[wib], 1);
     bulk::fence_mbar_init();
@@ -107,8 +153,7 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
 
     unsigned char *sm = smem_raw + (size_t)wib * L.per_warp;
     uint32_t *s_hdr = reinterpret_cast<uint32_t *>(sm) + lane;                          // word w at s_hdr[w * 32]
-    uint32_t *s_cm = reinterpret_cast<uint32_t *>(sm + L.o_cm) + lane;
-    uint32_t *s_kv = reinterpret_cast<uint32_t *>(sm + L.o_kv) + lane;
+    uint32_t *s_cm = reinterpret_cast<uint32_t *>(sm + L.o_cm) + lane;                  // completion bytes of the tick (k_serve)
 #define H(w) s_hdr[(w) * 32u]
 #define M_W0(k) s_hdr[(3u * (k)) * 32u]            /* n_wait | n_run << 16 */
 #define M_KV(k) s_hdr[(3u * (k) + 1u) * 32u]
@@ -116,16 +161,18 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
 #define OCC_LO(k) s_hdr[(P.hw_occ + 2u * (k)) * 32u]
 #define OCC_HI(k) s_hdr[(P.hw_occ + 2u * (k) + 1u) * 32u]
 #define QFREE(w) s_hdr[(P.hw_qfree + (w)) * 32u]
+#define META(w) s_hdr[(P.hw_meta + (w)) * 32u]      /* owner nibbles of 8 chunks */
+#define USED(w) s_hdr[(P.hw_used + (w)) * 32u]
+#define TAILW(k) s_hdr[(P.hw_tail + ((k) >> 2)) * 32u]
 
     uint8_t *blkp = P.env_base + (size_t)blk * P.blk_stride;
-    if (lane == 0) {
-        bulk::mbar_expect_tx(&s_bar[wib], L.hdr_bytes);
-        bulk::g2s(sm, blkp, L.hdr_bytes, &s_bar[wib]);
+    if (lane == 0) {                                             // header + completion bytes: contiguous in the block
+        bulk::mbar_expect_tx(&s_bar[wib], L.per_warp);
+        bulk::g2s(sm, blkp, L.per_warp, &s_bar[wib]);
     }
     uint4 *hot4 = reinterpret_cast<uint4 *>(blkp + P.off_hot) + lane;                   // group g at hot4[g * 32]
     uint16_t *hot16 = reinterpret_cast<uint16_t *>(blkp + P.off_hot) + lane * 8u;       // slot gs at hot16[(gs >> 3) * 256 + (gs & 7)]
-    uint32_t *wkey = reinterpret_cast<uint32_t *>(blkp + P.off_wkey) + lane * 4u;       // key j at wkey[(j >> 2) * 128 + (j & 3)]
-    const uint4 *wkey4 = reinterpret_cast<const uint4 *>(blkp + P.off_wkey) + lane;     // unit u at wkey4[u * 32]
+    uint32_t *wkey = reinterpret_cast<uint32_t *>(blkp + P.off_wkey + (size_t)lane * P.wkey_stride);   // entry i of chunk c at [c * 16 + i]
     uint4 *cold = reinterpret_cast<uint4 *>(blkp + P.off_cold + (size_t)lane * P.cold_stride);
     uint2 *waux = reinterpret_cast<uint2 *>(blkp + P.off_waux + (size_t)lane * P.waux_stride);
     uint4 *qtab = reinterpret_cast<uint4 *>(blkp + P.off_q + (size_t)lane * P.q_stride);
@@ -147,25 +194,76 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         if (idx0 >= P.exec.regcap) idx0 -= P.exec.regcap;
         return true;
     };
-    // waiting list: append one entry at position nw (the rest of a freshly started unit gets the 0xFFFFFFFF filler)
-    uint32_t nw = 0;
-    auto list_append = [&](uint32_t key, uint2 aux) {
-        uint32_t *dst = wkey + (nw >> 2) * 128u + (nw & 3u);
-        if ((nw & 3u) == 0) *reinterpret_cast<uint4 *>(dst) = make_uint4(key, ~0u, ~0u, ~0u);
-        else *dst = key;
-        waux[nw] = aux;
-        nw++;
-    };
-    // remove entry j: the last entry fills the hole
-    auto list_remove = [&](uint32_t j) {
-        const uint32_t last = nw - 1u;
-        uint32_t *lp = wkey + (last >> 2) * 128u + (last & 3u);
-        if (j != last) {
-            wkey[(j >> 2) * 128u + (j & 3u)] = *lp;
-            waux[j] = waux[last];
+    // ---- waiting lists: one unordered list per model, built from 16-entry chunks of a per-env pool (im_device.cuh).
+    // insert: into the model's tail chunk (the one with room), else into a fresh chunk (lowest free one)
+    auto list_insert = [&](uint32_t k, uint32_t key, uint2 aux) {
+        const uint32_t w0 = M_W0(k), sh = 8u * (k & 3u);
+        uint32_t tw = TAILW(k), c = (tw >> sh) & 0xFFu, pos;
+        if (c == 0xFFu) {
+            uint32_t w = 0;
+            while (USED(w) == 0xFFFFFFFFu) w++;                  // the pool always has a free chunk here (rcap >= 3 qcap, R9)
+            const uint32_t bit = (uint32_t)__ffs(~USED(w)) - 1u;
+            USED(w) |= 1u << bit;
+            c = w * 32u + bit;
+            const uint32_t mw = META(c >> 3), msh = 4u * (c & 7u);
+            META(c >> 3) = (mw & ~(0xFu << msh)) | (k << msh);
+            uint4 *ck = reinterpret_cast<uint4 *>(wkey + c * 16u);
+            ck[0] = make_uint4(key, ~0u, ~0u, ~0u);
+            ck[1] = ck[2] = ck[3] = make_uint4(~0u, ~0u, ~0u, ~0u);
+            pos = 0;
+        } else {
+            pos = w0 & 15u;                                      // every other chunk of the model is full
+            wkey[c * 16u + pos] = key;
         }
-        *lp = ~0u;
-        nw = last;
+        waux[c * 16u + pos] = aux;
+        TAILW(k) = (tw & ~(0xFFu << sh)) | ((pos == 15u ? 0xFFu : c) << sh);
+        M_W0(k) = w0 + 1u;
+    };
+    // smallest key of model k: chunk and position; `lastc` = some chunk of the model (the tail to be, if all are full)
+    uint32_t meta_words = 0;
+    auto list_min = [&](uint32_t k, uint32_t &bkey, uint32_t &bc, uint32_t &bp, uint32_t &lastc) {
+        bkey = ~0u; bc = 0; bp = 0; lastc = 0;
+#pragma unroll 1
+        for (uint32_t w = 0; w < meta_words; w++) {
+            const uint32_t x = META(w) ^ (k * 0x11111111u);
+            uint32_t z = ~(((x & 0x77777777u) + 0x77777777u) | x) & 0x88888888u;     // nibbles equal to k
+#pragma unroll 1
+            while (z) {
+                const uint32_t c = w * 8u + (((uint32_t)__ffs(z) - 1u) >> 2);
+                z &= z - 1u;
+                if (!((USED(c >> 5) >> (c & 31u)) & 1u)) continue;                  // a stale nibble of a free chunk
+                lastc = c;
+                const uint4 *ck = reinterpret_cast<const uint4 *>(wkey + c * 16u);
+                const uint4 a = ck[0], b = ck[1], cc = ck[2], d = ck[3];
+                const uint32_t m = min(min(min(a.x, a.y), min(a.z, a.w)), min(min(b.x, b.y), min(b.z, b.w)));
+                const uint32_t n = min(min(min(cc.x, cc.y), min(cc.z, cc.w)), min(min(d.x, d.y), min(d.z, d.w)));
+                const uint32_t mn = min(m, n);
+                if (mn < bkey) {
+                    bkey = mn; bc = c;
+                    const uint32_t kk[16] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w, d.x, d.y, d.z, d.w};
+                    uint32_t eq = 0;
+#pragma unroll
+                    for (int i = 0; i < 16; i++) eq |= (kk[i] == mn ? 1u : 0u) << i;
+                    bp = (uint32_t)__ffs(eq) - 1u;                                  // keys are unique
+                }
+            }
+        }
+    };
+    // remove entry (c, p) of model k: the last entry of the model's tail chunk fills the hole
+    auto list_remove = [&](uint32_t k, uint32_t c, uint32_t p, uint32_t lastc) {
+        const uint32_t w0 = M_W0(k), n = w0 & 0xFFFFu, sh = 8u * (k & 3u);
+        const uint32_t tw = TAILW(k);
+        uint32_t tc = (tw >> sh) & 0xFFu;
+        if (tc == 0xFFu) tc = lastc;                             // all chunks full: any of them becomes the tail
+        const uint32_t lp = (n - 1u) & 15u;
+        if (tc != c || lp != p) {
+            wkey[c * 16u + p] = wkey[tc * 16u + lp];
+            waux[c * 16u + p] = waux[tc * 16u + lp];
+        }
+        wkey[tc * 16u + lp] = ~0u;
+        if (lp == 0) { USED(tc >> 5) &= ~(1u << (tc & 31u)); tc = 0xFFu; }           // the tail chunk is empty: back to the pool
+        TAILW(k) = (tw & ~(0xFFu << sh)) | (tc << sh);
+        M_W0(k) = w0 - 1u;
     };
 
     if (t_post >= 0) {
@@ -174,62 +272,32 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         const bool emit = (pre_mode == 1) && !done;
         const uint32_t t_rel_next = (uint32_t)(t + 1 - t0);
 
-        // =============================================================== F serve (R11): one streaming pass over the slots.
-        // It needs nothing from the header (a free slot holds 0), so it runs while the header block is in flight.
-        // The requests admitted in THIS tick are served in phase E below (prefill, R11): they are not in `hot` yet.
+        // F serve ran in k_serve: its tokens per model are fetched now and used after the admission phase
+        uint32_t kvt[kMaxModels];
         {
-            const uint32_t n_grp = P.n_grp;
-            uint32_t kprev = 0, tot = 0, cword = 0;
-            uint4 nxt = hot4[0];
-#pragma unroll 1
-            for (uint32_t g = 0; g < n_grp; g++) {
-                const uint4 h = nxt;
-                if (g + 1 < n_grp) nxt = hot4[(g + 1) * 32u];
-                const uint32_t k = s_gmodel[g];                                  // uniform across the warp
-                if (k != kprev) { s_kv[kprev * 32u] = tot; tot = 0; kprev = k; }
-                const bool any = (h.x | h.y | h.z | h.w) != 0;
-                uint32_t cacc = 0;
-                if (__any_sync(kFull, any)) {
-                    const Ph4 u = philox4x32_10_rk(gid, (uint32_t)t, g, 0u, P.svc_rk);
-                    const uint32_t base2 = s_base2[k], thr2 = s_thr2[k];
-                    uint32_t totp = 0;
-                    uint4 r;
-                    r.x = serve_pair(h.x, u.x, base2, thr2, 0, totp, cacc);
-                    r.y = serve_pair(h.y, u.y, base2, thr2, 1, totp, cacc);
-                    r.z = serve_pair(h.z, u.z, base2, thr2, 2, totp, cacc);
-                    r.w = serve_pair(h.w, u.w, base2, thr2, 3, totp, cacc);
-                    tot += (totp & 0xFFFFu) + (totp >> 16);
-                    if (any) hot4[g * 32u] = r;
-                }
-                // completion byte of the group: bits 0-3 = slots 0, 2, 4, 6; bits 4-7 = slots 1, 3, 5, 7
-                cword |= ((cacc & 0xFu) | ((cacc >> 12) & 0xF0u)) << (8u * (g & 3u));
-                if ((g & 3u) == 3u || g + 1 == n_grp) { s_cm[(g >> 2) * 32u] = cword; cword = 0; }
-            }
-            s_kv[kprev * 32u] = tot;
+            const uint32_t *kvs = reinterpret_cast<const uint32_t *>(blkp + P.off_kvt) + lane;
+#pragma unroll
+            for (uint32_t k = 0; k < kMaxModels; k++) kvt[k] = k < N ? kvs[k * 32u] : 0u;
         }
         bulk::mbar_wait(&s_bar[wib], 0);
 
         // =============================================================== D-issue (R18): the new calls join the waiting list
-        const uint32_t misc0 = H(P.hw_misc);
-        nw = misc0 & 0xFFFFu;
-        const uint32_t drops_in = misc0 >> 16;                   // R9: drops of this tick's phase A
+        const uint32_t drops_in = H(P.hw_misc);                  // R9: drops of this tick's phase A
         {
             uint32_t icnt = H(P.hw_misc + 1u);
             if (icnt > kIssueCap) icnt = kIssueCap;              // the executor kernel flags the overflow (err_flag)
-            if (nw + icnt > P.RCAP) { atomicOr(P.err_flag, 8u); icnt = 0; }      // cannot happen: rcap >= 3 qcap (R9)
             const uint2 *iss = reinterpret_cast<const uint2 *>(blkp + P.off_iss) + lane;
 #pragma unroll 1
             for (uint32_t j = 0; j < icnt; j++) {
                 const uint2 r = iss[j * 32u];
-                list_append(r.x, make_uint2(((uint32_t)t & 0xFFFFu) | ((r.y & SW_TOK_MASK) << 16), r.y));   // issue = t, remaining = out_total
-                M_W0(r.x >> 28) += 1u;
+                list_insert(r.x >> 28, r.x, make_uint2(((uint32_t)t & 0xFFFFu) | ((r.y & SW_TOK_MASK) << 16), r.y));   // issue = t, remaining = out_total
             }
             c_issued += icnt;
         }
 
         // =============================================================== E admit (R20, R21): smallest key first, per model.
-        // Judged on the state before this tick's service (admission precedes service); the tokens the admitted requests
-        // decode in their first tick join the service totals in s_kv.
+        // Judged on the state before this tick's service (admission precedes service): the tokens the admitted requests
+        // decode in their first tick are added when the lane is done with the model, the tokens of k_serve after the phase.
         {
             uint32_t madm = 0;
 #pragma unroll 1
@@ -237,79 +305,66 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 const uint32_t w0 = M_W0(k);
                 if ((w0 & 0xFFFFu) > 0 && (w0 >> 16) < s_slots[k] && M_KV(k) <= s_kvcap[k]) madm |= 1u << k;
             }
-            // one admission attempt of model k whose smallest key sits at list index j; returns true when k may admit again
-            auto attempt = [&](uint32_t k, uint32_t key, uint32_t j, uint32_t &removed) -> bool {
-                const uint2 wa = waux[j];
-                const uint32_t sw = wa.y, rem0 = wa.x >> 16, id = key & 0xFFFu;
-                const uint32_t need = ((sw >> SW_IN_SHIFT) & SW_TOK_MASK) + ((sw & SW_TOK_MASK) - rem0);     // R12
-                const uint32_t w0 = M_W0(k), nr = w0 >> 16, kv = M_KV(k), slots = s_slots[k];
-                if (!(nr < slots && kv + need <= s_kvcap[k])) return false;                    // stop at the first misfit (R21)
-                uint32_t olo = OCC_LO(k), ohi = OCC_HI(k);
-                const uint32_t sl = ~olo ? (uint32_t)__ffs(~olo) - 1u : 31u + (uint32_t)__ffs(~ohi);   // lowest free slot (R10)
-                if (sl < 32) OCC_LO(k) = olo | (1u << sl); else OCC_HI(k) = ohi | (1u << (sl - 32));
-                const uint32_t gs = s_sbase[k] + sl;
-                const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
-                // prefill, then its first tick of service (R11)
-                const uint32_t pf = (uint32_t)(((unsigned long long)s_prefill[k] * need) / 1000u);
-                const uint32_t usable = kDtUs - min(pf, kDtUs);
-                const uint32_t x = s_rate[k] * usable;
-                const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
-                const uint32_t thr = (uint32_t)(((unsigned long long)fr << 16) / 1000000u);
-                const uint32_t u16 = u16_field(philox4x32_10_rk(gid, (uint32_t)t, gs >> 3, 0u, P.svc_rk), gs & 7u);
-                const uint32_t tok = min(bs + (u16 < thr ? 1u : 0u), rem0);
-                const uint32_t rem = rem0 - tok;
-                hot16[(gs >> 3) * 256u + (gs & 7u)] = (uint16_t)rem;
-                cold[gs] = make_uint4((wa.x & 0xFFFFu) | (dl << 16), sw, id, 0u);
-                if (rem == 0) {
-                    const uint32_t g = gs >> 3;
-                    s_cm[(g >> 2) * 32u] |= 1u << (8u * (g & 3u) + ((gs & 7u) >> 1) + 4u * (gs & 1u));
+            // chunks in use end at the highest set bit of the used bitmap (chunks that do not exist are marked used: skip them)
+            {
+                const uint32_t real_chunks = P.RCAP / 16u + N;
+                uint32_t hi = 0;
+#pragma unroll 1
+                for (uint32_t w = 0; w < P.n_chunks / 32u; w++) {
+                    uint32_t u = USED(w);
+                    const uint32_t c0 = w * 32u;
+                    if (c0 + 32u > real_chunks) u &= c0 >= real_chunks ? 0u : ((1u << (real_chunks - c0)) - 1u);
+                    if (u) hi = c0 + 32u - (uint32_t)__clz(u);
                 }
-                M_W0(k) = w0 - 1u + 0x10000u;                     // n_wait--, n_run++
-                M_KV(k) = kv + need;
-                s_kv[k * 32u] += tok;
-                removed = j;
-                return (w0 & 0xFFFFu) > 1u && nr + 1u < slots;
-            };
+                meta_words = (hi + 7u) >> 3;
+            }
+            uint32_t tokacc = 0;
 #pragma unroll 1
             while (__any_sync(kFull, madm != 0)) {
                 if (madm) {
-                    // per-model minimum of the waiting keys and its list index, two admitting models per pass over the
-                    // list.  The keys of model k are those in [k<<28, (k+1)<<28): for them, and only for them,
-                    // key - (k<<28) is below 2^28 - 1 in unsigned arithmetic (the filler 0xFFFFFFFF never is).
-                    const uint32_t k0 = __ffs(madm) - 1u, rest = madm & (madm - 1u);
-                    const uint32_t k1 = rest ? __ffs(rest) - 1u : k0;
-                    const uint32_t b0 = k0 << 28, b1 = k1 << 28;
-                    uint32_t d0 = 0x0FFFFFFFu, d1 = 0x0FFFFFFFu, i0 = 0, i1 = 0;
-                    const uint32_t n4 = (nw + 3u) >> 2;
-#pragma unroll 1
-                    for (uint32_t u0 = 0; u0 < n4; u0 += 2) {
-                        const uint4 ka = wkey4[u0 * 32u];
-                        uint4 kb = make_uint4(~0u, ~0u, ~0u, ~0u);
-                        if (u0 + 1 < n4) kb = wkey4[(u0 + 1) * 32u];
-                        const uint32_t kk[8] = {ka.x, ka.y, ka.z, ka.w, kb.x, kb.y, kb.z, kb.w};
-#pragma unroll
-                        for (int i = 0; i < 8; i++) {
-                            const uint32_t da = kk[i] - b0, db = kk[i] - b1;
-                            if (da < d0) { d0 = da; i0 = u0 * 4u + i; }
-                            if (db < d1) { d1 = db; i1 = u0 * 4u + i; }
+                    const uint32_t k = (uint32_t)__ffs(madm) - 1u;
+                    uint32_t key, c, p, lastc;
+                    list_min(k, key, c, p, lastc);
+                    bool again = false;
+                    if (key != ~0u) {
+                        const uint2 wa = waux[c * 16u + p];
+                        const uint32_t sw = wa.y, rem0 = wa.x >> 16, id = key & 0xFFFu;
+                        const uint32_t need = ((sw >> SW_IN_SHIFT) & SW_TOK_MASK) + ((sw & SW_TOK_MASK) - rem0);     // R12
+                        const uint32_t w0 = M_W0(k), nr = w0 >> 16, kv = M_KV(k), slots = s_slots[k];
+                        if (nr < slots && kv + need <= s_kvcap[k]) {                          // else: stop at the first misfit (R21)
+                            const uint32_t olo = OCC_LO(k), ohi = OCC_HI(k);
+                            const uint32_t sl = ~olo ? (uint32_t)__ffs(~olo) - 1u : 31u + (uint32_t)__ffs(~ohi);   // lowest free slot (R10)
+                            if (sl < 32) OCC_LO(k) = olo | (1u << sl); else OCC_HI(k) = ohi | (1u << (sl - 32));
+                            const uint32_t gs = s_sbase[k] + sl;
+                            const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
+                            // prefill, then its first tick of service (R11)
+                            const uint32_t pf = (uint32_t)(((unsigned long long)s_prefill[k] * need) / 1000u);
+                            const uint32_t usable = kDtUs - min(pf, kDtUs);
+                            const uint32_t x = s_rate[k] * usable;
+                            const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
+                            const uint32_t thr = (uint32_t)(((unsigned long long)fr << 16) / 1000000u);
+                            const uint32_t u16 = u16_field(philox4x32_10_rk(gid, (uint32_t)t, gs >> 3, 0u, P.svc_rk), gs & 7u);
+                            const uint32_t tok = min(bs + (u16 < thr ? 1u : 0u), rem0);
+                            const uint32_t rem = rem0 - tok;
+                            hot16[(gs >> 3) * 256u + (gs & 7u)] = (uint16_t)rem;
+                            cold[gs] = make_uint4((wa.x & 0xFFFFu) | (dl << 16), sw, id, 0u);
+                            if (rem == 0) {
+                                const uint32_t g = gs >> 3;
+                                s_cm[(g >> 2) * 32u] |= 1u << (8u * (g & 3u) + ((gs & 7u) >> 1) + 4u * (gs & 1u));
+                            }
+                            M_W0(k) = w0 + 0x10000u;                  // n_run++ (list_remove takes the request off n_wait)
+                            M_KV(k) = kv + need;
+                            tokacc += tok;
+                            list_remove(k, c, p, lastc);
+                            again = (w0 & 0xFFFFu) > 1u && nr + 1u < slots;
                         }
                     }
-                    uint32_t r0 = ~0u, r1 = ~0u;
-                    bool again0 = false, again1 = false;
-                    if (d0 != 0x0FFFFFFFu) again0 = attempt(k0, b0 + d0, i0, r0);
-                    if (k1 != k0 && d1 != 0x0FFFFFFFu) again1 = attempt(k1, b1 + d1, i1, r1);
-                    // remove the admitted entries, larger index first (the entry that fills a hole comes from the tail)
-                    if (r0 != ~0u && r1 != ~0u) { const uint32_t hi = max(r0, r1), lo = min(r0, r1); list_remove(hi); list_remove(lo); }
-                    else if (r0 != ~0u) list_remove(r0);
-                    else if (r1 != ~0u) list_remove(r1);
-                    madm &= ~((1u << k0) | (1u << k1));
-                    if (again0) madm |= 1u << k0;
-                    if (again1) madm |= 1u << k1;
+                    if (!again) { madm &= madm - 1u; M_KV(k) += tokacc; tokacc = 0; }
                 }
             }
-            // service totals of the tick: requests RUNNING before this tick + first tick of the admitted ones
-#pragma unroll 1
-            for (uint32_t k = 0; k < N; k++) M_KV(k) += s_kv[k * 32u];
+            // service totals of the requests that were RUNNING before this tick
+#pragma unroll
+            for (uint32_t k = 0; k < kMaxModels; k++) if (k < N) M_KV(k) += kvt[k];
         }
 
         // =============================================================== G complete (R1, R13, R27, R28): completion bits in
@@ -426,13 +481,13 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                     const uint32_t rem = *hp;
                     *hp = 0;                                                            // a free slot holds 0
                     const uint32_t tm = P.sched_mode ? (bcd.x >> 16) : (bcd.x & 0xFFFFu);
-                    list_append((k << 28) | (tm << 12) | bcd.z, make_uint2((bcd.x & 0xFFFFu) | (rem << 16), bcd.y));   // keeps progress and issue tick
+                    list_insert(k, (k << 28) | (tm << 12) | bcd.z, make_uint2((bcd.x & 0xFFFFu) | (rem << 16), bcd.y));   // keeps progress and issue tick; n_wait++
                     if (bsl < 32) olo &= ~(1u << bsl); else ohi &= ~(1u << (bsl - 32));
                     kv -= ((bcd.y >> SW_IN_SHIFT) & SW_TOK_MASK) + ((bcd.y & SW_TOK_MASK) - rem);
                     npre++;
                 }
                 M_KV(k) = kv; OCC_LO(k) = olo; OCC_HI(k) = ohi;
-                M_W0(k) += npre - (npre << 16);                                          // n_wait += npre, n_run -= npre
+                M_W0(k) -= npre << 16;                                                   // n_run -= npre
                 c_preempt += npre;
             }
         }
@@ -460,12 +515,19 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 for (uint32_t w = 0; w < P.hw_qfree; w++) H(w) = 0;                        // m and occ
 #pragma unroll 1
                 for (uint32_t g = 0; g < P.n_grp; g++) hot4[g * 32u] = make_uint4(0, 0, 0, 0);
-                nw = 0;
+                // the waiting lists: every chunk back to the pool (chunks that do not exist stay marked used)
+                const uint32_t real_chunks = P.RCAP / 16u + N;
+#pragma unroll 1
+                for (uint32_t w = 0; w < P.n_chunks / 32u; w++) {
+                    const uint32_t c0 = w * 32u;
+                    USED(w) = c0 >= real_chunks ? 0xFFFFFFFFu : (real_chunks - c0 >= 32u ? 0u : ~((1u << (real_chunks - c0)) - 1u));
+                }
+#pragma unroll 1
+                for (uint32_t w = 0; w < 4; w++) H(P.hw_tail + w) = 0xFFFFFFFFu;
             }
         }
     } else {
         bulk::mbar_wait(&s_bar[wib], 0);
-        nw = H(P.hw_misc) & 0xFFFFu;
     }
 
     // ===================================================================== pre(t_pre): A arrive, B snapshot, work lists
@@ -567,16 +629,16 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
             sn[2 * N + k] = __fmul_rn(__uint2float_rn(M_KV(k)), s_kvinv[k]);
         }
     }
-    // ---- counters: only the rows some env of the block changed
+    // ---- counters
     {
         const uint32_t cv[C_N] = {c_arr, c_drop, c_fin, c_solved, c_missed, c_issued, c_done, c_preempt, c_soj, c_live, c_plans,
                                   c_issued, c_run, c_wait, 0u, c_aband};
 #pragma unroll
         for (int c = 0; c < (int)C_N; c++)
-            if (__any_sync(kFull, cv[c] != 0)) ctr[c * 32] += cv[c];
+            if (cv[c] != 0) atomicAdd(&ctr[c * 32], cv[c]);      // no return value: a fire-and-forget reduction, no round trip
     }
     // ---- header back to HBM: one bulk copy
-    H(P.hw_misc) = nw | (drops_out << 16);
+    H(P.hw_misc) = drops_out;
     H(P.hw_misc + 1u) = 0;
     bulk::fence_proxy_async();
     __syncwarp();
@@ -592,12 +654,21 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
 #undef OCC_LO
 #undef OCC_HI
 #undef QFREE
+#undef META
+#undef USED
+#undef TAILW
 }
 
 // opt-in to the dynamic shared memory the kernel needs on the CURRENT device (attributes are per device: im_bind calls this)
 int sim_prepare_device()
 {
     return cudaFuncSetAttribute(k_sim, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) == cudaSuccess ? 0 : -1;
+}
+
+void launch_serve(const Params &P, int32_t t, cudaStream_t st)
+{
+    const uint32_t warps = P.NB * P.N;
+    k_serve<<<(warps + kServeWarps - 1) / kServeWarps, kServeWarps * 32, 0, st>>>(P, t);
 }
 
 void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st)
