@@ -32,16 +32,15 @@ void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t
 __global__ void k_reset(const Params P)
 {
     const uint32_t words = P.off_iss / 4;                        // hdr | cm | kvt | ctr | hot
-    const uint32_t real_chunks = P.RCAP / 16 + P.N;
     const size_t n = (size_t)P.NB * words;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const uint32_t b = (uint32_t)(i / words), w = (uint32_t)(i % words), hw = w >> 5;
         uint32_t v = 0;
         if (hw >= P.hw_qfree && hw < P.hw_qfree + P.QW && b * 32u + (w & 31u) < P.E) v = 0xFFFFFFFFu;
-        if (hw >= P.hw_tail && hw < P.hw_tail + 4) v = 0xFFFFFFFFu;                       // no model has a tail chunk
-        if (hw >= P.hw_used && hw < P.hw_tail) {                                          // chunks that do not exist are "used"
-            const uint32_t c0 = (hw - P.hw_used) * 32u;
-            v = c0 >= real_chunks ? 0xFFFFFFFFu : (real_chunks - c0 >= 32u ? 0u : ~((1u << (real_chunks - c0)) - 1u));
+        if (hw >= P.hw_head && hw < P.hw_head + 4) v = 0xFFFFFFFFu;                       // every model's list is empty
+        if (hw >= P.hw_next && hw < P.hw_head) {                                          // all chunks on the free list: 0 -> 1 -> ... -> end
+            const uint32_t c0 = (hw - P.hw_next) * 4u;
+            for (uint32_t j = 0; j < 4; j++) v |= (c0 + j + 1u < P.n_chunks ? c0 + j + 1u : 0xFFu) << (8u * j);
         }
         reinterpret_cast<uint32_t *>(P.env_base + (size_t)b * P.blk_stride)[w] = v;
     }
@@ -273,9 +272,9 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     for (uint32_t k = 0; k < kMaxModels; k++) P.slot_base[k + 1] = P.slot_base[k] + (k < N ? ((s.model[k].slots + 7u) & ~7u) : 0u);
     P.SP = P.slot_base[N];
     P.n_grp = P.SP / 8; P.cm_words = (P.n_grp + 3u) / 4u;
-    P.n_chunks = (R / 16 + N + 31u) & ~31u;                    // usable: R / 16 + N (the rest is marked used by k_reset)
-    P.hw_occ = 3 * N; P.hw_qfree = P.hw_occ + 2 * N; P.hw_meta = P.hw_qfree + P.QW; P.hw_used = P.hw_meta + P.n_chunks / 8;
-    P.hw_tail = P.hw_used + P.n_chunks / 32; P.hw_misc = P.hw_tail + 4; P.hdr_words = P.hw_misc + 2;
+    P.n_chunks = R / kChunk + N;                               // <= 4096 / 32 + 16 = 144: chunk ids fit a byte
+    P.hw_occ = 3 * N; P.hw_qfree = P.hw_occ + (P.SP + 31u) / 32u + 2u; P.hw_next = P.hw_qfree + P.QW; P.hw_head = P.hw_next + (P.n_chunks + 3u) / 4u;
+    P.hw_used = P.hw_head + 4; P.hw_misc = P.hw_used + (P.n_chunks + 31u) / 32u; P.hdr_words = P.hw_misc + 2;
     auto up128 = [](uint32_t x) { return (x + 127u) & ~127u; };
     uint32_t off = P.hdr_words * 128u;
     P.off_cm = off; off += P.cm_words * 128u;                 // directly behind the header: one bulk copy brings both
@@ -284,7 +283,7 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     P.off_hot = off; off += P.n_grp * 512u;
     P.off_iss = off; off += kIssueCap * 256u;
     P.off_qready = off; off += P.QW * 128u;
-    P.cold_stride = up128(P.SP * 16u); P.wkey_stride = P.n_chunks * 64u; P.waux_stride = P.n_chunks * 128u; P.q_stride = Q * 16u;
+    P.cold_stride = up128(P.SP * 16u); P.wkey_stride = P.n_chunks * kChunk * 4u; P.waux_stride = P.n_chunks * kChunk * 8u; P.q_stride = Q * 16u;
     P.off_cold = off; off += 32u * P.cold_stride;
     P.off_wkey = off; off += 32u * P.wkey_stride;
     P.off_waux = off; off += 32u * P.waux_stride;
@@ -730,14 +729,14 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
                 };
                 for (uint32_t k = 0; k < N; k++)
                     for (uint32_t sl = 0; sl < c->spec.model[k].slots; sl++) {
-                        if (!((H(P.hw_occ + 2 * k + (sl >> 5)) >> (sl & 31)) & 1u)) continue;
                         const uint32_t gs = P.slot_base[k] + sl;
+                        if (!((H(P.hw_occ + (gs >> 5)) >> (gs & 31)) & 1u)) continue;
                         const uint32_t rem = hot[((gs >> 3) * 32 + l) * 8 + (gs & 7)];
                         put(cold[gs].z & 0xFFFu, ST_RUN, k, cold[gs].y, cold[gs].x >> 16, cold[gs].x & 0xFFFFu, rem, sl + 1);
                     }
-                for (uint32_t ch = 0; ch < P.RCAP / 16 + P.N; ch++) {          // waiting lists: the chunks in use
+                for (uint32_t ch = 0; ch < P.n_chunks; ch++) {                // waiting lists: the chunks in use
                     if (!((H(P.hw_used + (ch >> 5)) >> (ch & 31)) & 1u)) continue;
-                    for (uint32_t j = ch * 16; j < ch * 16 + 16; j++) {
+                    for (uint32_t j = ch * kChunk; j < (ch + 1) * kChunk; j++) {
                         const uint32_t key = wkey[j];
                         if (key == 0xFFFFFFFFu) continue;
                         const uint32_t id = key & 0xFFFu, tm = (key >> 12) & 0xFFFFu;

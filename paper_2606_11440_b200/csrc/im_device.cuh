@@ -12,9 +12,10 @@
 // word index) with ONE bulk copy (cp.async.bulk) per block.  The last four parts are per-env arrays (lane l at
 // part + l * stride): they are touched only at data-dependent positions by the few requests that change state.
 //   hdr   u32 units (hdr_words): m[3k] = n_wait | n_run << 16, m[3k+1] = kv_used, m[3k+2] = ewma_q8 |
-//         occ[2k], occ[2k+1] (bit s = slot s of model k taken) | qfree[QW] | the chunk directory of the waiting
-//         lists: owner nibbles (8 chunks per word) | used bitmap | tail chunk of every model (4 bytes per word,
-//         0xFF = none) | misc0 = drops | misc1 = icnt
+//         occ (bit gs = global slot gs taken; SP bits + two padding words) | qfree[QW] | the chunk directory of the waiting
+//         lists: next[c] (one byte per chunk, 0xFF = end: every model's chunks and the free chunks are linked lists) |
+//         head[k] (one byte per model, 0xFF = empty) | used bitmap (telemetry) | misc0 = drops | free head << 16 |
+//         misc1 = icnt
 //   cm    u32 units (cm_words): completion bytes of the tick's service pass, one per slot group (k_serve -> k_sim)
 //   kvt   u32 units (N): tokens decoded per model by the tick's service pass (k_serve -> k_sim)
 //   ctr   u32 units (16): the counters of enum Counter (absolute ticks < 65536 keep every sum below 2^32)
@@ -24,8 +25,8 @@
 //   iss   uint2 units (kIssueCap): {key, static word} written by the executor kernel for this tick (phase D)
 //   qready u32 units (QW): queries whose next stage is due, kept only ACROSS im_rollout calls
 //   cold[gs] uint4 = {issue(16) | deadline<<16, sw, id, 0}    sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
-//   wkey[c][16], waux[c][16]: the waiting lists, ONE UNORDERED LIST PER MODEL built from chunks of 16 entries out of a
-//         pool of n_chunks = RCAP/16 + N per env (a model has at most one partly filled chunk, its tail, so the pool
+//   wkey[c][32], waux[c][32]: the waiting lists, ONE UNORDERED LIST PER MODEL built from chunks of 32 entries out of a
+//         pool of n_chunks = RCAP/32 + N per env (only the head chunk of a model is partly filled, so the pool
 //         always suffices): admission only reads the chunks of the model that admits.  key = model<<28 |
 //         time(16)<<12 | id, time = deadline (EDF) or issue tick (FCFS): one u32 compare is the R20 order; id =
 //         4*query + agent; an empty entry of a chunk in use holds 0xFFFFFFFF (never a valid key).
@@ -43,6 +44,7 @@ namespace im {
 constexpr uint32_t kMaxModels = 16;
 constexpr uint32_t kRegions = 64;        // row-list / log regions (one atomic counter each), region = (env / 32) % n_regions
 constexpr uint32_t kDtUs = 50000;
+constexpr uint32_t kChunk = 32;          // entries per waiting-list chunk
 constexpr uint32_t kIssueCap = 128;      // issue records per env per tick (31 arrivals x 3 calls + continuing stages)
 
 constexpr uint32_t ST_FREE = 0, ST_WAIT = 1, ST_RUN = 2;
@@ -97,11 +99,11 @@ struct Params {
     // env state: one record per block of 32 envs (layout at the top of this file)
     uint8_t *env_base;
     unsigned long long blk_stride;           // bytes, multiple of 128
-    uint32_t hw_occ, hw_qfree, hw_meta, hw_used, hw_tail, hw_misc, hdr_words;   // header word indices (m at word 0)
+    uint32_t hw_occ, hw_qfree, hw_next, hw_head, hw_used, hw_misc, hdr_words;   // header word indices (m at word 0)
     uint32_t off_cm, off_kvt, off_ctr, off_hot, off_iss, off_qready;      // SoA-32 parts: byte offsets inside the block (hdr at 0)
     uint32_t off_cold, off_wkey, off_waux, off_q, cold_stride, wkey_stride, waux_stride, q_stride;   // per-env parts: lane 0 and lane stride
     uint32_t n_grp, cm_words;                // SP / 8 slot groups; completion-mask words per env = ceil(n_grp / 4)
-    uint32_t n_chunks;                       // waiting-list chunks per env (multiple of 32 for the bitmap; those beyond RCAP/16 + N are marked used)
+    uint32_t n_chunks;                       // waiting-list chunks per env: RCAP / 32 + N (< 255: chunk ids are bytes)
     float *snap;                             // [E][3N] telemetry features of the current tick (R14)
     const uint32_t *tab_mult, *tab_intok, *tab_cdf;
     const uint8_t *env_level;

@@ -132,7 +132,7 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const uint32_t e = blockIdx.x * kQoWarps + wib;
     if (e >= P.E) return;
-    const uint32_t n_ent = P.n_chunks * 16u;
+    const uint32_t n_ent = P.n_chunks * kChunk;
     uint32_t n2cap = 32;
     while (n2cap < n_ent) n2cap <<= 1;
     uint32_t *keys = s_keys + (size_t)wib * n2cap;
@@ -143,8 +143,8 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
     n = min(n, P.RCAP);
     const uint32_t n2 = n2cap;
     for (uint32_t i = lane; i < n2; i += 32) {
-        const uint32_t ch = i >> 4;
-        const bool used = i < n_ent && ((*hdr_word(P, e, P.hw_used + (ch >> 5)) >> (ch & 31u)) & 1u) && ch < P.RCAP / 16 + P.N;
+        const uint32_t ch = i / kChunk;
+        const bool used = i < n_ent && ((*hdr_word(P, e, P.hw_used + (ch >> 5)) >> (ch & 31u)) & 1u);
         keys[i] = used ? wkey[i] : 0xFFFFFFFFu;
     }
     __syncwarp();
@@ -185,7 +185,7 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st)
 {
     uint32_t n2cap = 32;
-    while (n2cap < P.n_chunks * 16u) n2cap <<= 1;
+    while (n2cap < P.n_chunks * kChunk) n2cap <<= 1;
     const size_t smem = (size_t)kQoWarps * n2cap * 4;
     cudaFuncSetAttribute(k_queue_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_queue_order<<<(P.E + kQoWarps - 1) / kQoWarps, kQoWarps * 32, smem, st>>>(P, t, out);

@@ -31,14 +31,17 @@ constexpr int kSimWarps = 2;            // 32-env blocks per CTA
 constexpr int kServeWarps = 8;
 constexpr uint32_t kFull = 0xffffffffu;
 
-// per-warp dynamic shared memory of k_sim: header [hdr_words][32] | completion masks [cm_words][32] (one bulk copy)
-struct SimSmem { uint32_t hdr_bytes, o_cm, per_warp; };
+// per-warp dynamic shared memory of k_sim: header [hdr_words][32] | completion masks [cm_words][32] (one bulk copy);
+// the snapshot is staged in [32][9] words: over the completion masks (done with by then) when they are large enough
+struct SimSmem { uint32_t hdr_bytes, o_cm, o_stage, tma_bytes, per_warp; };
 static SimSmem sim_smem(const Params &P)
 {
     SimSmem L;
     L.hdr_bytes = P.hdr_words * 128u;
     L.o_cm = L.hdr_bytes;
-    L.per_warp = L.o_cm + P.cm_words * 128u;
+    L.tma_bytes = L.o_cm + P.cm_words * 128u;
+    L.o_stage = P.cm_words >= 9u ? L.o_cm : L.tma_bytes;
+    L.per_warp = P.cm_words >= 9u ? L.tma_bytes : L.tma_bytes + 9u * 128u;
     return L;
 }
 
@@ -72,7 +75,7 @@ __device__ __forceinline__ uint32_t u16_field(const Ph4 &u, uint32_t f)
 // the model's parameters are uniform.  Results for k_sim: the tokens decoded per (env, model) and one completion byte
 // per (env, group) (bits 0-3 = slots 0, 2, 4, 6; bits 4-7 = slots 1, 3, 5, 7), both SoA-32 behind the header.
 // The requests admitted in THIS tick are served by k_sim's admission phase (prefill, R11): they are not in `hot` yet.
-__global__ void __launch_bounds__(kServeWarps * 32)
+__global__ void __launch_bounds__(kServeWarps * 32, 4)
 k_serve(const Params P, int32_t t)
 {
     const uint32_t lane = threadIdx.x & 31u;
@@ -90,7 +93,7 @@ k_serve(const Params P, int32_t t)
     uint4 h[8];
 #pragma unroll
     for (int i = 0; i < 8; i++) if ((uint32_t)i < ng) h[i] = hot4[(g0 + i) * 32u];
-    uint32_t tot = 0;
+    uint32_t tot = 0, cb_lo = 0, cb_hi = 0;                      // completion bytes of groups 0-3 / 4-7 of the model
 #pragma unroll
     for (int i = 0; i < 8; i++) {
         if ((uint32_t)i < ng) {
@@ -108,14 +111,32 @@ k_serve(const Params P, int32_t t)
                 tot += (totp & 0xFFFFu) + (totp >> 16);
                 if (any) hot4[g * 32u] = r;
             }
-            cmb[(g >> 2) * 128u + (g & 3u)] = (uint8_t)((cacc & 0xFu) | ((cacc >> 12) & 0xF0u));
+            const uint32_t c8 = (cacc & 0xFu) | ((cacc >> 12) & 0xF0u);
+            cmb[(g >> 2) * 128u + (g & 3u)] = (uint8_t)c8;
+            if (i < 4) cb_lo |= c8 << (8 * i); else cb_hi |= c8 << (8 * (i - 4));
         }
     }
     reinterpret_cast<uint32_t *>(blkp + P.off_kvt)[k * 32u + lane] = tot;
+    // Warm the L2 for k_sim's completion phase: the cold word of every completed slot and the table entry of its query
+    // (two dependent accesses at data-dependent addresses, cheap here where 32 warps per SM hide them)
+    const uint4 *cold = reinterpret_cast<const uint4 *>(blkp + P.off_cold + (size_t)lane * P.cold_stride);
+    const uint4 *qtab = reinterpret_cast<const uint4 *>(blkp + P.off_q + (size_t)lane * P.q_stride);
+#pragma unroll 1
+    for (uint32_t half = 0; half < 2; half++) {
+        uint32_t bits = half ? cb_hi : cb_lo;
+#pragma unroll 1
+        while (bits) {
+            const uint32_t b = (uint32_t)__ffs(bits) - 1u;
+            bits &= bits - 1u;
+            const uint32_t bb = b & 7u, gs = (g0 + half * 4u + (b >> 3)) * 8u + (((bb & 3u) << 1) | (bb >> 2));
+            const uint32_t id = cold[gs].z;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(qtab + (id >> 2)));
+        }
+    }
 }
 
 // tick arguments: t_post < 0 => no post phases; pre_mode 0 none, 1 full (A, B, rows), 2 snapshot only
-__global__ void __launch_bounds__(kSimWarps * 32, 5)
+__global__ void __launch_bounds__(kSimWarps * 32, 7)
 k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -158,17 +179,16 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
 #define M_W0(k) s_hdr[(3u * (k)) * 32u]            /* n_wait | n_run << 16 */
 #define M_KV(k) s_hdr[(3u * (k) + 1u) * 32u]
 #define M_EWMA(k) s_hdr[(3u * (k) + 2u) * 32u]
-#define OCC_LO(k) s_hdr[(P.hw_occ + 2u * (k)) * 32u]
-#define OCC_HI(k) s_hdr[(P.hw_occ + 2u * (k) + 1u) * 32u]
+#define OCC(w) s_hdr[(P.hw_occ + (w)) * 32u]       /* bit gs = global slot gs taken */
 #define QFREE(w) s_hdr[(P.hw_qfree + (w)) * 32u]
-#define META(w) s_hdr[(P.hw_meta + (w)) * 32u]      /* owner nibbles of 8 chunks */
+#define NEXTW(c) s_hdr[(P.hw_next + ((c) >> 2)) * 32u]    /* next[c]: byte c & 3 */
+#define HEADW(k) s_hdr[(P.hw_head + ((k) >> 2)) * 32u]    /* head[k]: byte k & 3 */
 #define USED(w) s_hdr[(P.hw_used + (w)) * 32u]
-#define TAILW(k) s_hdr[(P.hw_tail + ((k) >> 2)) * 32u]
 
     uint8_t *blkp = P.env_base + (size_t)blk * P.blk_stride;
     if (lane == 0) {                                             // header + completion bytes: contiguous in the block
-        bulk::mbar_expect_tx(&s_bar[wib], L.per_warp);
-        bulk::g2s(sm, blkp, L.per_warp, &s_bar[wib]);
+        bulk::mbar_expect_tx(&s_bar[wib], L.tma_bytes);
+        bulk::g2s(sm, blkp, L.tma_bytes, &s_bar[wib]);
     }
     uint4 *hot4 = reinterpret_cast<uint4 *>(blkp + P.off_hot) + lane;                   // group g at hot4[g * 32]
     uint16_t *hot16 = reinterpret_cast<uint16_t *>(blkp + P.off_hot) + lane * 8u;       // slot gs at hot16[(gs >> 3) * 256 + (gs & 7)]
@@ -194,75 +214,72 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         if (idx0 >= P.exec.regcap) idx0 -= P.exec.regcap;
         return true;
     };
-    // ---- waiting lists: one unordered list per model, built from 16-entry chunks of a per-env pool (im_device.cuh).
-    // insert: into the model's tail chunk (the one with room), else into a fresh chunk (lowest free one)
+    // the (<= 64) occupancy bits of the model whose slots start at global slot sb (a multiple of 8): bit s = slot s
+    auto occ_window = [&](uint32_t sb, uint32_t &olo, uint32_t &ohi) {
+        const uint32_t w = sb >> 5, sh = sb & 31u;
+        const uint32_t a = OCC(w), b = OCC(w + 1u), c = OCC(w + 2u);     // two padding words follow the bitmap
+        olo = __funnelshift_r(a, b, sh); ohi = __funnelshift_r(b, c, sh);
+    };
+    // ---- waiting lists: one unordered list per model, a linked list of 32-entry chunks of a per-env pool (im_device.cuh).
+    // Only the HEAD chunk of a model is partly filled: with n entries it holds ((n - 1) & 31) + 1 of them.
+    auto byte_get = [](uint32_t w, uint32_t i) { return (w >> (8u * (i & 3u))) & 0xFFu; };
+    auto byte_put = [](uint32_t w, uint32_t i, uint32_t v) { const uint32_t sh = 8u * (i & 3u); return (w & ~(0xFFu << sh)) | (v << sh); };
+    uint32_t free_head = 0xFFu;                                  // head of the free-chunk list (kept in misc0 between launches)
+    // insert: into the head chunk if it has room, else into a fresh chunk that becomes the head
     auto list_insert = [&](uint32_t k, uint32_t key, uint2 aux) {
-        const uint32_t w0 = M_W0(k), sh = 8u * (k & 3u);
-        uint32_t tw = TAILW(k), c = (tw >> sh) & 0xFFu, pos;
-        if (c == 0xFFu) {
-            uint32_t w = 0;
-            while (USED(w) == 0xFFFFFFFFu) w++;                  // the pool always has a free chunk here (rcap >= 3 qcap, R9)
-            const uint32_t bit = (uint32_t)__ffs(~USED(w)) - 1u;
-            USED(w) |= 1u << bit;
-            c = w * 32u + bit;
-            const uint32_t mw = META(c >> 3), msh = 4u * (c & 7u);
-            META(c >> 3) = (mw & ~(0xFu << msh)) | (k << msh);
-            uint4 *ck = reinterpret_cast<uint4 *>(wkey + c * 16u);
+        const uint32_t w0 = M_W0(k), n = w0 & 0xFFFFu;
+        uint32_t c = byte_get(HEADW(k), k), pos = n & (kChunk - 1u);
+        if (pos == 0) {                                          // empty list or full head chunk
+            const uint32_t nc = free_head;                       // the pool always has a free chunk here (rcap >= 3 qcap, R9)
+            free_head = byte_get(NEXTW(nc), nc);
+            NEXTW(nc) = byte_put(NEXTW(nc), nc, n ? c : 0xFFu);
+            HEADW(k) = byte_put(HEADW(k), k, nc);
+            USED(nc >> 5) |= 1u << (nc & 31u);
+            c = nc;
+            uint4 *ck = reinterpret_cast<uint4 *>(wkey + c * kChunk);
             ck[0] = make_uint4(key, ~0u, ~0u, ~0u);
-            ck[1] = ck[2] = ck[3] = make_uint4(~0u, ~0u, ~0u, ~0u);
-            pos = 0;
+#pragma unroll
+            for (int i = 1; i < (int)kChunk / 4; i++) ck[i] = make_uint4(~0u, ~0u, ~0u, ~0u);
         } else {
-            pos = w0 & 15u;                                      // every other chunk of the model is full
-            wkey[c * 16u + pos] = key;
+            wkey[c * kChunk + pos] = key;
         }
-        waux[c * 16u + pos] = aux;
-        TAILW(k) = (tw & ~(0xFFu << sh)) | ((pos == 15u ? 0xFFu : c) << sh);
+        waux[c * kChunk + pos] = aux;
         M_W0(k) = w0 + 1u;
     };
-    // smallest key of model k: chunk and position; `lastc` = some chunk of the model (the tail to be, if all are full)
-    uint32_t meta_words = 0;
-    auto list_min = [&](uint32_t k, uint32_t &bkey, uint32_t &bc, uint32_t &bp, uint32_t &lastc) {
-        bkey = ~0u; bc = 0; bp = 0; lastc = 0;
+    // smallest key of model k: walk its chunks (the lanes of a warp walk theirs in step, so their loads go out together);
+    // returns the key and the 4-entry unit that holds it
+    auto list_min = [&](uint32_t k, uint32_t &bkey, uint32_t &bunit) {
+        bkey = ~0u; bunit = 0;
+        uint32_t c = byte_get(HEADW(k), k);
 #pragma unroll 1
-        for (uint32_t w = 0; w < meta_words; w++) {
-            const uint32_t x = META(w) ^ (k * 0x11111111u);
-            uint32_t z = ~(((x & 0x77777777u) + 0x77777777u) | x) & 0x88888888u;     // nibbles equal to k
-#pragma unroll 1
-            while (z) {
-                const uint32_t c = w * 8u + (((uint32_t)__ffs(z) - 1u) >> 2);
-                z &= z - 1u;
-                if (!((USED(c >> 5) >> (c & 31u)) & 1u)) continue;                  // a stale nibble of a free chunk
-                lastc = c;
-                const uint4 *ck = reinterpret_cast<const uint4 *>(wkey + c * 16u);
-                const uint4 a = ck[0], b = ck[1], cc = ck[2], d = ck[3];
-                const uint32_t m = min(min(min(a.x, a.y), min(a.z, a.w)), min(min(b.x, b.y), min(b.z, b.w)));
-                const uint32_t n = min(min(min(cc.x, cc.y), min(cc.z, cc.w)), min(min(d.x, d.y), min(d.z, d.w)));
-                const uint32_t mn = min(m, n);
-                if (mn < bkey) {
-                    bkey = mn; bc = c;
-                    const uint32_t kk[16] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w, d.x, d.y, d.z, d.w};
-                    uint32_t eq = 0;
+        while (c != 0xFFu) {
+            const uint4 *ck = reinterpret_cast<const uint4 *>(wkey + c * kChunk);
+            uint4 v[kChunk / 4];
 #pragma unroll
-                    for (int i = 0; i < 16; i++) eq |= (kk[i] == mn ? 1u : 0u) << i;
-                    bp = (uint32_t)__ffs(eq) - 1u;                                  // keys are unique
-                }
+            for (int i = 0; i < (int)kChunk / 4; i++) v[i] = ck[i];
+            const uint32_t cn = byte_get(NEXTW(c), c);
+#pragma unroll
+            for (int i = 0; i < (int)kChunk / 4; i++) {
+                const uint32_t m = min(min(v[i].x, v[i].y), min(v[i].z, v[i].w));
+                if (m < bkey) { bkey = m; bunit = c * (kChunk / 4) + i; }
             }
+            c = cn;
         }
     };
-    // remove entry (c, p) of model k: the last entry of the model's tail chunk fills the hole
-    auto list_remove = [&](uint32_t k, uint32_t c, uint32_t p, uint32_t lastc) {
-        const uint32_t w0 = M_W0(k), n = w0 & 0xFFFFu, sh = 8u * (k & 3u);
-        const uint32_t tw = TAILW(k);
-        uint32_t tc = (tw >> sh) & 0xFFu;
-        if (tc == 0xFFu) tc = lastc;                             // all chunks full: any of them becomes the tail
-        const uint32_t lp = (n - 1u) & 15u;
-        if (tc != c || lp != p) {
-            wkey[c * 16u + p] = wkey[tc * 16u + lp];
-            waux[c * 16u + p] = waux[tc * 16u + lp];
+    // remove entry j (= chunk * 32 + position) of model k: the last entry of the head chunk fills the hole; `lk` / `la`
+    // are that entry's key and aux word, fetched by the caller ahead of time
+    auto list_remove = [&](uint32_t k, uint32_t j, uint32_t lk, uint2 la) {
+        const uint32_t w0 = M_W0(k), n = w0 & 0xFFFFu;
+        const uint32_t h = byte_get(HEADW(k), k), lp = (n - 1u) & (kChunk - 1u), lj = h * kChunk + lp;
+        if (lj != j) { wkey[j] = lk; waux[j] = la; }
+        wkey[lj] = ~0u;
+        if (lp == 0) {                                           // the head chunk is empty: back to the pool
+            const uint32_t nx = byte_get(NEXTW(h), h);
+            HEADW(k) = byte_put(HEADW(k), k, nx);
+            NEXTW(h) = byte_put(NEXTW(h), h, free_head);
+            free_head = h;
+            USED(h >> 5) &= ~(1u << (h & 31u));
         }
-        wkey[tc * 16u + lp] = ~0u;
-        if (lp == 0) { USED(tc >> 5) &= ~(1u << (tc & 31u)); tc = 0xFFu; }           // the tail chunk is empty: back to the pool
-        TAILW(k) = (tw & ~(0xFFu << sh)) | (tc << sh);
         M_W0(k) = w0 - 1u;
     };
 
@@ -282,15 +299,21 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         bulk::mbar_wait(&s_bar[wib], 0);
 
         // =============================================================== D-issue (R18): the new calls join the waiting list
-        const uint32_t drops_in = H(P.hw_misc);                  // R9: drops of this tick's phase A
+        const uint32_t drops_in = H(P.hw_misc) & 0xFFFFu;        // R9: drops of this tick's phase A
+        free_head = H(P.hw_misc) >> 16;
         {
             uint32_t icnt = H(P.hw_misc + 1u);
             if (icnt > kIssueCap) icnt = kIssueCap;              // the executor kernel flags the overflow (err_flag)
             const uint2 *iss = reinterpret_cast<const uint2 *>(blkp + P.off_iss) + lane;
 #pragma unroll 1
-            for (uint32_t j = 0; j < icnt; j++) {
-                const uint2 r = iss[j * 32u];
-                list_insert(r.x >> 28, r.x, make_uint2(((uint32_t)t & 0xFFFFu) | ((r.y & SW_TOK_MASK) << 16), r.y));   // issue = t, remaining = out_total
+            for (uint32_t j0 = 0; j0 < icnt; j0 += 4) {            // four records in flight per lane
+                uint2 r[4];
+#pragma unroll
+                for (uint32_t i = 0; i < 4; i++) if (j0 + i < icnt) r[i] = iss[(j0 + i) * 32u];
+#pragma unroll
+                for (uint32_t i = 0; i < 4; i++)
+                    if (j0 + i < icnt)   // issue = t, remaining = out_total
+                        list_insert(r[i].x >> 28, r[i].x, make_uint2(((uint32_t)t & 0xFFFFu) | ((r[i].y & SW_TOK_MASK) << 16), r[i].y));
             }
             c_issued += icnt;
         }
@@ -305,37 +328,34 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 const uint32_t w0 = M_W0(k);
                 if ((w0 & 0xFFFFu) > 0 && (w0 >> 16) < s_slots[k] && M_KV(k) <= s_kvcap[k]) madm |= 1u << k;
             }
-            // chunks in use end at the highest set bit of the used bitmap (chunks that do not exist are marked used: skip them)
-            {
-                const uint32_t real_chunks = P.RCAP / 16u + N;
-                uint32_t hi = 0;
-#pragma unroll 1
-                for (uint32_t w = 0; w < P.n_chunks / 32u; w++) {
-                    uint32_t u = USED(w);
-                    const uint32_t c0 = w * 32u;
-                    if (c0 + 32u > real_chunks) u &= c0 >= real_chunks ? 0u : ((1u << (real_chunks - c0)) - 1u);
-                    if (u) hi = c0 + 32u - (uint32_t)__clz(u);
-                }
-                meta_words = (hi + 7u) >> 3;
-            }
             uint32_t tokacc = 0;
 #pragma unroll 1
             while (__any_sync(kFull, madm != 0)) {
                 if (madm) {
                     const uint32_t k = (uint32_t)__ffs(madm) - 1u;
-                    uint32_t key, c, p, lastc;
-                    list_min(k, key, c, p, lastc);
+                    // the entry that will fill the hole if the head of the queue is admitted (last of the head chunk):
+                    // its address is known now, so it is fetched together with the keys
+                    const uint32_t n0 = M_W0(k) & 0xFFFFu;
+                    const uint32_t lj = byte_get(HEADW(k), k) * kChunk + ((n0 - 1u) & (kChunk - 1u));
+                    const uint32_t lk = wkey[lj];
+                    const uint2 la = waux[lj];
+                    uint32_t key, bunit;
+                    list_min(k, key, bunit);
                     bool again = false;
                     if (key != ~0u) {
-                        const uint2 wa = waux[c * 16u + p];
+                        // position of the key inside its unit (keys are unique)
+                        const uint4 bu = *reinterpret_cast<const uint4 *>(wkey + bunit * 4u);
+                        const uint32_t j = bunit * 4u + (bu.x == key ? 0u : (bu.y == key ? 1u : (bu.z == key ? 2u : 3u)));
+                        const uint2 wa = waux[j];
                         const uint32_t sw = wa.y, rem0 = wa.x >> 16, id = key & 0xFFFu;
                         const uint32_t need = ((sw >> SW_IN_SHIFT) & SW_TOK_MASK) + ((sw & SW_TOK_MASK) - rem0);     // R12
                         const uint32_t w0 = M_W0(k), nr = w0 >> 16, kv = M_KV(k), slots = s_slots[k];
                         if (nr < slots && kv + need <= s_kvcap[k]) {                          // else: stop at the first misfit (R21)
-                            const uint32_t olo = OCC_LO(k), ohi = OCC_HI(k);
-                            const uint32_t sl = ~olo ? (uint32_t)__ffs(~olo) - 1u : 31u + (uint32_t)__ffs(~ohi);   // lowest free slot (R10)
-                            if (sl < 32) OCC_LO(k) = olo | (1u << sl); else OCC_HI(k) = ohi | (1u << (sl - 32));
+                            uint32_t olo, ohi;
+                            occ_window(s_sbase[k], olo, ohi);
+                            const uint32_t sl = ~olo ? (uint32_t)__ffs(~olo) - 1u : 31u + (uint32_t)__ffs(~ohi);   // lowest free slot (R10): n_run < S_k, so it is one of the model's
                             const uint32_t gs = s_sbase[k] + sl;
+                            OCC(gs >> 5) |= 1u << (gs & 31u);
                             const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
                             // prefill, then its first tick of service (R11)
                             const uint32_t pf = (uint32_t)(((unsigned long long)s_prefill[k] * need) / 1000u);
@@ -355,7 +375,7 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                             M_W0(k) = w0 + 0x10000u;                  // n_run++ (list_remove takes the request off n_wait)
                             M_KV(k) = kv + need;
                             tokacc += tok;
-                            list_remove(k, c, p, lastc);
+                            list_remove(k, j, lk, la);
                             again = (w0 & 0xFFFFu) > 1u && nr + 1u < slots;
                         }
                     }
@@ -368,7 +388,11 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         }
 
         // =============================================================== G complete (R1, R13, R27, R28): completion bits in
-        // slot order = model order, so the per-model latency mean of the EWMA (R13) is a run-length accumulation
+        // slot order = model order, so the per-model latency mean of the EWMA (R13) is a run-length accumulation.
+        // A three-stage software pipeline per lane hides the two dependent loads of a completion (the slot's cold word,
+        // then the plan word of its query): while completion i is processed, the query of i+1 and the cold word of i+2
+        // are in flight.  Rows / log records are claimed with one atomic each and written one iteration later, so the
+        // claim's round trip overlaps the next completion instead of stalling this one.
         uint32_t rew = 0, miss = 0;
         unsigned long long cost = 0;
         {
@@ -381,70 +405,86 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                     M_EWMA(curk) = (uint32_t)ew;
                 }
             };
-#pragma unroll 1
-            for (;;) {
+            // next completion bit of this lane: global slot, or ~0u
+            auto next_slot = [&]() -> uint32_t {
                 while (bits == 0 && wi < P.cm_words) { bits = s_cm[wi * 32u]; wi++; }
-                const bool have = bits != 0;
-                if (!__any_sync(kFull, have)) break;
+                if (bits == 0) return ~0u;
+                const uint32_t b = (uint32_t)__ffs(bits) - 1u;
+                bits &= bits - 1u;
+                const uint32_t g = (wi - 1u) * 4u + (b >> 3), bb = b & 7u;
+                return g * 8u + (((bb & 3u) << 1) | (bb >> 2));
+            };
+            // deferred writes of the previous iteration
+            bool p_fin = false, p_rdy = false;
+            uint32_t p_li = 0, p_idx = 0, p_q = 0, p_pw = 0, p_a0 = 0, p_nc = 0;
+            uint4 p_rec = make_uint4(0, 0, 0, 0), p_qr = make_uint4(0, 0, 0, 0);
+            auto flush_deferred = [&]() {
+                if (p_fin) {
+                    if (p_li + 1u > P.qlog.regcap) atomicOr(P.err_flag, 2u);
+                    P.qlog.rec[(size_t)region * P.qlog.regcap + (p_li % P.qlog.regcap)] = p_rec;
+                    p_fin = false;
+                }
+                if (p_rdy) {
+                    if (P.log_mode && p_idx + p_nc > P.exec.regcap) atomicOr(P.err_flag, 1u);
+                    uint32_t idx0 = p_idx % P.exec.regcap;
+                    write_exec_rows(P, region, idx0, e, p_q, p_pw, p_qr.y >> 16, (int32_t)p_qr.z, t_rel_next, p_a0, p_nc);
+                    p_rdy = false;
+                }
+            };
+            uint32_t gs0 = next_slot(), gs1 = ~0u, gs2 = ~0u;
+            uint4 cd0 = make_uint4(0, 0, 0, 0), cd1 = cd0, cd2 = cd0, qr0 = cd0, qr1 = cd0;
+            if (gs0 != ~0u) { cd0 = cold[gs0]; gs1 = next_slot(); }
+            if (gs1 != ~0u) cd1 = cold[gs1];
+            if (gs0 != ~0u) qr0 = qtab[cd0.z >> 2];
+#pragma unroll 1
+            while (gs0 != ~0u) {
+                if (gs1 != ~0u) { gs2 = next_slot(); if (gs2 != ~0u) cd2 = cold[gs2]; qr1 = qtab[cd1.z >> 2]; }
+                else gs2 = ~0u;
+                // ---- completion of the request in slot gs0
+                const uint32_t k = s_gmodel[gs0 >> 3];
+                const uint32_t q = cd0.z >> 2;                                  // id = 4 q + agent
+                const uint32_t ell = (uint32_t)(t + 1) - (cd0.x & 0xFFFFu);
+                cost += (unsigned long long)((ell << 16) / (qr0.y & 0xFFFFu));  // C_k = l_k / beta, Q16 (R28); l < 2^16
+                if (k != curk) { ewma_flush(); curk = k; latsum = 0; latn = 0; }
+                latsum += ell; latn++;
+                M_W0(k) -= 0x10000u;                                            // n_run--
+                M_KV(k) -= (cd0.y & SW_TOK_MASK) + ((cd0.y >> SW_IN_SHIFT) & SW_TOK_MASK);
+                OCC(gs0 >> 5) &= ~(1u << (gs0 & 31u));
+                c_done++;
+                uint32_t pw = qr0.x;
+                const uint32_t pend = ((pw >> QP_PEND_SHIFT) & 3u) - 1u;
+                pw = (pw & ~(3u << QP_PEND_SHIFT)) | (pend << QP_PEND_SHIFT) | (((cd0.y >> SW_SUCC_SHIFT) & 1u) << QP_SUCC_SHIFT);   // R19: OR
                 bool fin = false, ready = false;
-                uint32_t q = 0, pw = 0, nc = 0, a0 = 0;
-                uint4 qr = make_uint4(0, 0, 0, 0);
-                if (have) {
-                    const uint32_t b = (uint32_t)__ffs(bits) - 1u;
-                    bits &= bits - 1u;
-                    const uint32_t g = (wi - 1u) * 4u + (b >> 3), bb = b & 7u;
-                    const uint32_t gs = g * 8u + (((bb & 3u) << 1) | (bb >> 2));
-                    const uint32_t k = s_gmodel[g], sl = gs - s_sbase[k];
-                    const uint4 cd = cold[gs];
-                    q = cd.z >> 2;                                              // id = 4 q + agent
-                    qr = qtab[q];
-                    const uint32_t ell = (uint32_t)(t + 1) - (cd.x & 0xFFFFu);
-                    cost += (unsigned long long)((ell << 16) / (qr.y & 0xFFFFu));   // C_k = l_k / beta, Q16 (R28); l < 2^16
-                    if (k != curk) { ewma_flush(); curk = k; latsum = 0; latn = 0; }
-                    latsum += ell; latn++;
-                    M_W0(k) -= 0x10000u;                                        // n_run--
-                    M_KV(k) -= (cd.y & SW_TOK_MASK) + ((cd.y >> SW_IN_SHIFT) & SW_TOK_MASK);
-                    if (sl < 32) OCC_LO(k) &= ~(1u << sl); else OCC_HI(k) &= ~(1u << (sl - 32));
-                    c_done++;
-                    pw = qr.x;
-                    const uint32_t pend = ((pw >> QP_PEND_SHIFT) & 3u) - 1u;
-                    pw = (pw & ~(3u << QP_PEND_SHIFT)) | (pend << QP_PEND_SHIFT) | (((cd.y >> SW_SUCC_SHIFT) & 1u) << QP_SUCC_SHIFT);   // R19: OR
-                    if (pend == 0) { if (((pw >> 9) & 7u) == ((pw >> 12) & 7u)) fin = true; else ready = true; }
-                    if (!fin && !(ready && emit)) qtab[q].x = pw;
-                    if (ready && !emit) atomicOr(&qready[(q >> 5) * 32u], 1u << (q & 31u));    // dispatched by the next im_rollout
+                if (pend == 0) { if (((pw >> 9) & 7u) == ((pw >> 12) & 7u)) fin = true; else ready = true; }
+                flush_deferred();
+                if (fin) {
+                    // finalise (R27): reward, SLO miss, sojourn, query log
+                    const uint32_t solved = (pw >> QP_SUCC_SHIFT) & 1u;
+                    const uint32_t sojourn = (uint32_t)(t + 1 - (int32_t)qr0.w);
+                    const uint32_t late = (t + 1 > (int32_t)qr0.z) ? 1u : 0u;
+                    rew += solved; miss += late;
+                    c_fin++; c_solved += solved; c_missed += late; c_soj += sojourn;
+                    p_li = atomicAdd(&P.qlog.cnt[region], 1u);
+                    p_rec = make_uint4(gid, qr0.w, sojourn, (qr0.y & 0xFFFFu) | (solved << 16) | (((pw >> 2) & 3u) << 17) | (((pw >> 6) & 7u) << 19));
+                    p_fin = true;
+                    QFREE(q >> 5) |= 1u << (q & 31u);
+                } else if (ready && emit) {
+                    // next stage of a query whose calls all completed (R17): executor rows of tick t + 1;
+                    // stage++, pending = nc: the calls are issued in phase D of the coming tick
+                    stage_calls((pw >> 2) & 3u, (pw >> 6) & 7u, (pw >> 9) & 7u, p_a0, p_nc);
+                    p_idx = atomicAdd(&P.exec.cnt[region], p_nc);      // (the overflow check of rows_claim waits for the result: deferred too)
+                    p_q = q; p_pw = pw; p_qr = qr0; p_rdy = true;
+                    pw = (pw & ~((7u << 9) | (3u << QP_PEND_SHIFT))) | ((((pw >> 9) & 7u) + 1u) << 9) | (p_nc << QP_PEND_SHIFT);
+                    qtab[q].x = pw;
+                } else {
+                    qtab[q].x = pw;
+                    if (ready) atomicOr(&qready[(q >> 5) * 32u], 1u << (q & 31u));    // dispatched by the next im_rollout
                 }
-                // finalise (R27): reward, SLO miss, sojourn, query log (one claim per warp)
-                const uint32_t finm = __ballot_sync(kFull, fin);
-                if (finm) {
-                    uint32_t lbase = 0;
-                    if (lane == 0) {
-                        lbase = atomicAdd(&P.qlog.cnt[region], (uint32_t)__popc(finm));
-                        if (lbase + __popc(finm) > P.qlog.regcap) atomicOr(P.err_flag, 2u);
-                    }
-                    lbase = __shfl_sync(kFull, lbase, 0);
-                    if (fin) {
-                        const uint32_t solved = (pw >> QP_SUCC_SHIFT) & 1u;
-                        const uint32_t sojourn = (uint32_t)(t + 1 - (int32_t)qr.w);
-                        const uint32_t late = (t + 1 > (int32_t)qr.z) ? 1u : 0u;
-                        rew += solved; miss += late;
-                        c_fin++; c_solved += solved; c_missed += late; c_soj += sojourn;
-                        const uint32_t li = lbase + __popc(finm & lt_mask);
-                        P.qlog.rec[(size_t)region * P.qlog.regcap + (li % P.qlog.regcap)] =
-                            make_uint4(gid, qr.w, sojourn, (qr.y & 0xFFFFu) | (solved << 16) | (((pw >> 2) & 3u) << 17) | (((pw >> 6) & 7u) << 19));
-                        QFREE(q >> 5) |= 1u << (q & 31u);
-                    }
-                }
-                // next stage of a query whose calls all completed (R17): executor rows of tick t + 1
-                if (emit) {
-                    if (ready) stage_calls((pw >> 2) & 3u, (pw >> 6) & 7u, (pw >> 9) & 7u, a0, nc);
-                    uint32_t idx0 = 0;
-                    if (claim_exec_rows(nc, idx0) && ready) {
-                        write_exec_rows(P, region, idx0, e, q, pw, qr.y >> 16, (int32_t)qr.z, t_rel_next, a0, nc);
-                        // stage++, pending = nc: the calls are issued in phase D of the coming tick
-                        qtab[q].x = (pw & ~((7u << 9) | (3u << QP_PEND_SHIFT))) | ((((pw >> 9) & 7u) + 1u) << 9) | (nc << QP_PEND_SHIFT);
-                    }
-                }
+                // the next completion may belong to the same query: its plan word was fetched before this update
+                if (gs1 != ~0u && (cd1.z >> 2) == q) qr1.x = pw;
+                gs0 = gs1; cd0 = cd1; qr0 = qr1; gs1 = gs2; cd1 = cd2;
             }
+            flush_deferred();
             ewma_flush();
         }
 
@@ -458,7 +498,13 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 const uint32_t k = __ffs(mover) - 1u;
                 mover &= mover - 1u;
                 const uint32_t sb = s_sbase[k], cap = s_kvcap[k];
-                uint32_t kv = M_KV(k), npre = 0, olo = OCC_LO(k), ohi = OCC_HI(k);
+                uint32_t kv = M_KV(k), npre = 0, olo, ohi;
+                occ_window(sb, olo, ohi);
+                {   // the window also shows the slots of the models behind k: keep the S_k bits of this one
+                    const uint32_t S = s_slots[k];
+                    if (S < 32) { olo &= (1u << S) - 1u; ohi = 0; }
+                    else if (S < 64) ohi &= (1u << (S - 32)) - 1u;
+                }
 #pragma unroll 1
                 while (kv > cap) {
                     uint32_t best = 0, bsl = 0;
@@ -483,10 +529,11 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                     const uint32_t tm = P.sched_mode ? (bcd.x >> 16) : (bcd.x & 0xFFFFu);
                     list_insert(k, (k << 28) | (tm << 12) | bcd.z, make_uint2((bcd.x & 0xFFFFu) | (rem << 16), bcd.y));   // keeps progress and issue tick; n_wait++
                     if (bsl < 32) olo &= ~(1u << bsl); else ohi &= ~(1u << (bsl - 32));
+                    OCC(gs >> 5) &= ~(1u << (gs & 31u));
                     kv -= ((bcd.y >> SW_IN_SHIFT) & SW_TOK_MASK) + ((bcd.y & SW_TOK_MASK) - rem);
                     npre++;
                 }
-                M_KV(k) = kv; OCC_LO(k) = olo; OCC_HI(k) = ohi;
+                M_KV(k) = kv;
                 M_W0(k) -= npre << 16;                                                   // n_run -= npre
                 c_preempt += npre;
             }
@@ -515,19 +562,24 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 for (uint32_t w = 0; w < P.hw_qfree; w++) H(w) = 0;                        // m and occ
 #pragma unroll 1
                 for (uint32_t g = 0; g < P.n_grp; g++) hot4[g * 32u] = make_uint4(0, 0, 0, 0);
-                // the waiting lists: every chunk back to the pool (chunks that do not exist stay marked used)
-                const uint32_t real_chunks = P.RCAP / 16u + N;
+                // the waiting lists: every chunk back on the free list (0 -> 1 -> ... -> end), every model's list empty
 #pragma unroll 1
-                for (uint32_t w = 0; w < P.n_chunks / 32u; w++) {
-                    const uint32_t c0 = w * 32u;
-                    USED(w) = c0 >= real_chunks ? 0xFFFFFFFFu : (real_chunks - c0 >= 32u ? 0u : ~((1u << (real_chunks - c0)) - 1u));
+                for (uint32_t w = 0; w < (P.n_chunks + 3u) / 4u; w++) {
+                    uint32_t v = 0;
+#pragma unroll
+                    for (uint32_t jj = 0; jj < 4; jj++) v |= (4u * w + jj + 1u < P.n_chunks ? 4u * w + jj + 1u : 0xFFu) << (8u * jj);
+                    H(P.hw_next + w) = v;
                 }
 #pragma unroll 1
-                for (uint32_t w = 0; w < 4; w++) H(P.hw_tail + w) = 0xFFFFFFFFu;
+                for (uint32_t w = 0; w < 4; w++) H(P.hw_head + w) = 0xFFFFFFFFu;
+#pragma unroll 1
+                for (uint32_t w = 0; w < (P.n_chunks + 31u) / 32u; w++) USED(w) = 0;
+                free_head = 0;
             }
         }
     } else {
         bulk::mbar_wait(&s_bar[wib], 0);
+        free_head = H(P.hw_misc) >> 16;
     }
 
     // ===================================================================== pre(t_pre): A arrive, B snapshot, work lists
@@ -577,56 +629,66 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 }
                 n = lo;
             }
-            uint32_t wq = 0, n_ok = 0;
-#pragma unroll 1
-            for (uint32_t j = 0; __any_sync(kFull, j < n); j++) {
-                bool act = j < n;
-                uint32_t q = 0;
-                if (act) {
-                    // the j-th arrival takes the j-th lowest free query index; a full table drops the rest (R9)
-                    while (wq < QW && QFREE(wq) == 0) wq++;
-                    if (wq == QW) { n_ok = j; j = n; act = false; }      // (j is bumped again by the loop: j > n, still done)
-                    else {
-                        const uint32_t fb = QFREE(wq), bit = (uint32_t)__ffs(fb) - 1u;
-                        QFREE(wq) = fb & (fb - 1u);
-                        q = wq * 32u + bit;
-                        n_ok = j + 1;
-                    }
-                }
-                uint32_t in_tok = 0;
-                int32_t dl = 0;
-                if (act) {
-                    const Ph4 d = draw(P, STREAM_QRY, gid, t, j, 0);
-                    const uint32_t comp = d.z < P.mix_thresh ? 0u : 1u;
-                    const uint32_t budget = P.mix_lo[comp] + __umulhi(d.x, P.mix_hi[comp] - P.mix_lo[comp] + 1u);
-                    in_tok = P.has_intok ? __ldg(&P.tab_intok[d.y >> 22]) : P.in_tok_const;
-                    dl = t + (int32_t)budget;                            // PAPER.md:117 deadline = t_arrive + beta
-                    qtab[q] = make_uint4(QP_LIVE, budget | (in_tok << 16), (uint32_t)dl, (uint32_t)t);
-                }
-                const uint32_t pm = __ballot_sync(kFull, act);
-                if (pm) {
-                    uint32_t pbase = 0;
-                    if (lane == 0) pbase = rows_claim(P, P.plan, region, (uint32_t)__popc(pm)) % P.plan.regcap;
-                    pbase = __shfl_sync(kFull, pbase, 0);
-                    if (act) P.plan.row[row_gid_wrapped(P.plan, region, pbase, (uint32_t)__popc(pm & lt_mask))] = make_uint4(e, q | (t_rel << 19), (uint32_t)dl, in_tok);
-                }
-            }
-            c_arr += n; c_drop += n - n_ok; c_plans += n_ok;
-            drops_out = n - n_ok;                                        // carried to phase I of this tick
+            // the j-th arrival takes the j-th lowest free query index; a full table drops the rest (R9)
             uint32_t nfree = 0;
 #pragma unroll 1
             for (uint32_t w = 0; w < QW; w++) nfree += __popc(QFREE(w));
-            if (active) c_live += P.QCAP - nfree;
+            const uint32_t n_ok = min(n, nfree);
+            // planner rows: one claim per warp, lane l writes its rows behind those of the lanes below it
+            uint32_t inc = n_ok;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(kFull, inc, o); if (lane >= (uint32_t)o) inc += v; }
+            const uint32_t ptot = __shfl_sync(kFull, inc, 31);
+            uint32_t pbase = 0;
+            if (ptot) {
+                if (lane == 0) pbase = rows_claim(P, P.plan, region, ptot);
+                pbase = __shfl_sync(kFull, pbase, 0) + inc - n_ok;
+            }
+            uint32_t wq = 0;
+#pragma unroll 1
+            for (uint32_t j = 0; j < n_ok; j++) {
+                while (QFREE(wq) == 0) wq++;
+                const uint32_t fb = QFREE(wq), q = wq * 32u + (uint32_t)__ffs(fb) - 1u;
+                QFREE(wq) = fb & (fb - 1u);
+                const Ph4 d = draw(P, STREAM_QRY, gid, t, j, 0);
+                const uint32_t comp = d.z < P.mix_thresh ? 0u : 1u;
+                const uint32_t budget = P.mix_lo[comp] + __umulhi(d.x, P.mix_hi[comp] - P.mix_lo[comp] + 1u);
+                const uint32_t in_tok = P.has_intok ? __ldg(&P.tab_intok[d.y >> 22]) : P.in_tok_const;
+                const int32_t dl = t + (int32_t)budget;                  // PAPER.md:117 deadline = t_arrive + beta
+                qtab[q] = make_uint4(QP_LIVE, budget | (in_tok << 16), (uint32_t)dl, (uint32_t)t);
+                P.plan.row[region * P.plan.regcap + (pbase + j) % P.plan.regcap] = make_uint4(e, q | (t_rel << 19), (uint32_t)dl, in_tok);
+            }
+            c_arr += n; c_drop += n - n_ok; c_plans += n_ok;
+            drops_out = n - n_ok;                                        // carried to phase I of this tick
+            if (active) c_live += P.QCAP - (nfree - n_ok);
         }
     }
-    // ---- B snapshot (R14): telemetry features of the state left by the tick just finished
-    if (pre_mode != 0 && active) {
-        float *sn = P.snap + (size_t)e * 3 * N;
+    // ---- B snapshot (R14): telemetry features of the state left by the tick just finished.  A lane holds the 3N
+    // features of ITS env, the policy kernels want them contiguous per env: eight features at a time go through a
+    // [32][9] staging tile, so that the stores are whole 32-byte sectors (eight lanes per env) instead of 3N scattered words
+    if (pre_mode != 0) {
+        float *stage = reinterpret_cast<float *>(sm + L.o_stage);
+        float *snb = P.snap + (size_t)blk * 32u * 3u * N;                      // the block's rows: 32 x 3N contiguous floats
+        const uint32_t N3 = 3u * N, n_valid = min(32u, P.E - blk * 32u);
+        __syncwarp();
 #pragma unroll 1
-        for (uint32_t k = 0; k < N; k++) {
-            sn[k] = __uint2float_rn(M_W0(k) & 0xFFFFu) * 0x1p-6f;
-            sn[N + k] = __uint2float_rn(M_EWMA(k)) * 0x1p-18f;
-            sn[2 * N + k] = __fmul_rn(__uint2float_rn(M_KV(k)), s_kvinv[k]);
+        for (uint32_t f0 = 0; f0 < N3; f0 += 8) {
+#pragma unroll
+            for (uint32_t j = 0; j < 8; j++) {
+                const uint32_t f = f0 + j;
+                float v = 0.0f;
+                if (f < N) v = __uint2float_rn(M_W0(f) & 0xFFFFu) * 0x1p-6f;
+                else if (f < 2 * N) v = __uint2float_rn(M_EWMA(f - N)) * 0x1p-18f;
+                else if (f < N3) v = __fmul_rn(__uint2float_rn(M_KV(f - 2 * N)), s_kvinv[f - 2 * N]);
+                stage[lane * 9u + j] = v;
+            }
+            __syncwarp();
+#pragma unroll
+            for (uint32_t i = 0; i < 8; i++) {
+                const uint32_t idx = i * 32u + lane, env = idx >> 3, j = idx & 7u;
+                if (env < n_valid && f0 + j < N3) snb[env * N3 + f0 + j] = stage[env * 9u + j];
+            }
+            __syncwarp();
         }
     }
     // ---- counters
@@ -638,7 +700,7 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
             if (cv[c] != 0) atomicAdd(&ctr[c * 32], cv[c]);      // no return value: a fire-and-forget reduction, no round trip
     }
     // ---- header back to HBM: one bulk copy
-    H(P.hw_misc) = drops_out;
+    H(P.hw_misc) = drops_out | (free_head << 16);
     H(P.hw_misc + 1u) = 0;
     bulk::fence_proxy_async();
     __syncwarp();
@@ -651,12 +713,11 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
 #undef M_W0
 #undef M_KV
 #undef M_EWMA
-#undef OCC_LO
-#undef OCC_HI
+#undef OCC
 #undef QFREE
-#undef META
+#undef NEXTW
+#undef HEADW
 #undef USED
-#undef TAILW
 }
 
 // opt-in to the dynamic shared memory the kernel needs on the CURRENT device (attributes are per device: im_bind calls this)
