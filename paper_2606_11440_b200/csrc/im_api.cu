@@ -295,9 +295,9 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     const size_t ctl_off = cv.off;
     P.snap = cv.take<float>((size_t)E * 3 * N);
     P.err_flag = cv.take<uint32_t>(64);
-    P.exec.cnt = cv.take<uint32_t>(kRegions); P.exec.base = cv.take<uint32_t>(2 * kRegions);
-    P.plan.cnt = cv.take<uint32_t>(kRegions); P.plan.base = cv.take<uint32_t>(2 * kRegions);
-    P.qlog.cnt = cv.take<uint32_t>(kRegions);
+    P.exec.cnt = cv.take<uint32_t>(kRegions * kCntStride); P.exec.base = cv.take<uint32_t>(2 * kRegions);
+    P.plan.cnt = cv.take<uint32_t>(kRegions * kCntStride); P.plan.base = cv.take<uint32_t>(2 * kRegions);
+    P.qlog.cnt = cv.take<uint32_t>(kRegions * kCntStride);
     double *sums = cv.take<double>(8);
     const size_t ctl_end = cv.off;
     // ---- tables
@@ -375,6 +375,15 @@ static int copy_out(im_ctx *c, const void *src, size_t bytes, void *dst, size_t 
     if (cap < bytes) return fail(c, IM_ERR_CAPACITY, "dst too small: %zu < %zu", cap, bytes);
     CUDA_TRY(c, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return IM_OK;
+}
+
+// the append counters of the kRegions regions of a list (one 128-byte line apart on the device)
+static int read_counts(im_ctx *c, const uint32_t *dev_cnt, uint32_t (&cnt)[kRegions])
+{
+    std::vector<uint32_t> h(kRegions * kCntStride);
+    CUDA_TRY(c, cudaMemcpy(h.data(), dev_cnt, h.size() * 4, cudaMemcpyDeviceToHost));
+    for (uint32_t r = 0; r < kRegions; r++) cnt[r] = h[r * kCntStride];
     return IM_OK;
 }
 
@@ -499,12 +508,12 @@ int im_rollout(im_ctx *c, const void *policy_weights, uint32_t n_ticks)
     const Params &P = c->P;
     const bool bf16 = c->spec.policy_dtype == IM_DTYPE_BF16;
     if (P.log_mode) {   // logs restart with every rollout
-        CUDA_TRY(c, cudaMemsetAsync(P.exec.cnt, 0, sizeof(uint32_t) * kRegions, st));
+        CUDA_TRY(c, cudaMemsetAsync(P.exec.cnt, 0, sizeof(uint32_t) * kRegions * kCntStride, st));
         CUDA_TRY(c, cudaMemsetAsync(P.exec.base, 0, sizeof(uint32_t) * 2 * kRegions, st));
-        CUDA_TRY(c, cudaMemsetAsync(P.plan.cnt, 0, sizeof(uint32_t) * kRegions, st));
+        CUDA_TRY(c, cudaMemsetAsync(P.plan.cnt, 0, sizeof(uint32_t) * kRegions * kCntStride, st));
         CUDA_TRY(c, cudaMemsetAsync(P.plan.base, 0, sizeof(uint32_t) * 2 * kRegions, st));
     }
-    CUDA_TRY(c, cudaMemsetAsync(P.qlog.cnt, 0, sizeof(uint32_t) * kRegions, st));
+    CUDA_TRY(c, cudaMemsetAsync(P.qlog.cnt, 0, sizeof(uint32_t) * kRegions * kCntStride, st));
     const int32_t t0 = c->tick;
     prof_begin(c, IM_KERNEL_SIM);
     launch_sim(P, -1, 0, t0, 1, t0, st);                                   // A, B of the first tick
@@ -615,8 +624,8 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         double s[8] = {0, 0, 0, 0, 0, 0, 0, 0}, out[8];
         if (c->have_returns) CUDA_TRY(c, cudaMemcpy(s, c->sums, 32, cudaMemcpyDeviceToHost));
         uint32_t ce[kRegions], cp[kRegions];
-        CUDA_TRY(c, cudaMemcpy(ce, P.exec.cnt, sizeof ce, cudaMemcpyDeviceToHost));
-        CUDA_TRY(c, cudaMemcpy(cp, P.plan.cnt, sizeof cp, cudaMemcpyDeviceToHost));
+        if (int rc = read_counts(c, P.exec.cnt, ce)) return rc;
+        if (int rc = read_counts(c, P.plan.cnt, cp)) return rc;
         double ne = 0, np = 0;
         for (uint32_t r = 0; r < kRegions; r++) { ne += ce[r]; np += cp[r]; }
         const double cnt = s[3], mean = cnt > 0 ? s[1] / cnt : 0.0;
@@ -637,7 +646,7 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         const RowBuf &rb = ex ? P.exec : P.plan;
         if (lg && !rb.logits) return fail(c, IM_ERR_STATE, "logits need IM_FLAG_LOG_LOGITS");
         uint32_t cnt[kRegions];
-        CUDA_TRY(c, cudaMemcpy(cnt, rb.cnt, sizeof cnt, cudaMemcpyDeviceToHost));
+        if (int rc = read_counts(c, rb.cnt, cnt)) return rc;
         size_t n = 0;
         for (uint32_t r = 0; r < kRegions; r++) n += cnt[r];
         const size_t rec = lg ? 4 * rb.n_out : 24;
@@ -676,7 +685,7 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
     case IM_TEL_UNORM: {
         if (what == IM_TEL_UNORM && !c->have_returns) return fail(c, IM_ERR_STATE, "UNORM read before im_returns");
         uint32_t cnt[kRegions];
-        CUDA_TRY(c, cudaMemcpy(cnt, P.qlog.cnt, sizeof cnt, cudaMemcpyDeviceToHost));
+        if (int rc = read_counts(c, P.qlog.cnt, cnt)) return rc;
         size_t n = 0;
         for (uint32_t r = 0; r < kRegions; r++) n += cnt[r];
         const size_t rec = what == IM_TEL_QUERIES ? 16 : 4;

@@ -44,6 +44,8 @@ namespace im {
 constexpr uint32_t kMaxModels = 16;
 constexpr uint32_t kRegions = 64;        // row-list / log regions (one atomic counter each), region = (env / 32) % n_regions
 constexpr uint32_t kDtUs = 50000;
+constexpr uint32_t kCntStride = 32;      // words between the append counters of two regions: one 128-byte line each, so that
+                                         // the claims of different regions never queue on the same L2 line
 constexpr uint32_t kChunk = 32;          // entries per waiting-list chunk
 constexpr uint32_t kIssueCap = 128;      // issue records per env per tick (31 arrivals x 3 calls + continuing stages)
 
@@ -73,7 +75,7 @@ struct RowBuf {
     float *logp;
     float *val;          // exec only
     float *logits;       // optional [rows][n_out]
-    uint32_t *cnt;       // [kRegions] monotonically increasing append counters
+    uint32_t *cnt;       // [kRegions * kCntStride] monotonically increasing append counters, counter of region r at r * kCntStride
     uint32_t *base;      // [2][kRegions] start of the current tick's rows (parity double buffer)
     uint32_t regcap;
     uint32_t n_out;
@@ -82,7 +84,7 @@ struct RowBuf {
 struct QLog {
     uint4 *rec;          // {env (global), arrive, sojourn, budget | solved<<16 | topo<<17 | keff<<19}
     float *unorm;
-    uint32_t *cnt;       // [kRegions]
+    uint32_t *cnt;       // [kRegions * kCntStride], as RowBuf::cnt
     uint32_t regcap;
 };
 
@@ -259,7 +261,7 @@ __device__ __forceinline__ uint32_t row_gid_wrapped(const RowBuf &rb, uint32_t r
 // im_policy.cu) flags a tick that produced more rows than the ring holds.
 __device__ __forceinline__ uint32_t rows_claim(const Params &P, const RowBuf &rb, uint32_t region, uint32_t n)
 {
-    const uint32_t idx = atomicAdd(&rb.cnt[region], n);
+    const uint32_t idx = atomicAdd(&rb.cnt[region * kCntStride], n);
     if (P.log_mode && idx + n > rb.regcap) atomicOr(P.err_flag, 1u);
     return idx;
 }

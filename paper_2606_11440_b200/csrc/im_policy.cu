@@ -24,7 +24,7 @@ struct TileSched {
 __device__ __forceinline__ void sched_init(const Params &P, TileSched &S, const RowBuf &rb, uint32_t parity, uint32_t rows_per_tile, uint32_t n_crit)
 {
     if (threadIdx.x < kRegions) {
-        const uint32_t b = rb.base[parity * kRegions + threadIdx.x], c = rb.cnt[threadIdx.x];
+        const uint32_t b = rb.base[parity * kRegions + threadIdx.x], c = rb.cnt[threadIdx.x * kCntStride];
         // a ring (no decision log) holds one tick's rows: more than regcap of them have overwritten each other
         if (blockIdx.x == 0 && !P.log_mode && c - b > rb.regcap) atomicOr(P.err_flag, 1u);
         S.base[threadIdx.x] = b;
@@ -57,7 +57,7 @@ __device__ __forceinline__ bool tile_row(const Params &P, const TileSched &S, co
     uint32_t lo = 0, hi = kRegions;
     while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
     const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * rows_per_tile + r;
-    if (idx >= rb.cnt[lo]) return false;
+    if (idx >= S.cnt[lo]) return false;
     const uint32_t g = row_gid(rb, lo, idx);
     const uint4 row = rb.row[g];
     ri.env = row.x; ri.a = row.y; ri.dl = (int32_t)row.z; ri.c = row.w; ri.gidx = g; ri.critic = false;

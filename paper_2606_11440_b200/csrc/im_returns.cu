@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(256)
 k_utility(const QLog ql, float mu, double *__restrict__ sums)
 {
     const uint32_t region = blockIdx.y;
-    const uint32_t n = min(ql.cnt[region], ql.regcap);
+    const uint32_t n = min(ql.cnt[region * kCntStride], ql.regcap);
     double su = 0.0, su2 = 0.0, cn = 0.0;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const size_t g = (size_t)region * ql.regcap + i;
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(256)
 k_unorm(const QLog ql, const double *__restrict__ sums)
 {
     const uint32_t region = blockIdx.y;
-    const uint32_t n = min(ql.cnt[region], ql.regcap);
+    const uint32_t n = min(ql.cnt[region * kCntStride], ql.regcap);
     const double cnt = sums[3];
     const double mean = cnt > 0 ? sums[1] / cnt : 0.0;
     double var = cnt > 0 ? sums[2] / cnt - mean * mean : 0.0;

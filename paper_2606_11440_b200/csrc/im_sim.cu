@@ -93,7 +93,7 @@ k_serve(const Params P, int32_t t)
     uint4 h[8];
 #pragma unroll
     for (int i = 0; i < 8; i++) if ((uint32_t)i < ng) h[i] = hot4[(g0 + i) * 32u];
-    uint32_t tot = 0, cb_lo = 0, cb_hi = 0;                      // completion bytes of groups 0-3 / 4-7 of the model
+    uint32_t tot = 0;
 #pragma unroll
     for (int i = 0; i < 8; i++) {
         if ((uint32_t)i < ng) {
@@ -111,28 +111,10 @@ k_serve(const Params P, int32_t t)
                 tot += (totp & 0xFFFFu) + (totp >> 16);
                 if (any) hot4[g * 32u] = r;
             }
-            const uint32_t c8 = (cacc & 0xFu) | ((cacc >> 12) & 0xF0u);
-            cmb[(g >> 2) * 128u + (g & 3u)] = (uint8_t)c8;
-            if (i < 4) cb_lo |= c8 << (8 * i); else cb_hi |= c8 << (8 * (i - 4));
+            cmb[(g >> 2) * 128u + (g & 3u)] = (uint8_t)((cacc & 0xFu) | ((cacc >> 12) & 0xF0u));
         }
     }
     reinterpret_cast<uint32_t *>(blkp + P.off_kvt)[k * 32u + lane] = tot;
-    // Warm the L2 for k_sim's completion phase: the cold word of every completed slot and the table entry of its query
-    // (two dependent accesses at data-dependent addresses, cheap here where 32 warps per SM hide them)
-    const uint4 *cold = reinterpret_cast<const uint4 *>(blkp + P.off_cold + (size_t)lane * P.cold_stride);
-    const uint4 *qtab = reinterpret_cast<const uint4 *>(blkp + P.off_q + (size_t)lane * P.q_stride);
-#pragma unroll 1
-    for (uint32_t half = 0; half < 2; half++) {
-        uint32_t bits = half ? cb_hi : cb_lo;
-#pragma unroll 1
-        while (bits) {
-            const uint32_t b = (uint32_t)__ffs(bits) - 1u;
-            bits &= bits - 1u;
-            const uint32_t bb = b & 7u, gs = (g0 + half * 4u + (b >> 3)) * 8u + (((bb & 3u) << 1) | (bb >> 2));
-            const uint32_t id = cold[gs].z;
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(qtab + (id >> 2)));
-        }
-    }
 }
 
 // tick arguments: t_post < 0 => no post phases; pre_mode 0 none, 1 full (A, B, rows), 2 snapshot only
@@ -414,22 +396,16 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 const uint32_t g = (wi - 1u) * 4u + (b >> 3), bb = b & 7u;
                 return g * 8u + (((bb & 3u) << 1) | (bb >> 2));
             };
-            // deferred writes of the previous iteration
-            bool p_fin = false, p_rdy = false;
-            uint32_t p_li = 0, p_idx = 0, p_q = 0, p_pw = 0, p_a0 = 0, p_nc = 0;
-            uint4 p_rec = make_uint4(0, 0, 0, 0), p_qr = make_uint4(0, 0, 0, 0);
-            auto flush_deferred = [&]() {
-                if (p_fin) {
-                    if (p_li + 1u > P.qlog.regcap) atomicOr(P.err_flag, 2u);
-                    P.qlog.rec[(size_t)region * P.qlog.regcap + (p_li % P.qlog.regcap)] = p_rec;
-                    p_fin = false;
-                }
-                if (p_rdy) {
-                    if (P.log_mode && p_idx + p_nc > P.exec.regcap) atomicOr(P.err_flag, 1u);
-                    uint32_t idx0 = p_idx % P.exec.regcap;
-                    write_exec_rows(P, region, idx0, e, p_q, p_pw, p_qr.y >> 16, (int32_t)p_qr.z, t_rel_next, p_a0, p_nc);
-                    p_rdy = false;
-                }
+            // Log records and executor rows of the tick are buffered per lane (two of each; more than that is rare and
+            // claims for itself) and written after the loop with ONE claim per warp each: a claim is an atomic on the
+            // region's counter, and 32 lanes x several events per tick on the same line queue up in the L2
+            uint32_t nf = 0, nr = 0;                              // buffered finalisations / ready queries of this lane
+            uint4 f_rec[2];
+            uint32_t r_q[2], r_pw[2], r_io[2], r_dl[2];          // ready: query, plan word (stage to dispatch), in_tok, deadline
+            auto emit_rows = [&](uint32_t idx, uint32_t q, uint32_t pw, uint32_t in_tok, uint32_t dl) {
+                uint32_t a0, nc;
+                stage_calls((pw >> 2) & 3u, (pw >> 6) & 7u, (pw >> 9) & 7u, a0, nc);
+                write_exec_rows(P, region, idx % P.exec.regcap, e, q, pw, in_tok, (int32_t)dl, t_rel_next, a0, nc);
             };
             uint32_t gs0 = next_slot(), gs1 = ~0u, gs2 = ~0u;
             uint4 cd0 = make_uint4(0, 0, 0, 0), cd1 = cd0, cd2 = cd0, qr0 = cd0, qr1 = cd0;
@@ -456,7 +432,6 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 pw = (pw & ~(3u << QP_PEND_SHIFT)) | (pend << QP_PEND_SHIFT) | (((cd0.y >> SW_SUCC_SHIFT) & 1u) << QP_SUCC_SHIFT);   // R19: OR
                 bool fin = false, ready = false;
                 if (pend == 0) { if (((pw >> 9) & 7u) == ((pw >> 12) & 7u)) fin = true; else ready = true; }
-                flush_deferred();
                 if (fin) {
                     // finalise (R27): reward, SLO miss, sojourn, query log
                     const uint32_t solved = (pw >> QP_SUCC_SHIFT) & 1u;
@@ -464,17 +439,26 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                     const uint32_t late = (t + 1 > (int32_t)qr0.z) ? 1u : 0u;
                     rew += solved; miss += late;
                     c_fin++; c_solved += solved; c_missed += late; c_soj += sojourn;
-                    p_li = atomicAdd(&P.qlog.cnt[region], 1u);
-                    p_rec = make_uint4(gid, qr0.w, sojourn, (qr0.y & 0xFFFFu) | (solved << 16) | (((pw >> 2) & 3u) << 17) | (((pw >> 6) & 7u) << 19));
-                    p_fin = true;
+                    const uint4 rec = make_uint4(gid, qr0.w, sojourn, (qr0.y & 0xFFFFu) | (solved << 16) | (((pw >> 2) & 3u) << 17) | (((pw >> 6) & 7u) << 19));
+                    if (nf == 0) f_rec[0] = rec;
+                    else if (nf == 1) f_rec[1] = rec;
+                    else {
+                        const uint32_t li = atomicAdd(&P.qlog.cnt[region * kCntStride], 1u);
+                        if (li + 1u > P.qlog.regcap) atomicOr(P.err_flag, 2u);
+                        P.qlog.rec[(size_t)region * P.qlog.regcap + (li % P.qlog.regcap)] = rec;
+                    }
+                    nf++;
                     QFREE(q >> 5) |= 1u << (q & 31u);
                 } else if (ready && emit) {
                     // next stage of a query whose calls all completed (R17): executor rows of tick t + 1;
                     // stage++, pending = nc: the calls are issued in phase D of the coming tick
-                    stage_calls((pw >> 2) & 3u, (pw >> 6) & 7u, (pw >> 9) & 7u, p_a0, p_nc);
-                    p_idx = atomicAdd(&P.exec.cnt[region], p_nc);      // (the overflow check of rows_claim waits for the result: deferred too)
-                    p_q = q; p_pw = pw; p_qr = qr0; p_rdy = true;
-                    pw = (pw & ~((7u << 9) | (3u << QP_PEND_SHIFT))) | ((((pw >> 9) & 7u) + 1u) << 9) | (p_nc << QP_PEND_SHIFT);
+                    uint32_t a0, nc;
+                    stage_calls((pw >> 2) & 3u, (pw >> 6) & 7u, (pw >> 9) & 7u, a0, nc);
+                    if (nr == 0) { r_q[0] = q; r_pw[0] = pw; r_io[0] = qr0.y >> 16; r_dl[0] = qr0.z; }
+                    else if (nr == 1) { r_q[1] = q; r_pw[1] = pw; r_io[1] = qr0.y >> 16; r_dl[1] = qr0.z; }
+                    else emit_rows(rows_claim(P, P.exec, region, nc), q, pw, qr0.y >> 16, qr0.z);
+                    nr++;
+                    pw = (pw & ~((7u << 9) | (3u << QP_PEND_SHIFT))) | ((((pw >> 9) & 7u) + 1u) << 9) | (nc << QP_PEND_SHIFT);
                     qtab[q].x = pw;
                 } else {
                     qtab[q].x = pw;
@@ -484,8 +468,40 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 if (gs1 != ~0u && (cd1.z >> 2) == q) qr1.x = pw;
                 gs0 = gs1; cd0 = cd1; qr0 = qr1; gs1 = gs2; cd1 = cd2;
             }
-            flush_deferred();
             ewma_flush();
+            // ---- the buffered log records: one claim per warp
+            {
+                const uint32_t mine = min(nf, 2u);
+                const uint32_t b0 = __ballot_sync(kFull, (mine & 1u) != 0), b1 = __ballot_sync(kFull, (mine & 2u) != 0);
+                const uint32_t tot = __popc(b0) + 2u * __popc(b1);
+                if (tot) {
+                    uint32_t base = 0;
+                    if (lane == 0) {
+                        base = atomicAdd(&P.qlog.cnt[region * kCntStride], tot);
+                        if (base + tot > P.qlog.regcap) atomicOr(P.err_flag, 2u);
+                    }
+                    base = __shfl_sync(kFull, base, 0) + __popc(b0 & lt_mask) + 2u * __popc(b1 & lt_mask);
+                    if (mine > 0) P.qlog.rec[(size_t)region * P.qlog.regcap + (base % P.qlog.regcap)] = f_rec[0];
+                    if (mine > 1) P.qlog.rec[(size_t)region * P.qlog.regcap + ((base + 1u) % P.qlog.regcap)] = f_rec[1];
+                }
+            }
+            // ---- the buffered executor rows: one claim per warp (a ready query has 1 .. 3 calls in its next stage)
+            {
+                uint32_t n0 = 0, n1 = 0, a0;
+                if (nr > 0) stage_calls((r_pw[0] >> 2) & 3u, (r_pw[0] >> 6) & 7u, (r_pw[0] >> 9) & 7u, a0, n0);
+                if (nr > 1) stage_calls((r_pw[1] >> 2) & 3u, (r_pw[1] >> 6) & 7u, (r_pw[1] >> 9) & 7u, a0, n1);
+                uint32_t inc = n0 + n1;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(kFull, inc, o); if (lane >= (uint32_t)o) inc += v; }
+                const uint32_t tot = __shfl_sync(kFull, inc, 31);
+                if (tot) {
+                    uint32_t base = 0;
+                    if (lane == 0) base = rows_claim(P, P.exec, region, tot);
+                    base = __shfl_sync(kFull, base, 0) + inc - (n0 + n1);
+                    if (nr > 0) emit_rows(base, r_q[0], r_pw[0], r_io[0], r_dl[0]);
+                    if (nr > 1) emit_rows(base + n0, r_q[1], r_pw[1], r_io[1], r_dl[1]);
+                }
+            }
         }
 
         // =============================================================== H preempt (R21): largest (deadline, id) first
