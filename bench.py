@@ -260,9 +260,11 @@ def main():
         tms = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tms, op=dist.ReduceOp.MAX)
         ms = float(tms.item())
-        # the step's one collective: the four sums behind C-bar / U-bar / sigma_U over all ranks
-        from paper_2606_11440_b200.sharding import allreduce_scalars
-        sc.update(allreduce_scalars(sc, device=dev))
+        # the step's one collective: the four sums behind C-bar / U-bar / sigma_U over all ranks;
+        # every rank then re-normalises its UNORM with the job's statistics inside the library
+        from paper_2606_11440_b200.sharding import allreduce_sums
+        last.returns_finish(allreduce_sums(last.sums(), device=dev))
+        sc = last.scalars()
     ms_per_step = ms / args.steps
     env_ticks_per_s = world * E * T / (ms_per_step * 1e-3)
     model = algorithmic_model(spec, csum, T, E)

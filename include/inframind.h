@@ -126,6 +126,14 @@ int im_rollout(im_ctx *ctx, const void *policy_weights, uint32_t n_ticks);
  * (c) C-bar = sum(cost)/#finished for the dual update (Eq. 7). Asynchronous. */
 int im_returns(im_ctx *ctx, float gamma, float lambda, float lagrange_mu);
 
+/* Env-sharded jobs (one ctx per GPU): every rank calls im_returns, the four sums of IM_TEL_SUMS are
+ * added over the ranks (the job's ONE collective, e.g. an NCCL all-reduce of 4 doubles), and every rank calls
+ * im_returns_finish with the job-wide sums (HOST array of 4 doubles, same order as IM_TEL_SUMS).  UNORM is then
+ * re-normalised with the job's U-bar / sigma_U (Eq. 6) and SCALARS reports the job's C-bar, U-bar,
+ * sigma_U, sum_cost, n_finished: the sharded result equals the single-GPU result.  Without this call UNORM and
+ * SCALARS are those of the ctx's own envs.  IM_ERR_STATE before im_returns.  Asynchronous. */
+int im_returns_finish(im_ctx *ctx, const double *global_sums);
+
 /* selectors of im_read_telemetry / im_device_ptr */
 typedef enum im_telemetry {
     IM_TEL_SNAPSHOT = 1,   /* u32 [E][N][4] = {n_wait, n_run, kv_used, ewma_q8}: the paper's d vectors */
@@ -139,7 +147,8 @@ typedef enum im_telemetry {
     IM_TEL_MISS = 7,       /* u8  [T][E] (saturating) */
     IM_TEL_ADV = 8,        /* f32 [T][E]   (after im_returns) */
     IM_TEL_RET = 9,        /* f32 [T][E]   (after im_returns) */
-    IM_TEL_SCALARS = 10,   /* f64 [8]: cbar, ubar, usigma, sum_cost, n_finished, n_exec_decisions, n_plan_decisions, tick */
+    IM_TEL_SCALARS = 10,   /* f64 [8]: cbar, ubar, usigma, sum_cost, n_finished (of the ctx, or of the job after
+                              im_returns_finish), n_exec_decisions, n_plan_decisions, tick */
     IM_TEL_DECISIONS_EXEC = 11, /* u32 [n][6]: env(global), t(abs), q | agent<<16, action, logp(f32 bits), value(f32 bits) */
     IM_TEL_DECISIONS_PLAN = 12, /* u32 [n][6]: env(global), t(abs), q, topo | cnt<<2 | roles<<4, logp(f32 bits), 0 */
     IM_TEL_QUERIES = 13,   /* u32 [n][4]: env(global), arrive, sojourn, budget | solved<<16 | topo<<17 | keff<<19 */
@@ -149,7 +158,10 @@ typedef enum im_telemetry {
                               of model 0, model 1, ... each in slack (R20 key) order; unused tail = 0xFFFFFFFF */
     IM_TEL_TABLES = 17,    /* u32: out_tok_mult_q16[1024], in_tok[1024], arr_cdf[n_levels*32] as uploaded */
     IM_TEL_LOGITS_EXEC = 18,/* f32 [n][3N+1], same order as DECISIONS_EXEC (needs IM_FLAG_LOG_LOGITS) */
-    IM_TEL_LOGITS_PLAN = 19 /* f32 [n][24] */
+    IM_TEL_LOGITS_PLAN = 19,/* f32 [n][24] */
+    IM_TEL_SUMS = 20       /* f64 [4]: the raw sums of THIS ctx behind the scalars (after im_returns): sum of cost,
+                              number of finalised queries, sum of U_i, sum of U_i^2 - what an env-sharded job
+                              all-reduces before im_returns_finish */
 } im_telemetry;
 
 /* STATE dump, per env (free slots are all-zero words):

@@ -8,5 +8,5 @@ from .binding import (  # noqa: F401
     IM_FLAG_LOG_DECISIONS, IM_FLAG_LOG_LOGITS,
     IM_TEL_SNAPSHOT, IM_TEL_COUNTERS, IM_TEL_REW, IM_TEL_COST, IM_TEL_VAL, IM_TEL_DONE, IM_TEL_MISS, IM_TEL_ADV,
     IM_TEL_RET, IM_TEL_SCALARS, IM_TEL_DECISIONS_EXEC, IM_TEL_DECISIONS_PLAN, IM_TEL_QUERIES, IM_TEL_UNORM,
-    IM_TEL_STATE, IM_TEL_QUEUE_ORDER, IM_TEL_TABLES, IM_TEL_LOGITS_EXEC, IM_TEL_LOGITS_PLAN,
+    IM_TEL_STATE, IM_TEL_QUEUE_ORDER, IM_TEL_TABLES, IM_TEL_LOGITS_EXEC, IM_TEL_LOGITS_PLAN, IM_TEL_SUMS,
 )

@@ -20,9 +20,9 @@ IM_ABI_VERSION = 1
 IM_FLAG_LOG_DECISIONS, IM_FLAG_LOG_LOGITS = 1, 2
 (IM_TEL_SNAPSHOT, IM_TEL_COUNTERS, IM_TEL_REW, IM_TEL_COST, IM_TEL_VAL, IM_TEL_DONE, IM_TEL_MISS, IM_TEL_ADV, IM_TEL_RET,
  IM_TEL_SCALARS, IM_TEL_DECISIONS_EXEC, IM_TEL_DECISIONS_PLAN, IM_TEL_QUERIES, IM_TEL_UNORM, IM_TEL_STATE,
- IM_TEL_QUEUE_ORDER, IM_TEL_TABLES, IM_TEL_LOGITS_EXEC, IM_TEL_LOGITS_PLAN) = range(1, 20)
+ IM_TEL_QUEUE_ORDER, IM_TEL_TABLES, IM_TEL_LOGITS_EXEC, IM_TEL_LOGITS_PLAN, IM_TEL_SUMS) = range(1, 21)
 
-EXPORTS = ["im_arena_bytes", "im_create", "im_bind", "im_reset", "im_rollout", "im_returns", "im_read_telemetry",
+EXPORTS = ["im_arena_bytes", "im_create", "im_bind", "im_reset", "im_rollout", "im_returns", "im_returns_finish", "im_read_telemetry",
            "im_device_ptr", "im_launch_count", "im_set_profiling", "im_kernel_times", "im_destroy", "im_last_error"]
 
 
@@ -61,6 +61,7 @@ def load_library():
         L.im_reset.argtypes = [C.c_void_p]
         L.im_rollout.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32]
         L.im_returns.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float]
+        L.im_returns_finish.argtypes = [C.c_void_p, C.c_void_p]
         L.im_read_telemetry.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_size_t, C.c_void_p]
         L.im_device_ptr.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
         L.im_launch_count.restype = C.c_uint64
@@ -175,6 +176,16 @@ class InfraMind:
 
     def returns(self, gamma: float, lam: float, mu: float):
         self._check(self._L.im_returns(self._h, gamma, lam, mu))
+
+    def sums(self) -> np.ndarray:
+        """IM_TEL_SUMS: float64 [sum_cost, n_final, sum_U, sum_U2] of this ctx (what an env-sharded job all-reduces)."""
+        return self.read(IM_TEL_SUMS, np.float64, (4,))
+
+    def returns_finish(self, global_sums):
+        """im_returns_finish: re-normalise UNORM / SCALARS with the job-wide sums (host array of 4 doubles)."""
+        g = np.ascontiguousarray(global_sums, dtype=np.float64)
+        assert g.shape == (4,)
+        self._check(self._L.im_returns_finish(self._h, g.ctypes.data_as(C.c_void_p)))
 
     def read(self, what: int, dtype, shape=None, out: Optional[np.ndarray] = None) -> np.ndarray:
         """im_read_telemetry into a numpy array (size queried first when shape is None)."""

@@ -20,6 +20,7 @@ int sim_prepare_device();
 int policy_prepare_device(const Params &P);
 int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity, int32_t t0, uint32_t trow, int n_sm, bool bf16, cudaStream_t st);
 int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st);
+int launch_unorm(const Params &P, float mu, const double *sums_used, cudaStream_t st);
 int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t st);
 size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP);
 bool tc_supported(uint32_t F, uint32_t H);
@@ -107,6 +108,7 @@ struct im_ctx {
     int32_t tick = 0, last_t0 = 0;
     uint32_t last_T = 0;
     bool have_returns = false;
+    float last_mu = 0.0f;
     uint32_t par_exec = 0, par_plan = 0;
     int n_sm = 148;
     uint64_t launches = 0;
@@ -554,7 +556,21 @@ int im_returns(im_ctx *c, float gamma, float lambda, float lagrange_mu)
     c->launches += launch_returns(c->P, c->last_T, gamma, lambda, lagrange_mu, c->adv, c->ret, c->sums, c->stream);
     prof_end(c);
     CUDA_TRY(c, cudaGetLastError());
-    c->have_returns = true;
+    c->have_returns = true; c->last_mu = lagrange_mu;
+    return IM_OK;
+}
+
+int im_returns_finish(im_ctx *c, const double *global_sums)
+{
+    if (!c || !global_sums) return fail(c, IM_ERR_INVALID_ARG, "null ctx or sums");
+    if (!c->bound || !c->have_returns) return fail(c, IM_ERR_STATE, "im_returns_finish before im_returns");
+    // device order of the sums: {cost, sum U, sum U^2, count}; the job-wide ones live behind the ctx's own
+    const double dev[4] = {global_sums[0], global_sums[2], global_sums[3], global_sums[1]};
+    CUDA_TRY(c, cudaMemcpyAsync(c->sums + 4, dev, sizeof dev, cudaMemcpyHostToDevice, c->stream));   // pageable source: staged before the call returns
+    prof_begin(c, IM_KERNEL_RETURNS);
+    c->launches += launch_unorm(c->P, c->last_mu, c->sums + 4, c->stream);
+    prof_end(c);
+    CUDA_TRY(c, cudaGetLastError());
     return IM_OK;
 }
 
@@ -622,7 +638,7 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         if (!dst) return IM_OK;
         if (dst_bytes < 64) return fail(c, IM_ERR_CAPACITY, "dst too small");
         double s[8] = {0, 0, 0, 0, 0, 0, 0, 0}, out[8];
-        if (c->have_returns) CUDA_TRY(c, cudaMemcpy(s, c->sums, 32, cudaMemcpyDeviceToHost));
+        if (c->have_returns) CUDA_TRY(c, cudaMemcpy(s, c->sums + 4, 32, cudaMemcpyDeviceToHost));   // the sums in use: own, or the job's
         uint32_t ce[kRegions], cp[kRegions];
         if (int rc = read_counts(c, P.exec.cnt, ce)) return rc;
         if (int rc = read_counts(c, P.plan.cnt, cp)) return rc;
@@ -634,6 +650,17 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
         out[0] = cnt > 0 ? s[0] / cnt : 0.0; out[1] = mean; out[2] = std::sqrt(var); out[3] = s[0]; out[4] = cnt;
         out[5] = P.log_mode ? ne : -1.0; out[6] = P.log_mode ? np : -1.0; out[7] = (double)c->tick;
         memcpy(dst, out, 64);
+        return IM_OK;
+    }
+    case IM_TEL_SUMS: {
+        if (!c->have_returns) return fail(c, IM_ERR_STATE, "SUMS read before im_returns");
+        if (written) *written = 32;
+        if (!dst) return IM_OK;
+        if (dst_bytes < 32) return fail(c, IM_ERR_CAPACITY, "dst too small");
+        double s[4];
+        CUDA_TRY(c, cudaMemcpy(s, c->sums, 32, cudaMemcpyDeviceToHost));
+        const double out[4] = {s[0], s[3], s[1], s[2]};           // sum cost, n finalised, sum U, sum U^2
+        memcpy(dst, out, 32);
         return IM_OK;
     }
     case IM_TEL_DECISIONS_EXEC:
@@ -777,8 +804,10 @@ int im_device_ptr(im_ctx *c, uint32_t what, void **dev_ptr, size_t *bytes)
     case IM_TEL_VAL: *dev_ptr = c->P.val; *bytes = 4 * (T + 1) * E; break;
     case IM_TEL_DONE: *dev_ptr = c->P.done; *bytes = T * E; break;
     case IM_TEL_MISS: *dev_ptr = c->P.miss; *bytes = T * E; break;
-    case IM_TEL_ADV: *dev_ptr = c->adv; *bytes = 4 * T * E; break;
-    case IM_TEL_RET: *dev_ptr = c->ret; *bytes = 4 * T * E; break;
+    case IM_TEL_ADV:
+    case IM_TEL_RET:
+        if (!c->have_returns) return fail(c, IM_ERR_STATE, "ADV/RET before im_returns");
+        *dev_ptr = what == IM_TEL_ADV ? c->adv : c->ret; *bytes = 4 * T * E; break;
     default: return fail(c, IM_ERR_INVALID_ARG, "selector %u has no device array", what);
     }
     return IM_OK;

@@ -90,9 +90,10 @@ k_utility(const QLog ql, float mu, double *__restrict__ sums)
     }
 }
 
-// (U - mean) / (sigma + 1e-8), population sigma
+// (U - mean) / (sigma + 1e-8), population sigma, from the four sums {cost, count, sum U, sum U^2}[4..7] (the job-wide
+// sums of an env-sharded run, or a copy of the ctx's own).  U is recomputed from the record, so the pass can be repeated.
 __global__ void __launch_bounds__(256)
-k_unorm(const QLog ql, const double *__restrict__ sums)
+k_unorm(const QLog ql, float mu, const double *__restrict__ sums)
 {
     const uint32_t region = blockIdx.y;
     const uint32_t n = min(ql.cnt[region * kCntStride], ql.regcap);
@@ -103,8 +104,20 @@ k_unorm(const QLog ql, const double *__restrict__ sums)
     const float fm = (float)mean, fs = (float)(sqrt(var) + 1e-8);
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const size_t g = (size_t)region * ql.regcap + i;
-        ql.unorm[g] = __fdiv_rn(__fsub_rn(ql.unorm[g], fm), fs);
+        const uint4 rec = ql.rec[g];
+        const float U = __fsub_rn(__uint2float_rn((rec.w >> 16) & 1u),
+                                  __fdiv_rn(__fmul_rn(mu, __uint2float_rn(rec.z)), __uint2float_rn(rec.w & 0xFFFFu)));
+        ql.unorm[g] = __fdiv_rn(__fsub_rn(U, fm), fs);
     }
+}
+
+// sums[4..7] = the sums the normalisation uses: the ctx's own until im_returns_finish supplies the job's
+__global__ void k_copy_sums(double *sums) { if (threadIdx.x < 4) sums[4 + threadIdx.x] = sums[threadIdx.x]; }
+
+int launch_unorm(const Params &P, float mu, const double *sums_used, cudaStream_t st)
+{
+    k_unorm<<<dim3(32, kRegions), 256, 0, st>>>(P.qlog, mu, sums_used);
+    return 1;
 }
 
 int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu, float *adv, float *ret, double *sums, cudaStream_t st)
@@ -113,8 +126,9 @@ int launch_returns(const Params &P, uint32_t T, float gamma, float lam, float mu
     k_gae<<<(P.E + 127) / 128, 128, 0, st>>>(P.rew, P.cost, P.val, P.done, adv, ret, T, P.E, gamma, lam, mu, sums);
     const dim3 grid(32, kRegions);
     k_utility<<<grid, 256, 0, st>>>(P.qlog, mu, sums);
-    k_unorm<<<grid, 256, 0, st>>>(P.qlog, sums);
-    return 3;
+    k_copy_sums<<<1, 32, 0, st>>>(sums);
+    k_unorm<<<grid, 256, 0, st>>>(P.qlog, mu, sums + 4);
+    return 4;
 }
 
 // ------------------------------------------------------------------------------------------------------------------

@@ -340,11 +340,13 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                             OCC(gs >> 5) |= 1u << (gs & 31u);
                             const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
                             // prefill, then its first tick of service (R11)
-                            const uint32_t pf = (uint32_t)(((unsigned long long)s_prefill[k] * need) / 1000u);
+                            // (32-bit arithmetic throughout: prefill * need <= 5e7 by the spec check "prefill is sub-tick",
+                            // rate * usable <= 4e9, and fr * 2^16 / 10^6 = fr * 1024 / 15625 exactly, fr * 1024 < 2^30)
+                            const uint32_t pf = (s_prefill[k] * need) / 1000u;
                             const uint32_t usable = kDtUs - min(pf, kDtUs);
                             const uint32_t x = s_rate[k] * usable;
                             const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
-                            const uint32_t thr = (uint32_t)(((unsigned long long)fr << 16) / 1000000u);
+                            const uint32_t thr = (fr * 1024u) / 15625u;
                             const uint32_t u16 = u16_field(philox4x32_10_rk(gid, (uint32_t)t, gs >> 3, 0u, P.svc_rk), gs & 7u);
                             const uint32_t tok = min(bs + (u16 < thr ? 1u : 0u), rem0);
                             const uint32_t rem = rem0 - tok;

@@ -115,6 +115,48 @@ def test_env_id_base_shard_equals_full():
     a.close(); b.close()
 
 
+def test_two_shards_normalise_like_one_context():
+    """SURVEY 8(e) / PAPER.md:127-129: an env-sharded job must produce the single-GPU result.  Two contexts with
+    env_id_base 0 and E/2 stand in for two ranks: their IM_TEL_SUMS are added (the job's one all-reduce) and handed
+    to im_returns_finish; every rank's UNORM and scalars then equal those of one context over all envs."""
+    from paper_2606_11440_b200 import InfraMind
+    full = make_pool_spec(1, n_envs=64, n_ticks=200)
+    blob = make_policy_blob(full)
+    mu = 0.5
+    one = InfraMind(full, seed=0, debug_flags=1)
+    one.rollout(blob, 200); one.returns(0.99, 0.95, mu)
+    ref_q, ref_s = one.queries(unorm=True), one.scalars()
+    ref_sums = one.sums()
+    assert abs(ref_sums[0] - ref_s["sum_cost"]) < 1e-9 and int(ref_sums[1]) == ref_s["n_final"] > 200
+    parts = []
+    for base in (0, 32):
+        sh = full.with_(n_envs=32, env_id_base=base, env_level=full.env_level[base:base + 32].copy())
+        g = InfraMind(sh, seed=0, debug_flags=1)
+        g.rollout(blob, 200); g.returns(0.99, 0.95, mu)
+        parts.append(g)
+    local = [g.queries(unorm=True)["unorm"].copy() for g in parts]
+    total = parts[0].sums() + parts[1].sums()
+    assert np.allclose(total, ref_sums, rtol=1e-12, atol=1e-9)
+    # records with the same (env, arrive, sojourn, info) have the same utility: sort on those and compare in that order
+    order = lambda q: np.lexsort((q["info"], q["sojourn"], q["arrive"], q["env"]))
+    ro = order(ref_q)
+    moved = 0.0
+    for g, loc in zip(parts, local):
+        g.returns_finish(total)
+        q, sc = g.queries(unorm=True), g.scalars()
+        for k in ("cbar", "ubar", "usigma"):
+            assert abs(sc[k] - ref_s[k]) <= 1e-9 * max(1.0, abs(ref_s[k])), k
+        assert sc["n_final"] == ref_s["n_final"]
+        mine = ref_q["env"][ro] // 32 == (0 if g is parts[0] else 1)        # this shard's envs in the full run
+        go = order(q)
+        assert np.array_equal(q["sojourn"][go], ref_q["sojourn"][ro][mine]) and np.array_equal(q["info"][go], ref_q["info"][ro][mine])
+        assert np.max(np.abs(q["unorm"][go] - ref_q["unorm"][ro][mine])) <= 1e-6
+        moved = max(moved, float(np.max(np.abs(q["unorm"] - loc))))
+        g.close()
+    assert moved > 1e-4                      # the shard-local normalisation really was different
+    one.close()
+
+
 def test_determinism_and_split():
     from paper_2606_11440_b200 import InfraMind
     spec = make_pool_spec(3, n_envs=96, n_ticks=200)

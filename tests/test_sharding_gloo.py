@@ -1,6 +1,8 @@
 """N > 1 path on CPU: world_size 2 over gloo.  Each rank runs the oracle on its shard of the env ids (the product's
-sharding rule, paper_2606_11440_b200/sharding.py), the four sums are all-reduced, and the result must equal the
-unsharded run: trajectories column for column (R2: draws keyed by global env id), C-bar / U-bar / sigma_U to rounding."""
+sharding rule, paper_2606_11440_b200/sharding.py), the four sums of SURVEY 8(e) are all-reduced (the product's one
+collective, sharding.allreduce_sums), and the result must equal the unsharded run: trajectories column for column
+(R2: draws keyed by global env id), C-bar / U-bar / sigma_U to rounding.  What each rank does with the job-wide sums on
+the GPU (im_returns_finish) is covered by tests/test_gpu_parity.py::test_two_shards_normalise_like_one_context."""
 import os
 import socket
 
@@ -10,7 +12,7 @@ import torch.multiprocessing as mp
 
 from helpers import tiny_spec
 from im_workload import make_policy_blob
-from paper_2606_11440_b200.sharding import allreduce_scalars, combine_sums, partial_sums, shard_range, shard_spec
+from paper_2606_11440_b200.sharding import allreduce_sums, shard_range, shard_spec
 
 
 def _free_port():
@@ -35,9 +37,14 @@ def _worker(rank, world, port, out_dir):
     o = O.Oracle(mine, seed=7, env_ids=np.arange(base, base + cnt, dtype=np.uint32))
     o.rollout(blob, full.n_ticks, n_threads=1)
     o.returns(0.97, 0.9, 0.4)
-    red = allreduce_scalars(o.scalars(), device="cpu")
+    # the rank's four sums, from its own query log and cost array (what IM_TEL_SUMS holds on the GPU)
+    q = o.queries()
+    U = ((q["info"] >> 16) & 1).astype(np.float64) - 0.4 * q["sojourn"].astype(np.float64) / (q["info"] & 0xFFFF)
+    mine = np.array([o.cost().astype(np.float64).sum(), U.size, U.sum(), (U * U).sum()])
+    tot = allreduce_sums(mine, device="cpu")
+    ubar = tot[2] / tot[1]
     np.savez(os.path.join(out_dir, f"rank{rank}.npz"), rew=o.rew(), cost=o.cost(), adv=o.adv(), base=base, cnt=cnt,
-             cbar=red["cbar"], ubar=red["ubar"], usigma=red["usigma"], n_final=red["n_final"])
+             cbar=tot[0] / tot[1], ubar=ubar, usigma=np.sqrt(max(tot[3] / tot[1] - ubar * ubar, 0.0)), n_final=int(tot[1]))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -51,13 +58,14 @@ def test_shard_range_covers_everything_once():
         assert max(c for _, c in got) - min(c for _, c in got) <= 1
 
 
-def test_combine_sums_matches_direct_moments():
-    rng = np.random.default_rng(0)
-    u = rng.normal(0.3, 0.5, size=1000)
-    parts = [dict(sum_cost=float(i + 1), n_final=len(x), ubar=float(x.mean()), usigma=float(x.std())) for i, x in enumerate(np.split(u, [300, 650]))]
-    tot = np.sum([partial_sums(p) for p in parts], axis=0)
-    c = combine_sums(*tot)
-    assert c["n_final"] == 1000 and abs(c["ubar"] - u.mean()) < 1e-12 and abs(c["usigma"] - u.std()) < 1e-12 and abs(c["cbar"] - 6.0 / 1000) < 1e-15
+def test_shard_spec_sizes_caps_from_the_shards_own_levels():
+    """A utilisation sweep over contiguous shards: the last shard carries more load than the first, and its log
+    capacities follow; a capacity of 0 (library default) stays 0."""
+    full = tiny_spec(n_envs=64, N=2, n_ticks=100, qcap=16, rcap=64, rate_tick=[0.1, 0.2, 0.4, 0.8], slots=3, seed=5)
+    full = full.with_(env_level=(np.arange(64) * 4 // 64).astype(np.uint8), log_cap_exec=100000, log_cap_plan=0)
+    first, last = shard_spec(full, 0, 4), shard_spec(full, 3, 4)
+    assert last.log_cap_exec > 3 * first.log_cap_exec and first.log_cap_plan == 0 == last.log_cap_plan
+    assert first.env_id_base == 0 and last.env_id_base == 48 and first.n_envs == last.n_envs == 16
 
 
 def test_two_ranks_over_gloo_equal_the_unsharded_run(tmp_path):
