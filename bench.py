@@ -31,6 +31,16 @@ DEFAULT_CONFIG = 5
 GAMMA, LAM, MU = 0.99, 0.95, 0.5
 
 
+def csrc_sha():
+    """First 12 hex digits of the sha256 over the kernel sources (name-sorted): ties an ncu capture to the code it profiled."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2606_11440_b200", "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        h.update(name.encode()); h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:12]
+
+
 def _peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -93,7 +103,8 @@ def algorithmic_model(spec, counters_sum, T, E):
     n_run, n_wait = float(counters_sum[12]), float(counters_sum[13])
     n_exec, n_arr = float(counters_sum[11]), float(counters_sum[0])
     env_ticks = float(E) * T
-    sim_bytes = 8 * n_run + 4 * n_wait + (24 * N + 10) * env_ticks + 52 * n_exec + 16 * n_arr
+    serve_bytes = 8 * n_run                                     # k_serve: the slots of the running requests, read + write
+    sim_bytes = 4 * n_wait + (24 * N + 10) * env_ticks + 52 * n_exec + 16 * n_arr   # k_sim: everything else of SURVEY 8(d)
     F, H = spec.f_in, spec.hidden
     mac_exec = F * H + H * H + H * (3 * N + 1)
     mac_plan = F * H + H * H + H * 24
@@ -101,9 +112,16 @@ def algorithmic_model(spec, counters_sum, T, E):
     plan_flops = 2.0 * mac_plan * float(counters_sum[10])
     exec_bytes = (24 + 4) * n_exec + (12 * N + 4) * (env_ticks + E)   # row r/w + snapshot read + val write
     plan_bytes = (20 + 24) * float(counters_sum[10])
-    ret_bytes = 21.0 * env_ticks
-    return dict(sim_bytes=sim_bytes, exec_flops=exec_flops, plan_flops=plan_flops, exec_bytes=exec_bytes, plan_bytes=plan_bytes,
+    # returns: GAE reads 13 B and writes 8 B per env-tick; the utility pass reads a 16-byte query record, the
+    # normalisation pass reads it again and writes 4 B (R32)
+    ret_bytes = 21.0 * env_ticks + 36.0 * float(counters_sum[2])
+    return dict(sim_bytes=sim_bytes, serve_bytes=serve_bytes, exec_flops=exec_flops, plan_flops=plan_flops, exec_bytes=exec_bytes, plan_bytes=plan_bytes,
                 ret_bytes=ret_bytes, n_exec=n_exec, n_plan=float(counters_sum[10]), env_ticks=env_ticks)
+
+
+def baseline_sample(cfg: int, cores: int):
+    """(envs, ticks) of the bounded sample the oracle is timed on: the first envs x the first ticks of the config."""
+    return max(cores * 4, 32), {1: 200, 2: 500, 3: 300, 4: 200, 5: 512}[cfg]
 
 
 def run_reference(args, rank, world):
@@ -114,8 +132,7 @@ def run_reference(args, rank, world):
     cfg = args.config
     full = CONFIGS[cfg]
     cores = os.cpu_count() or 1
-    n_envs = {1: 64, 2: 64, 3: 16, 4: 8, 5: 16}[cfg]
-    T = {1: 200, 2: 400, 3: 200, 4: 100, 5: 128}[cfg]
+    n_envs, T = baseline_sample(cfg, cores)              # the same sample as the cpu_baseline leg of the main arm
     spec = make_pool_spec(cfg, n_envs=n_envs, n_ticks=T)
     blob = make_policy_blob(spec)
     o = O.Oracle(spec, seed=0)
@@ -147,8 +164,7 @@ def cpu_baseline(cfg: int, budget_s: float = 15.0):
     """The oracle timed on the host cores on a bounded sample of the same workload (about 10-30 s of CPU work)."""
     from oracle import oracle as O
     cores = os.cpu_count() or 1
-    n_envs = max(cores * 4, 32)
-    T = {1: 200, 2: 500, 3: 300, 4: 200, 5: 512}[cfg]
+    n_envs, T = baseline_sample(cfg, cores)
     full = CONFIGS[cfg]
     spec = make_pool_spec(cfg, n_envs=n_envs, n_ticks=T)
     blob = make_policy_blob(spec)
@@ -191,6 +207,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2606_11440_b200 import (InfraMind, IM_TEL_ADV, IM_TEL_RET, IM_TEL_SCALARS, build)
+    from paper_2606_11440_b200.sharding import allreduce_sums
     build.build()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
@@ -225,6 +242,10 @@ def main():
             n = min(chunk, T - done)
             c.rollout(blob, n)
             c.returns(GAMMA, LAM, MU)
+            if world > 1:
+                # the step's one collective: the four sums behind C-bar / U-bar / sigma_U over all ranks;
+                # every rank then re-normalises its UNORM with the job's statistics inside the library
+                c.returns_finish(allreduce_sums(c.sums(), device=dev))
             done += n
         return c
 
@@ -260,11 +281,6 @@ def main():
         tms = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tms, op=dist.ReduceOp.MAX)
         ms = float(tms.item())
-        # the step's one collective: the four sums behind C-bar / U-bar / sigma_U over all ranks;
-        # every rank then re-normalises its UNORM with the job's statistics inside the library
-        from paper_2606_11440_b200.sharding import allreduce_sums
-        last.returns_finish(allreduce_sums(last.sums(), device=dev))
-        sc = last.scalars()
     ms_per_step = ms / args.steps
     env_ticks_per_s = world * E * T / (ms_per_step * 1e-3)
     model = algorithmic_model(spec, csum, T, E)
@@ -276,49 +292,62 @@ def main():
     ksteps = max(1, min(args.steps, 2))
     for i in range(ksteps):
         cprof = step(args.warmup + args.steps + i, blob_dev)
-    kt = {"sim": [0.0, 0], "plan": [0.0, 0], "exec": [0.0, 0], "returns": [0.0, 0]}
+    kt = {"sim": [0.0, 0], "plan": [0.0, 0], "exec": [0.0, 0], "returns": [0.0, 0], "serve": [0.0, 0]}
     for c in ctxs:
         for k, (m, n) in c.kernel_times().items():
             kt[k][0] += m; kt[k][1] += n
         c.set_profiling(False)
     tot_k = sum(v[0] for v in kt.values()) or 1.0
     share = {k: v[0] / tot_k for k, v in kt.items()}
-    dominant = max(("sim", "plan", "exec"), key=lambda k: kt[k][0])
+    dominant = max(("sim", "serve", "plan", "exec"), key=lambda k: kt[k][0])
     per_launch_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in kt.items()}
-    n_l = {k: (kt[k][1] / ksteps if kt[k][1] else 1.0) for k in kt}
+    n_l = {k: (kt[k][1] / ksteps if kt[k][1] else 1.0) for k in kt}      # launches (timed brackets) of the class per step
     bf16 = spec.policy_dtype == 1
-    if dominant == "sim":
-        achieved = model["sim_bytes"] / n_l["sim"] / (per_launch_ms["sim"] * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k_sim", "achieved": achieved, "peak": peaks["hbm"], "unit": "GB/s", "frac": achieved / peaks["hbm"], "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
+    tunit = "GB per launch (ncu dram__bytes_read+write)"
+    if dominant in ("sim", "serve"):
+        achieved = model[dominant + "_bytes"] / n_l[dominant] / (per_launch_ms[dominant] * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_" + dominant, "achieved": achieved, "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm"], "traffic": None, "traffic_unit": tunit}
     else:
         fl = model["exec_flops"] if dominant == "exec" else model["plan_flops"]
         achieved = fl / n_l[dominant] / (per_launch_ms[dominant] * 1e-3) / 1e12
         if bf16:
             pk = peaks["bf16_sustained"]
-            roof = {"bound": "tensor", "kernel": f"k_policy_bf16<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
+            kname = ("k_policy_tc" if spec.hidden == 256 else "k_policy_bf16") + f"<{dominant}>"
+            roof = {"bound": "tensor", "kernel": kname, "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": tunit}
         else:
             pk = 148 * 128 * 2 * 1.965e9 / 1e12       # fp32 FFMA: 148 SMs x 128 lanes x 2 flop x max clock
-            roof = {"bound": "alu", "kernel": f"k_policy_f32<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": "GB per launch (ncu dram__bytes_read+write)"}
-    # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this command, if any
+            roof = {"bound": "alu", "kernel": f"k_policy_f32<{dominant}>", "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": tunit}
+    # DRAM bytes per launch of the dominant kernel: taken from the committed ncu --set full capture only if that capture was
+    # made from the kernel sources this run was built from (sha256 of csrc/, first 12 hex digits); otherwise null
     try:
         import csv
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
             for row in csv.DictReader(f):
-                if row["config"] == f"cfg{cfg}" and row["kernel"] == roof["kernel"].split("<")[0] and E == CONFIGS[cfg]["E"]:
+                if (row["config"] == f"cfg{cfg}" and row["kernel"] == roof["kernel"].split("<")[0] and E == CONFIGS[cfg]["E"]
+                        and row["csrc_sha"] == csrc_sha()):
                     roof["traffic"] = float(row["dram_bytes_per_launch"]) / 1e9
                     roof["traffic_source"] = row["source"]
     except (OSError, ValueError, KeyError):
         pass
+    roof["csrc_sha"] = csrc_sha()
     roof["peak_source"] = f"MEASURED_PEAKS.json ({peaks['src']})"
     roof["kernel_share_of_step"] = share
     roof["kernel_ms_per_launch"] = per_launch_ms
-    hbm_frac_sim = model["sim_bytes"] / n_l["sim"] / max(per_launch_ms["sim"] * 1e-3, 1e-12) / 1e9 / peaks["hbm"]
-    roof["sim_hbm_frac"] = hbm_frac_sim
-    roof["step_hbm_frac"] = (model["sim_bytes"] + model["exec_bytes"] + model["plan_bytes"] + model["ret_bytes"]) / (ms_per_step * 1e-3) / 1e9 / peaks["hbm"]
+    per_s = lambda key, cls: model[key] / n_l[cls] / max(per_launch_ms[cls] * 1e-3, 1e-12)
+    roof["sim_hbm_frac"] = per_s("sim_bytes", "sim") / 1e9 / peaks["hbm"]
+    roof["serve_hbm_frac"] = per_s("serve_bytes", "serve") / 1e9 / peaks["hbm"]
+    # the tick simulation as a whole (k_serve + k_sim: the SURVEY 8(d) byte formula over both kernels' time)
+    t_tick = per_launch_ms["sim"] * n_l["sim"] + per_launch_ms["serve"] * n_l["serve"]
+    roof["tick_sim_hbm_frac"] = (model["sim_bytes"] + model["serve_bytes"]) / max(t_tick * 1e-3, 1e-12) / 1e9 / peaks["hbm"]
+    roof["exec_tensor_frac"] = per_s("exec_flops", "exec") / 1e12 / peaks["bf16_sustained"] if bf16 else None
+    roof["plan_tensor_frac"] = per_s("plan_flops", "plan") / 1e12 / peaks["bf16_sustained"] if bf16 else None
+    roof["step_hbm_frac"] = (model["sim_bytes"] + model["serve_bytes"] + model["exec_bytes"] + model["plan_bytes"] + model["ret_bytes"]) / (ms_per_step * 1e-3) / 1e9 / peaks["hbm"]
     roof["step_tensor_frac"] = (model["exec_flops"] + model["plan_flops"]) / (ms_per_step * 1e-3) / 1e12 / peaks["bf16_sustained"] if bf16 else None
     # t_lb / t, t_lb = the larger of the two bound times of the whole step
     roof["step_lb_frac"] = max(roof["step_hbm_frac"], roof["step_tensor_frac"] or 0.0)
-    roof["returns_hbm_frac"] = model["ret_bytes"] / max(per_launch_ms["returns"] * 1e-3, 1e-12) / 1e9 / peaks["hbm"]
+    # one im_returns call covers one rollout call (chunk): bytes of that call over the time of that call
+    roof["returns_hbm_frac"] = per_s("ret_bytes", "returns") / 1e9 / peaks["hbm"]
 
     # ---- end to end through the C ABI with HOST buffers: host blob in, ADV / RET / scalars out to pinned host memory
     adv_h = torch.empty((chunk, E), dtype=torch.float32, pin_memory=True)

@@ -88,8 +88,9 @@ typedef struct im_pool_spec {
     uint32_t depth_median_tok[3];    /* output-token medians per depth (R18) */
     uint32_t mix_lo[2], mix_hi[2];   /* budget components, ticks, inclusive (R7); hi <= 65535 */
     uint32_t reserved;
-    uint64_t log_cap_exec;           /* capacity (rows) of the executor decision log / work list */
-    uint64_t log_cap_plan;           /* capacity (rows) of the planner decision log / work list */
+    uint64_t log_cap_exec;           /* rows of the executor decision log of one im_rollout (0 = default); used only with
+                                        IM_FLAG_LOG_DECISIONS: without it the work list is a ring sized by the library */
+    uint64_t log_cap_plan;           /* the same for the planner */
     uint64_t log_cap_query;          /* capacity (records) of the finished-query log */
     im_model_spec model[IM_MAX_MODELS];
     const uint32_t *out_tok_mult_q16;/* HOST [1024]: Q16 output-token multipliers (lognormal quantiles, R18) */
@@ -116,7 +117,9 @@ int im_reset(im_ctx *ctx);
 
 /* Advance every env by n_ticks <= max_ticks fixed 50 ms ticks under the given policy (canonical tick
  * A..I of DESIGN.md).  `policy_weights` is the R26 blob, HOST or DEVICE pointer (detected; a host blob is
- * copied before the call returns).  Overwrites trajectory rows 0..n_ticks-1 (row n_ticks of VAL = bootstrap
+ * checked and copied before the call returns, pinned or not; a device blob must stay valid until the stream has
+ * passed the call, and a header that does not match the spec surfaces as IM_ERR_BAD_SPEC at the next
+ * im_read_telemetry).  Overwrites trajectory rows 0..n_ticks-1 (row n_ticks of VAL = bootstrap
  * value) and the decision / query logs.  Env state persists across calls (split-invariance, P15).
  * Asynchronous on the bound stream. */
 int im_rollout(im_ctx *ctx, const void *policy_weights, uint32_t n_ticks);
@@ -188,11 +191,12 @@ uint64_t im_launch_count(const im_ctx *ctx);
 /* Per-kernel-class device timing for roofline reports: when enabled, every launch of im_rollout / im_returns is
  * bracketed by CUDA events on the bound stream. im_kernel_times synchronises, returns the accumulated
  * milliseconds and launch counts per class since the last call, and clears them. HOST arrays of IM_KERNEL_CLASSES. */
-#define IM_KERNEL_SIM 0       /* k_sim: tick phases A, B, D-issue .. I */
+#define IM_KERNEL_SIM 0       /* k_sim: tick phases A, B, D-issue, E, G .. I */
 #define IM_KERNEL_PLAN 1      /* planner MLP + sampling */
 #define IM_KERNEL_EXEC 2      /* executor + critic MLP + sampling */
 #define IM_KERNEL_RETURNS 3   /* GAE + utility kernels of one im_returns */
-#define IM_KERNEL_CLASSES 4
+#define IM_KERNEL_SERVE 4     /* k_serve: tick phase F (token-level service pass) */
+#define IM_KERNEL_CLASSES 5
 int im_set_profiling(im_ctx *ctx, int enable);
 int im_kernel_times(im_ctx *ctx, double *ms, uint64_t *launches);
 

@@ -256,11 +256,11 @@ class InfraMind:
         self._check(self._L.im_set_profiling(self._h, 1 if on else 0))
 
     def kernel_times(self):
-        """{'sim': (ms, launches), 'plan': ..., 'exec': ..., 'returns': ...} since the last call."""
-        ms = (C.c_double * 4)()
-        n = (C.c_uint64 * 4)()
+        """{'sim': (ms, launches), 'plan': ..., 'exec': ..., 'returns': ..., 'serve': ...} since the last call."""
+        ms = (C.c_double * 5)()
+        n = (C.c_uint64 * 5)()
         self._check(self._L.im_kernel_times(self._h, ms, n))
-        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("sim", "plan", "exec", "returns"))}
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(("sim", "plan", "exec", "returns", "serve"))}
 
     @property
     def launches(self) -> int:

@@ -60,6 +60,14 @@ __global__ void k_gather_words(const Params P, uint32_t off, uint32_t w0, uint32
     }
 }
 
+// a DEVICE blob cannot be checked on the host without a synchronisation: its header is checked here and a mismatch
+// raises bit 16 of the error flag (IM_ERR_BAD_SPEC at the next im_read_telemetry)
+__global__ void k_check_blob(const uint32_t *h, uint32_t dtype, uint32_t F, uint32_t H, uint32_t n_exec_out, uint32_t *err_flag)
+{
+    if (threadIdx.x == 0 && (h[0] != 0x494D5042u || h[1] != dtype || h[2] != F || h[3] != H || h[4] != 24u || h[5] != n_exec_out))
+        atomicOr(err_flag, 16u);
+}
+
 // repack the R26 blob (device copy) into the kernels' layouts
 __global__ void k_repack(const uint8_t *blob, uint32_t dtype, uint32_t F, uint32_t H, uint32_t n_out, uint32_t n_out_pad,
                          size_t off_W1, size_t off_b1, size_t off_W2, size_t off_b2, size_t off_W3, size_t off_b3,
@@ -102,6 +110,7 @@ struct im_ctx {
     Weights Wp, We;
     uint8_t *d_blob = nullptr;
     size_t blob_bytes = 0;
+    std::vector<uint8_t> blob_stage;
     float *adv = nullptr, *ret = nullptr;
     double *sums = nullptr;
     uint32_t *qorder = nullptr;
@@ -120,8 +129,8 @@ struct im_ctx {
     std::vector<cudaEvent_t> ev;
     std::vector<int> ev_class;
     size_t ev_used = 0;
-    double prof_ms[IM_KERNEL_CLASSES] = {0, 0, 0, 0};
-    uint64_t prof_n[IM_KERNEL_CLASSES] = {0, 0, 0, 0};
+    double prof_ms[IM_KERNEL_CLASSES] = {0, 0, 0, 0, 0};
+    uint64_t prof_n[IM_KERNEL_CLASSES] = {0, 0, 0, 0, 0};
 };
 
 static void prof_begin(im_ctx *c, int cls)
@@ -473,7 +482,16 @@ static int upload_weights(im_ctx *c, const void *blob)
             h[5] != 3 * c->spec.n_models + 1)
             return fail(c, IM_ERR_BAD_SPEC, "policy blob header does not match the spec");
     }
-    CUDA_TRY(c, cudaMemcpyAsync(c->d_blob, blob, c->blob_bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (on_device) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_blob, blob, c->blob_bytes, cudaMemcpyDeviceToDevice, c->stream));
+        k_check_blob<<<1, 32, 0, c->stream>>>((const uint32_t *)c->d_blob, c->spec.policy_dtype, c->spec.f_in, c->spec.hidden, 3 * c->spec.n_models + 1, c->P.err_flag);
+        c->launches++;
+    } else {
+        // "a host blob is copied before the call returns": a pinned source would make the async copy truly asynchronous,
+        // so the bytes go through a buffer the ctx owns (pageable: the runtime stages it before returning)
+        c->blob_stage.assign((const uint8_t *)blob, (const uint8_t *)blob + c->blob_bytes);
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_blob, c->blob_stage.data(), c->blob_bytes, cudaMemcpyHostToDevice, c->stream));
+    }
     auto pad16 = [](size_t n) { return (n + 15) & ~(size_t)15; };
     const size_t F = c->spec.f_in, H = c->spec.hidden, ws = c->spec.policy_dtype ? 2 : 4;
     size_t off = 32;
@@ -532,8 +550,10 @@ int im_rollout(im_ctx *c, const void *policy_weights, uint32_t n_ticks)
         prof_end(c);
         c->par_exec ^= 1;
         const bool last = (i + 1 == n_ticks);
-        prof_begin(c, IM_KERNEL_SIM);
+        prof_begin(c, IM_KERNEL_SERVE);
         launch_serve(P, t, st);                                             // F of tick t
+        prof_end(c);
+        prof_begin(c, IM_KERNEL_SIM);
         launch_sim(P, t, i, t + 1, last ? 2u : 1u, t0, st);                 // D-issue, E, G .. I of tick t, A, B of tick t+1
         prof_end(c);
         c->launches += 4;
@@ -582,6 +602,7 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
     const Params &P = c->P;
     uint32_t flag = 0;
     CUDA_TRY(c, cudaMemcpy(&flag, P.err_flag, 4, cudaMemcpyDeviceToHost));
+    if (flag & 16u) return fail(c, IM_ERR_BAD_SPEC, "device policy blob header does not match the spec");
     if (flag) return fail(c, IM_ERR_CAPACITY, "log / work-list overflow during rollout (flag %u): raise log_cap_*", flag);
     const size_t E = c->E, T = c->last_T, N = P.N, Q = P.QCAP, R = P.RCAP;
     switch (what) {

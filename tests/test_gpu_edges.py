@@ -86,3 +86,33 @@ def test_arrival_bursts_of_sixteen_and_more():
         before = now
     g.close()
     assert burst >= 16
+
+
+def test_device_blob_of_another_spec_is_rejected():
+    """A DEVICE blob cannot be checked on the host without a synchronisation: its header is checked on the device and the
+    mismatch surfaces as IM_ERR_BAD_SPEC at the next read; ADV / RET device pointers need im_returns first."""
+    import torch
+    from im_workload import make_pool_spec
+    from paper_2606_11440_b200 import InfraMind, IMError, IM_TEL_ADV
+    spec = make_pool_spec(1, n_envs=8, n_ticks=10)
+    g = InfraMind(spec, seed=0, debug_flags=1)
+    with pytest.raises(IMError) as ei:
+        g.device_tensor(IM_TEL_ADV, torch.float32)
+    assert ei.value.code == -5
+    other = make_policy_blob(make_pool_spec(3, n_envs=8, n_ticks=10))
+    good = make_policy_blob(spec)
+    bad = torch.from_numpy(np.resize(other, good.size)).cuda()
+    g.rollout(bad, 2)
+    with pytest.raises(IMError) as ei:
+        g.rew()
+    assert ei.value.code == -2
+    g.close()
+    # a pinned host blob may be overwritten right after the call returns
+    g = InfraMind(spec, seed=0, debug_flags=1)
+    pin = torch.from_numpy(good.copy()).pin_memory()
+    g.rollout(pin.numpy(), 10)
+    pin.zero_()
+    a = g.rew().copy(); c1 = g.counters().copy()
+    g.reset(); g.rollout(good, 10)
+    assert np.array_equal(a, g.rew()) and np.array_equal(c1, g.counters())
+    g.close()
