@@ -181,6 +181,21 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
     uint32_t *qready = reinterpret_cast<uint32_t *>(blkp + P.off_qready) + lane;        // word w at qready[w * 32]
     uint32_t *ctr = reinterpret_cast<uint32_t *>(blkp + P.off_ctr) + lane;              // counter c at ctr[c * 32]
 
+    // The arrival count of tick t_pre (R5) depends on nothing but (env, tick): one Philox call and a binary search of
+    // the level's CDF row (count = #{j < 31 : x >= cdf[j]}; the row is monotone, so it is the first j with x < cdf[j]).
+    // Done here, its loads overlap the header's flight.
+    uint32_t n_arr_pre = 0;
+    if (pre_mode == 1 && active) {
+        const uint32_t xr = draw(P, STREAM_ARR, gid, t_pre, 0u, 0).x;
+        const uint32_t *cdf = P.tab_cdf + 32u * P.env_level[e];
+        uint32_t lo = 0, hi = 31;
+#pragma unroll
+        for (int s = 0; s < 5; s++) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (lo < hi) { if (xr >= __ldg(&cdf[mid])) lo = mid + 1; else hi = mid; }
+        }
+        n_arr_pre = lo;
+    }
     // counters of this launch (named registers: every site is static)
     uint32_t c_arr = 0, c_drop = 0, c_fin = 0, c_solved = 0, c_missed = 0, c_issued = 0, c_done = 0, c_preempt = 0, c_soj = 0,
              c_live = 0, c_plans = 0, c_run = 0, c_wait = 0, c_aband = 0;
@@ -278,6 +293,11 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
 #pragma unroll
             for (uint32_t k = 0; k < kMaxModels; k++) kvt[k] = k < N ? kvs[k * 32u] : 0u;
         }
+        // the first four issue records, fetched before their count is known (it sits in the header still in flight)
+        const uint2 *iss = reinterpret_cast<const uint2 *>(blkp + P.off_iss) + lane;
+        uint2 r[4];
+#pragma unroll
+        for (uint32_t i = 0; i < 4; i++) r[i] = iss[i * 32u];
         bulk::mbar_wait(&s_bar[wib], 0);
 
         // =============================================================== D-issue (R18): the new calls join the waiting list
@@ -286,12 +306,12 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         {
             uint32_t icnt = H(P.hw_misc + 1u);
             if (icnt > kIssueCap) icnt = kIssueCap;              // the executor kernel flags the overflow (err_flag)
-            const uint2 *iss = reinterpret_cast<const uint2 *>(blkp + P.off_iss) + lane;
 #pragma unroll 1
             for (uint32_t j0 = 0; j0 < icnt; j0 += 4) {            // four records in flight per lane
-                uint2 r[4];
+                if (j0) {
 #pragma unroll
-                for (uint32_t i = 0; i < 4; i++) if (j0 + i < icnt) r[i] = iss[(j0 + i) * 32u];
+                    for (uint32_t i = 0; i < 4; i++) if (j0 + i < icnt) r[i] = iss[(j0 + i) * 32u];
+                }
 #pragma unroll
                 for (uint32_t i = 0; i < 4; i++)
                     if (j0 + i < icnt)   // issue = t, remaining = out_total
@@ -315,20 +335,41 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
             while (__any_sync(kFull, madm != 0)) {
                 if (madm) {
                     const uint32_t k = (uint32_t)__ffs(madm) - 1u;
-                    // the entry that will fill the hole if the head of the queue is admitted (last of the head chunk):
-                    // its address is known now, so it is fetched together with the keys
-                    const uint32_t n0 = M_W0(k) & 0xFFFFu;
-                    const uint32_t lj = byte_get(HEADW(k), k) * kChunk + ((n0 - 1u) & (kChunk - 1u));
-                    const uint32_t lk = wkey[lj];
-                    const uint2 la = waux[lj];
-                    uint32_t key, bunit;
-                    list_min(k, key, bunit);
+                    const uint32_t n0 = M_W0(k) & 0xFFFFu, hc = byte_get(HEADW(k), k);
+                    uint32_t key, j = 0, lk;
+                    uint2 wa = make_uint2(0, 0), la;
+                    if (n0 <= 4u) {
+                        // a short queue (the usual case below saturation) is the first n0 entries of its head chunk: keys and
+                        // aux words come in ONE round trip (entries beyond n0 hold 0xFFFFFFFF)
+                        const uint4 ku = *reinterpret_cast<const uint4 *>(wkey + hc * kChunk);
+                        const uint4 a01 = *reinterpret_cast<const uint4 *>(waux + hc * kChunk), a23 = *reinterpret_cast<const uint4 *>(waux + hc * kChunk + 2);
+                        uint32_t p = 0;
+                        key = ku.x;
+                        if (ku.y < key) { key = ku.y; p = 1; }
+                        if (ku.z < key) { key = ku.z; p = 2; }
+                        if (ku.w < key) { key = ku.w; p = 3; }
+                        j = hc * kChunk + p;
+                        wa = p == 0 ? make_uint2(a01.x, a01.y) : (p == 1 ? make_uint2(a01.z, a01.w) : (p == 2 ? make_uint2(a23.x, a23.y) : make_uint2(a23.z, a23.w)));
+                        const uint32_t lp = n0 - 1u;             // the entry that fills the hole: the last one
+                        lk = lp == 0 ? ku.x : (lp == 1 ? ku.y : (lp == 2 ? ku.z : ku.w));
+                        la = lp == 0 ? make_uint2(a01.x, a01.y) : (lp == 1 ? make_uint2(a01.z, a01.w) : (lp == 2 ? make_uint2(a23.x, a23.y) : make_uint2(a23.z, a23.w)));
+                    } else {
+                        // the entry that will fill the hole if the head of the queue is admitted (last of the head chunk):
+                        // its address is known now, so it is fetched together with the keys
+                        const uint32_t lj = hc * kChunk + ((n0 - 1u) & (kChunk - 1u));
+                        lk = wkey[lj];
+                        la = waux[lj];
+                        uint32_t bunit;
+                        list_min(k, key, bunit);
+                        if (key != ~0u) {
+                            // position of the key inside its unit (keys are unique)
+                            const uint4 bu = *reinterpret_cast<const uint4 *>(wkey + bunit * 4u);
+                            j = bunit * 4u + (bu.x == key ? 0u : (bu.y == key ? 1u : (bu.z == key ? 2u : 3u)));
+                            wa = waux[j];
+                        }
+                    }
                     bool again = false;
                     if (key != ~0u) {
-                        // position of the key inside its unit (keys are unique)
-                        const uint4 bu = *reinterpret_cast<const uint4 *>(wkey + bunit * 4u);
-                        const uint32_t j = bunit * 4u + (bu.x == key ? 0u : (bu.y == key ? 1u : (bu.z == key ? 2u : 3u)));
-                        const uint2 wa = waux[j];
                         const uint32_t sw = wa.y, rem0 = wa.x >> 16, id = key & 0xFFFu;
                         const uint32_t need = ((sw >> SW_IN_SHIFT) & SW_TOK_MASK) + ((sw & SW_TOK_MASK) - rem0);     // R12
                         const uint32_t w0 = M_W0(k), nr = w0 >> 16, kv = M_KV(k), slots = s_slots[k];
@@ -634,19 +675,7 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         }
         // ---- A arrive (R5, R7, R8, R9)
         {
-            const uint32_t xr = draw(P, STREAM_ARR, gid, t, 0u, 0).x;
-            uint32_t n = 0;
-            if (active) {
-                // count = #{j < 31 : x >= cdf[j]}; the row is monotone, so it is the first j with x < cdf[j]
-                const uint32_t *cdf = P.tab_cdf + 32u * P.env_level[e];
-                uint32_t lo = 0, hi = 31;
-#pragma unroll
-                for (int s = 0; s < 5; s++) {
-                    const uint32_t mid = (lo + hi) >> 1;
-                    if (lo < hi) { if (xr >= __ldg(&cdf[mid])) lo = mid + 1; else hi = mid; }
-                }
-                n = lo;
-            }
+            const uint32_t n = n_arr_pre;                                // drawn at the top of the kernel
             // the j-th arrival takes the j-th lowest free query index; a full table drops the rest (R9)
             uint32_t nfree = 0;
 #pragma unroll 1
@@ -701,10 +730,15 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 stage[lane * 9u + j] = v;
             }
             __syncwarp();
+            // lane l copies feature (l & 7) of envs (l >> 3), (l >> 3) + 4, ...: eight lanes write one 32-byte sector
+            {
+                const uint32_t j = lane & 7u, env0 = lane >> 3;
+                const float *src = stage + env0 * 9u + j;
+                float *dst = snb + env0 * N3 + f0 + j;
+                const bool jok = f0 + j < N3;
 #pragma unroll
-            for (uint32_t i = 0; i < 8; i++) {
-                const uint32_t idx = i * 32u + lane, env = idx >> 3, j = idx & 7u;
-                if (env < n_valid && f0 + j < N3) snb[env * N3 + f0 + j] = stage[env * 9u + j];
+                for (uint32_t i = 0; i < 8; i++)
+                    if (jok && env0 + 4u * i < n_valid) dst[4u * i * N3] = src[36u * i];
             }
             __syncwarp();
         }
