@@ -585,17 +585,20 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     extern __shared__ __align__(1024) uint8_t smem_tc[];
     __shared__ TileSched sched;
     __shared__ uint64_t bars[5];                          // layer 1 half a / b, layer 2 half a / b, layer 3
+    __shared__ uint64_t wbar;                             // arrival of the weight image
     __shared__ uint32_t tmem_slot;
     uint8_t *img = smem_tc, *a1 = smem_tc + ((Net::kImageBytes + 1023u) & ~1023u);
     TcRowSlot *rowbuf = reinterpret_cast<TcRowSlot *>(a1 + Net::kA1Bytes);     // [2][128]
-    {
-        const uint4 *src = reinterpret_cast<const uint4 *>(W.tc_img);
-        uint4 *dst = reinterpret_cast<uint4 *>(img);
-        for (uint32_t i = threadIdx.x; i < Net::kImageBytes / 16; i += kTcThreads) dst[i] = __ldg(src + i);
-    }
+    // the weight image (194 KB) comes by bulk async copies (TMA): one thread issues them, they fly while the CTA allocates
+    // its tensor memory, builds the tile schedule and gathers its first tile; everybody waits on wbar before the first use
     if (threadIdx.x == 0) {
         for (int i = 0; i < 5; i++) tc::mbar_init(&bars[i], 1);
+        tc::mbar_init(&wbar, 1);
         tc::mbar_fence_init();
+        bulk::mbar_expect_tx(&wbar, Net::kImageBytes);
+        constexpr uint32_t kPiece = 48 * 1024;
+        for (uint32_t o = 0; o < Net::kImageBytes; o += kPiece)
+            bulk::g2s(img + o, W.tc_img + o, Net::kImageBytes - o < kPiece ? Net::kImageBytes - o : kPiece, &wbar);
     }
     if (threadIdx.x < 32) tc::tmem_alloc(&tmem_slot, Net::kTmemCols);
     const RowBuf &rb = EXEC ? P.exec : P.plan;
@@ -677,11 +680,13 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             build_a1(nxt, sn, rowbuf);
             tc::fence_proxy_async_smem();
             tc::bar_sync(4, 128);
+            tc::mbar_wait(&wbar, 0);
             if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
             nxt = tc_fetch_row(sched, rb, blockIdx.x + gridDim.x, r, n_crit);
             fetch_snap(nxt, sn);
         }
     }
+    tc::mbar_wait(&wbar, 0);
     for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
         if (wg == 1) {
             // ---- warpgroup 1: tanh of layer 1, packed in place (half a while the tensor core computes half b)
