@@ -319,6 +319,9 @@ __device__ __forceinline__ void s2g(void *dst_gmem, const void *src_smem, uint32
 }
 __device__ __forceinline__ void commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// the source (shared memory) of every committed bulk store has been read: enough before the CTA exits, the end of the
+// kernel orders the writes themselves
+__device__ __forceinline__ void wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 }  // namespace bulk
 

@@ -31,17 +31,15 @@ constexpr int kSimWarps = 2;            // 32-env blocks per CTA
 constexpr int kServeWarps = 8;
 constexpr uint32_t kFull = 0xffffffffu;
 
-// per-warp dynamic shared memory of k_sim: header [hdr_words][32] | completion masks [cm_words][32] (one bulk copy);
-// the snapshot is staged in [32][9] words: over the completion masks (done with by then) when they are large enough
-struct SimSmem { uint32_t hdr_bytes, o_cm, o_stage, tma_bytes, per_warp; };
+// per-warp dynamic shared memory of k_sim: header [hdr_words][32] | completion masks [cm_words][32] (one bulk copy)
+struct SimSmem { uint32_t hdr_bytes, o_cm, tma_bytes, per_warp; };
 static SimSmem sim_smem(const Params &P)
 {
     SimSmem L;
     L.hdr_bytes = P.hdr_words * 128u;
     L.o_cm = L.hdr_bytes;
     L.tma_bytes = L.o_cm + P.cm_words * 128u;
-    L.o_stage = P.cm_words >= 9u ? L.o_cm : L.tma_bytes;
-    L.per_warp = P.cm_words >= 9u ? L.tma_bytes : L.tma_bytes + 9u * 128u;
+    L.per_warp = L.tma_bytes;
     return L;
 }
 
@@ -710,37 +708,29 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
             if (active) c_live += P.QCAP - (nfree - n_ok);
         }
     }
-    // ---- B snapshot (R14): telemetry features of the state left by the tick just finished.  A lane holds the 3N
-    // features of ITS env, the policy kernels want them contiguous per env: eight features at a time go through a
-    // [32][9] staging tile, so that the stores are whole 32-byte sectors (eight lanes per env) instead of 3N scattered words
+    // ---- B snapshot (R14): telemetry features of the state left by the tick just finished.  The policy kernels want
+    // the 3N features of an env contiguous; the header sits in shared memory as [word][env], so any lane can read any
+    // env's words: lane l takes feature (l & 7) of envs (l >> 3), (l >> 3) + 4, ... and eight lanes write one whole
+    // 32-byte sector.  (The eight words of an env are in one bank: an 8-way conflict on 48 loads per block, nothing
+    // against the staging pass it replaces.)
     if (pre_mode != 0) {
-        float *stage = reinterpret_cast<float *>(sm + L.o_stage);
+        const uint32_t *hb = reinterpret_cast<const uint32_t *>(sm);           // word w of env x at hb[w * 32 + x]
         float *snb = P.snap + (size_t)blk * 32u * 3u * N;                      // the block's rows: 32 x 3N contiguous floats
         const uint32_t N3 = 3u * N, n_valid = min(32u, P.E - blk * 32u);
+        const uint32_t j = lane & 7u, env0 = lane >> 3;
         __syncwarp();
 #pragma unroll 1
-        for (uint32_t f0 = 0; f0 < N3; f0 += 8) {
+        for (uint32_t f = j; f < N3; f += 8) {
+            uint32_t word, mask = ~0u;
+            float scale;
+            if (f < N) { word = 3u * f; mask = 0xFFFFu; scale = 0x1p-6f; }                   // d_queue = n_wait 2^-6
+            else if (f < 2u * N) { word = 3u * (f - N) + 2u; scale = 0x1p-18f; }             // d_e2e = ewma_q8 2^-18
+            else { word = 3u * (f - 2u * N) + 1u; scale = s_kvinv[f - 2u * N]; }             // d_kv = kv_used * fp32(1 / KV)
+            const uint32_t *src = hb + word * 32u + env0;
+            float *dst = snb + env0 * N3 + f;
 #pragma unroll
-            for (uint32_t j = 0; j < 8; j++) {
-                const uint32_t f = f0 + j;
-                float v = 0.0f;
-                if (f < N) v = __uint2float_rn(M_W0(f) & 0xFFFFu) * 0x1p-6f;
-                else if (f < 2 * N) v = __uint2float_rn(M_EWMA(f - N)) * 0x1p-18f;
-                else if (f < N3) v = __fmul_rn(__uint2float_rn(M_KV(f - 2 * N)), s_kvinv[f - 2 * N]);
-                stage[lane * 9u + j] = v;
-            }
-            __syncwarp();
-            // lane l copies feature (l & 7) of envs (l >> 3), (l >> 3) + 4, ...: eight lanes write one 32-byte sector
-            {
-                const uint32_t j = lane & 7u, env0 = lane >> 3;
-                const float *src = stage + env0 * 9u + j;
-                float *dst = snb + env0 * N3 + f0 + j;
-                const bool jok = f0 + j < N3;
-#pragma unroll
-                for (uint32_t i = 0; i < 8; i++)
-                    if (jok && env0 + 4u * i < n_valid) dst[4u * i * N3] = src[36u * i];
-            }
-            __syncwarp();
+            for (uint32_t i = 0; i < 8; i++)
+                if (env0 + 4u * i < n_valid) dst[4u * i * N3] = __fmul_rn(__uint2float_rn(src[4u * i] & mask), scale);
         }
     }
     // ---- counters
@@ -759,7 +749,7 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
     if (lane == 0) {
         bulk::s2g(blkp, sm, L.hdr_bytes);
         bulk::commit();
-        bulk::wait_all();
+        bulk::wait_read();
     }
 #undef H
 #undef M_W0
