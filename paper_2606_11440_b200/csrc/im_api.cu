@@ -285,7 +285,7 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     P.n_grp = P.SP / 8; P.cm_words = (P.n_grp + 3u) / 4u;
     P.n_chunks = R / kChunk + N;                               // <= 4096 / 32 + 16 = 144: chunk ids fit a byte
     P.hw_occ = 3 * N; P.hw_qfree = P.hw_occ + (P.SP + 31u) / 32u + 2u; P.hw_next = P.hw_qfree + P.QW; P.hw_head = P.hw_next + (P.n_chunks + 3u) / 4u;
-    P.hw_used = P.hw_head + 4; P.hw_misc = P.hw_used + (P.n_chunks + 31u) / 32u; P.hdr_words = P.hw_misc + 2;
+    P.hw_misc = P.hw_head + 4; P.hdr_words = P.hw_misc + 2;
     auto up128 = [](uint32_t x) { return (x + 127u) & ~127u; };
     uint32_t off = P.hdr_words * 128u;
     P.off_cm = off; off += P.cm_words * 128u;                 // directly behind the header: one bulk copy brings both
@@ -294,7 +294,7 @@ static size_t carve(im_ctx *c, const im_pool_spec &s, uint32_t E, uint8_t *base)
     P.off_hot = off; off += P.n_grp * 512u;
     P.off_iss = off; off += kIssueCap * 256u;
     P.off_qready = off; off += P.QW * 128u;
-    P.cold_stride = up128(P.SP * 16u); P.wkey_stride = P.n_chunks * kChunk * 4u; P.waux_stride = P.n_chunks * kChunk * 8u; P.q_stride = Q * 16u;
+    P.cold_stride = up128(P.SP * 32u); P.wkey_stride = P.n_chunks * kChunk * 4u; P.waux_stride = P.n_chunks * kChunk * 8u; P.q_stride = Q * 16u;
     P.off_cold = off; off += 32u * P.cold_stride;
     P.off_wkey = off; off += 32u * P.wkey_stride;
     P.off_waux = off; off += 32u * P.waux_stride;
@@ -789,15 +789,18 @@ int im_read_telemetry(im_ctx *c, uint32_t what, void *dst, size_t dst_bytes, siz
                         const uint32_t gs = P.slot_base[k] + sl;
                         if (!((H(P.hw_occ + (gs >> 5)) >> (gs & 31)) & 1u)) continue;
                         const uint32_t rem = hot[((gs >> 3) * 32 + l) * 8 + (gs & 7)];
-                        put(cold[gs].z & 0xFFFu, ST_RUN, k, cold[gs].y, cold[gs].x >> 16, cold[gs].x & 0xFFFFu, rem, sl + 1);
+                        put(cold[2 * gs].z & 0xFFFu, ST_RUN, k, cold[2 * gs].y, cold[2 * gs].x >> 16, cold[2 * gs].x & 0xFFFFu, rem, sl + 1);
                     }
-                for (uint32_t ch = 0; ch < P.n_chunks; ch++) {                // waiting lists: the chunks in use
-                    if (!((H(P.hw_used + (ch >> 5)) >> (ch & 31)) & 1u)) continue;
-                    for (uint32_t j = ch * kChunk; j < (ch + 1) * kChunk; j++) {
-                        const uint32_t key = wkey[j];
-                        if (key == 0xFFFFFFFFu) continue;
-                        const uint32_t id = key & 0xFFFu, tm = (key >> 12) & 0xFFFFu;
-                        put(id, ST_WAIT, key >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
+                for (uint32_t k = 0; k < N; k++) {                            // waiting lists: model k's chunks, the head chunk partly filled
+                    const uint32_t n = H(3 * k) & 0xFFFFu;
+                    uint32_t ch = (H(P.hw_head + (k >> 2)) >> (8 * (k & 3))) & 0xFFu, cnt = ((n - 1u) & (kChunk - 1u)) + 1u;
+                    for (uint32_t left = n; left > 0 && ch != 0xFFu; left -= cnt, cnt = kChunk) {
+                        for (uint32_t j = ch * kChunk; j < ch * kChunk + cnt; j++) {
+                            const uint32_t key = wkey[j];
+                            const uint32_t id = key & 0xFFFu, tm = (key >> 12) & 0xFFFFu;
+                            put(id, ST_WAIT, key >> 28, waux[j].y, P.sched_mode ? tm : qt[id >> 2].z, waux[j].x & 0xFFFFu, waux[j].x >> 16, 0);
+                        }
+                        ch = (H(P.hw_next + (ch >> 2)) >> (8 * (ch & 3))) & 0xFFu;
                     }
                 }
                 w += 5 * RD;

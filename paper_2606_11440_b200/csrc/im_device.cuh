@@ -14,7 +14,7 @@
 //   hdr   u32 units (hdr_words): m[3k] = n_wait | n_run << 16, m[3k+1] = kv_used, m[3k+2] = ewma_q8 |
 //         occ (bit gs = global slot gs taken; SP bits + two padding words) | qfree[QW] | the chunk directory of the waiting
 //         lists: next[c] (one byte per chunk, 0xFF = end: every model's chunks and the free chunks are linked lists) |
-//         head[k] (one byte per model, 0xFF = empty) | used bitmap (telemetry) | misc0 = drops | free head << 16 |
+//         head[k] (one byte per model, 0xFF = empty) | misc0 = drops | free head << 16 |
 //         misc1 = icnt
 //   cm    u32 units (cm_words): completion bytes of the tick's service pass, one per slot group (k_serve -> k_sim)
 //   kvt   u32 units (N): tokens decoded per model by the tick's service pass (k_serve -> k_sim)
@@ -24,12 +24,15 @@
 //         models numbered consecutively (R10); a group belongs to ONE model and to ONE Philox call (R2)
 //   iss   uint2 units (kIssueCap): {key, static word} written by the executor kernel for this tick (phase D)
 //   qready u32 units (QW): queries whose next stage is due, kept only ACROSS im_rollout calls
-//   cold[gs] uint4 = {issue(16) | deadline<<16, sw, id, 0}    sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
+//   cold[gs] 32 bytes = {issue(16) | deadline<<16, sw, id, 0, 0, 0, 0, 0}: written whole (st256) at admission
+//         sw = out_total(13) | in_tok(13)<<13 | succ<<26 | depth<<27
 //   wkey[c][32], waux[c][32]: the waiting lists, ONE UNORDERED LIST PER MODEL built from chunks of 32 entries out of a
 //         pool of n_chunks = RCAP/32 + N per env (only the head chunk of a model is partly filled, so the pool
 //         always suffices): admission only reads the chunks of the model that admits.  key = model<<28 |
 //         time(16)<<12 | id, time = deadline (EDF) or issue tick (FCFS): one u32 compare is the R20 order; id =
-//         4*query + agent; an empty entry of a chunk in use holds 0xFFFFFFFF (never a valid key).
+//         4*query + agent.  A list of n entries fills its non-head chunks and the first ((n - 1) & 31) + 1 entries of
+//         its head chunk; the rest of the head chunk holds 0xFFFFFFFF (never a valid key): a chunk is written whole
+//         when it is taken from the pool.
 //         waux = {issue(16) | remaining<<16, sw}
 //   q[i]     uint4 = {plan word, budget | in_tok<<16, deadline, arrive}
 // Free query slots are defined by the qfree bitmap and free service slots by occ (their cold words hold stale data).
@@ -101,7 +104,7 @@ struct Params {
     // env state: one record per block of 32 envs (layout at the top of this file)
     uint8_t *env_base;
     unsigned long long blk_stride;           // bytes, multiple of 128
-    uint32_t hw_occ, hw_qfree, hw_next, hw_head, hw_used, hw_misc, hdr_words;   // header word indices (m at word 0)
+    uint32_t hw_occ, hw_qfree, hw_next, hw_head, hw_misc, hdr_words;   // header word indices (m at word 0)
     uint32_t off_cm, off_kvt, off_ctr, off_hot, off_iss, off_qready;      // SoA-32 parts: byte offsets inside the block (hdr at 0)
     uint32_t off_cold, off_wkey, off_waux, off_q, cold_stride, wkey_stride, waux_stride, q_stride;   // per-env parts: lane 0 and lane stride
     uint32_t n_grp, cm_words;                // SP / 8 slot groups; completion-mask words per env = ceil(n_grp / 4)
@@ -137,6 +140,16 @@ __device__ __forceinline__ uint2 *iss_rec(const Params &P, uint32_t e, uint32_t 
 __device__ __forceinline__ uint4 *env_q(const Params &P, uint32_t e)
 {
     return reinterpret_cast<uint4 *>(blk_rec(P, e) + P.off_q + (size_t)(e & 31u) * P.q_stride);
+}
+// A 32-byte record written with ONE 256-bit store is a full-sector write: the memory system takes it as one DRAM
+// transaction, where a narrower store to a sector that is not resident costs a fill read plus the write (measured:
+// 44 G/s against 22.6 G/s for random sectors).  The per-request records that are written at
+// data-dependent positions (running-slot records) are therefore 32 bytes and 32-byte aligned.
+__device__ __forceinline__ void st256(void *p, uint4 a, uint4 b)
+{
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x),
+                 "r"(b.y), "r"(b.z), "r"(b.w)
+                 : "memory");
 }
 // row-list / log region of an env: the 32 envs of a block share one, so that a warp claims rows with one atomic
 __device__ __forceinline__ uint32_t region_of(const Params &P, uint32_t e) { return (e >> 5) % P.n_regions; }

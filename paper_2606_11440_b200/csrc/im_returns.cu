@@ -154,17 +154,27 @@ k_queue_order(const Params P, int32_t t, uint32_t *__restrict__ out)
     uint32_t n2cap = 32;
     while (n2cap < n_ent) n2cap <<= 1;
     uint32_t *keys = s_keys + (size_t)wib * n2cap;
-    // the waiting lists of env e: the entries of its chunks in use (im_device.cuh); empty entries hold 0xFFFFFFFF and sort last
+    // the waiting lists of env e (im_device.cuh): lane k walks the chunks of model k and notes how many entries of each
+    // are valid (only the head chunk is partly filled); everything else sorts last as 0xFFFFFFFF
     const uint32_t *wkey = reinterpret_cast<const uint32_t *>(blk_rec(P, e) + P.off_wkey + (size_t)(e & 31u) * P.wkey_stride);
+    uint32_t *cnt = s_keys + (size_t)kQoWarps * n2cap + (size_t)wib * P.n_chunks;
+    for (uint32_t c = lane; c < P.n_chunks; c += 32) cnt[c] = 0;
+    __syncwarp();
     uint32_t n = 0;
     for (uint32_t k = 0; k < P.N; k++) n += *hdr_word(P, e, 3u * k) & 0xFFFFu;
     n = min(n, P.RCAP);
-    const uint32_t n2 = n2cap;
-    for (uint32_t i = lane; i < n2; i += 32) {
-        const uint32_t ch = i / kChunk;
-        const bool used = i < n_ent && ((*hdr_word(P, e, P.hw_used + (ch >> 5)) >> (ch & 31u)) & 1u);
-        keys[i] = used ? wkey[i] : 0xFFFFFFFFu;
+    if (lane < P.N) {
+        const uint32_t nk = *hdr_word(P, e, 3u * lane) & 0xFFFFu;
+        uint32_t ch = (*hdr_word(P, e, P.hw_head + (lane >> 2)) >> (8u * (lane & 3u))) & 0xFFu, c1 = ((nk - 1u) & (kChunk - 1u)) + 1u;
+        for (uint32_t left = nk; left > 0 && ch != 0xFFu; left -= c1, c1 = kChunk) {
+            cnt[ch] = c1;
+            ch = (*hdr_word(P, e, P.hw_next + (ch >> 2)) >> (8u * (ch & 3u))) & 0xFFu;
+        }
     }
+    __syncwarp();
+    const uint32_t n2 = n2cap;
+    for (uint32_t i = lane; i < n2; i += 32)
+        keys[i] = (i < n_ent && (i % kChunk) < cnt[i / kChunk]) ? wkey[i] : 0xFFFFFFFFu;
     __syncwarp();
     for (uint32_t k = 2; k <= n2; k <<= 1) {
         uint32_t j = k >> 1;
@@ -204,7 +214,7 @@ int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t s
 {
     uint32_t n2cap = 32;
     while (n2cap < P.n_chunks * kChunk) n2cap <<= 1;
-    const size_t smem = (size_t)kQoWarps * n2cap * 4;
+    const size_t smem = (size_t)kQoWarps * (n2cap + P.n_chunks) * 4;
     cudaFuncSetAttribute(k_queue_order, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_queue_order<<<(P.E + kQoWarps - 1) / kQoWarps, kQoWarps * 32, smem, st>>>(P, t, out);
     return 1;
