@@ -292,22 +292,81 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
         for (uint32_t i = 0; i < 4; i++) r[i] = iss[i * 32u];
         bulk::mbar_wait(&s_bar[wib], 0);
 
-        // =============================================================== D-issue (R18): the new calls join the waiting list
+        // A WAITING request of model k (key, aux word wa, KV need) becomes RUNNING (R10, R11): lowest free slot of the model,
+        // prefill, its first tick of service, the slot's record.  w0 / kv = the model's counts before; returns the tokens of
+        // the first tick (the caller adds them to kv_used when admission is over for the model: R21 judges on the state
+        // before the tick's service).  n_run < S_k is the caller's check.
+        auto place = [&](uint32_t k, uint32_t key, uint2 wa, uint32_t need, uint32_t w0, uint32_t kv) -> uint32_t {
+            const uint32_t sw = wa.y, rem0 = wa.x >> 16, id = key & 0xFFFu;
+            uint32_t olo, ohi;
+            occ_window(s_sbase[k], olo, ohi);
+            const uint32_t sl = ~olo ? (uint32_t)__ffs(~olo) - 1u : 31u + (uint32_t)__ffs(~ohi);   // lowest free slot (R10): n_run < S_k, so it is one of the model's
+            const uint32_t gs = s_sbase[k] + sl;
+            OCC(gs >> 5) |= 1u << (gs & 31u);
+            const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
+            // prefill, then its first tick of service (R11)
+            // (32-bit arithmetic throughout: prefill * need <= 5e7 by the spec check "prefill is sub-tick",
+            // rate * usable <= 4e9, and fr * 2^16 / 10^6 = fr * 1024 / 15625 exactly, fr * 1024 < 2^30)
+            const uint32_t pf = (s_prefill[k] * need) / 1000u;
+            const uint32_t usable = kDtUs - min(pf, kDtUs);
+            const uint32_t x = s_rate[k] * usable;
+            const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
+            const uint32_t thr = (fr * 1024u) / 15625u;
+            const uint32_t u16 = u16_field(philox4x32_10_rk(gid, (uint32_t)t, gs >> 3, 0u, P.svc_rk), gs & 7u);
+            const uint32_t tok = min(bs + (u16 < thr ? 1u : 0u), rem0);
+            const uint32_t rem = rem0 - tok;
+            hot16[(gs >> 3) * 256u + (gs & 7u)] = (uint16_t)rem;
+            st256(&cold[2u * gs], make_uint4((wa.x & 0xFFFFu) | (dl << 16), sw, id, 0u), make_uint4(0u, 0u, 0u, 0u));
+            if (rem == 0) {
+                const uint32_t g = gs >> 3;
+                cmg[(g >> 2) * 32u] |= 1u << (8u * (g & 3u) + ((gs & 7u) >> 1) + 4u * (gs & 1u));   // the lane's own word; rare
+            }
+            M_W0(k) = w0 + 0x10000u;                              // n_run++
+            M_KV(k) = kv + need;
+            return tok;
+        };
+
+        // =============================================================== D-issue (R18): the new calls join the waiting list -
+        // or skip it.  A call that is the model's ONLY issue of the tick and finds the model's queue empty is exactly what
+        // the admission phase would look at first for that model, alone: if a slot is free and its KV fits it is admitted
+        // here, straight from the issue record, and the list (two stores now, two loads and a store in the admission
+        // phase, all at data-dependent addresses) is never touched; if not, it waits like any other.  Below saturation
+        // that is most calls.  (Decided only when all of the tick's issue records are the four already in registers.)
         const uint32_t drops_in = H(P.hw_misc) & 0xFFFFu;        // R9: drops of this tick's phase A
         free_head = H(P.hw_misc) >> 16;
         {
             uint32_t icnt = H(P.hw_misc + 1u);
             if (icnt > kIssueCap) icnt = kIssueCap;              // the executor kernel flags the overflow (err_flag)
+            uint32_t queued = ~0u;                                // models whose issues must go through the list
+            if (icnt <= 4u) {
+                uint32_t seen = 0;
+                queued = 0;
+#pragma unroll
+                for (uint32_t i = 0; i < 4; i++)
+                    if (i < icnt) { const uint32_t b = 1u << (r[i].x >> 28); queued |= seen & b; seen |= b; }
+            }
 #pragma unroll 1
             for (uint32_t j0 = 0; j0 < icnt; j0 += 4) {            // four records in flight per lane
                 if (j0) {
 #pragma unroll
                     for (uint32_t i = 0; i < 4; i++) if (j0 + i < icnt) r[i] = iss[(j0 + i) * 32u];
                 }
-#pragma unroll
-                for (uint32_t i = 0; i < 4; i++)
-                    if (j0 + i < icnt)   // issue = t, remaining = out_total
-                        list_insert(r[i].x >> 28, r[i].x, make_uint2(((uint32_t)t & 0xFFFFu) | ((r[i].y & SW_TOK_MASK) << 16), r[i].y));
+#pragma unroll 1
+                for (uint32_t i = 0; i < 4 && j0 + i < icnt; i++) {
+                    const uint2 rec = i == 0 ? r[0] : (i == 1 ? r[1] : (i == 2 ? r[2] : r[3]));
+                    const uint32_t k = rec.x >> 28;
+                    const uint2 aux = make_uint2(((uint32_t)t & 0xFFFFu) | ((rec.y & SW_TOK_MASK) << 16), rec.y);   // issue = t, remaining = out_total
+                    bool direct = false;
+                    if (!((queued >> k) & 1u)) {
+                        const uint32_t w0 = M_W0(k), kv = M_KV(k);
+                        const uint32_t need = (rec.y >> SW_IN_SHIFT) & SW_TOK_MASK;                          // R12: nothing decoded yet
+                        if ((w0 & 0xFFFFu) == 0 && (w0 >> 16) < s_slots[k] && kv + need <= s_kvcap[k]) {
+                            M_KV(k) += place(k, rec.x, aux, need, w0, kv);
+                            direct = true;
+                        }
+                    }
+                    if (!direct) list_insert(k, rec.x, aux);
+                }
             }
             c_issued += icnt;
         }
@@ -362,36 +421,11 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                     }
                     bool again = false;
                     if (key != ~0u) {
-                        const uint32_t sw = wa.y, rem0 = wa.x >> 16, id = key & 0xFFFu;
+                        const uint32_t sw = wa.y, rem0 = wa.x >> 16;
                         const uint32_t need = ((sw >> SW_IN_SHIFT) & SW_TOK_MASK) + ((sw & SW_TOK_MASK) - rem0);     // R12
                         const uint32_t w0 = M_W0(k), nr = w0 >> 16, kv = M_KV(k), slots = s_slots[k];
                         if (nr < slots && kv + need <= s_kvcap[k]) {                          // else: stop at the first misfit (R21)
-                            uint32_t olo, ohi;
-                            occ_window(s_sbase[k], olo, ohi);
-                            const uint32_t sl = ~olo ? (uint32_t)__ffs(~olo) - 1u : 31u + (uint32_t)__ffs(~ohi);   // lowest free slot (R10): n_run < S_k, so it is one of the model's
-                            const uint32_t gs = s_sbase[k] + sl;
-                            OCC(gs >> 5) |= 1u << (gs & 31u);
-                            const uint32_t dl = P.sched_mode ? ((key >> 12) & 0xFFFFu) : (qtab[id >> 2].z & 0xFFFFu);
-                            // prefill, then its first tick of service (R11)
-                            // (32-bit arithmetic throughout: prefill * need <= 5e7 by the spec check "prefill is sub-tick",
-                            // rate * usable <= 4e9, and fr * 2^16 / 10^6 = fr * 1024 / 15625 exactly, fr * 1024 < 2^30)
-                            const uint32_t pf = (s_prefill[k] * need) / 1000u;
-                            const uint32_t usable = kDtUs - min(pf, kDtUs);
-                            const uint32_t x = s_rate[k] * usable;
-                            const uint32_t bs = x / 1000000u, fr = x - bs * 1000000u;
-                            const uint32_t thr = (fr * 1024u) / 15625u;
-                            const uint32_t u16 = u16_field(philox4x32_10_rk(gid, (uint32_t)t, gs >> 3, 0u, P.svc_rk), gs & 7u);
-                            const uint32_t tok = min(bs + (u16 < thr ? 1u : 0u), rem0);
-                            const uint32_t rem = rem0 - tok;
-                            hot16[(gs >> 3) * 256u + (gs & 7u)] = (uint16_t)rem;
-                            st256(&cold[2u * gs], make_uint4((wa.x & 0xFFFFu) | (dl << 16), sw, id, 0u), make_uint4(0u, 0u, 0u, 0u));
-                            if (rem == 0) {
-                                const uint32_t g = gs >> 3;
-                                cmg[(g >> 2) * 32u] |= 1u << (8u * (g & 3u) + ((gs & 7u) >> 1) + 4u * (gs & 1u));   // the lane's own word; rare
-                            }
-                            M_W0(k) = w0 + 0x10000u;                  // n_run++ (list_remove takes the request off n_wait)
-                            M_KV(k) = kv + need;
-                            tokacc += tok;
+                            tokacc += place(k, key, wa, need, w0, kv);
                             list_remove(k, j, lk, la);
                             again = (w0 & 0xFFFFu) > 1u && nr + 1u < slots;
                         }
