@@ -119,6 +119,54 @@ def algorithmic_model(spec, counters_sum, T, E):
                 ret_bytes=ret_bytes, n_exec=n_exec, n_plan=float(counters_sum[10]), env_ticks=env_ticks)
 
 
+def sim_access_model(spec, counters_sum, T, E):
+    """What one k_sim launch has to move, per launch (= E env-ticks), split by how the memory system sees it
+    (DESIGN.md section 7 'what bounds k_sim'): `stream_*` sectors are read / written in lane order by whole warps or by
+    the bulk copies (header in + out, k_serve's results, issue records, snapshot, trajectory rows); `rand_*` are the
+    ALGORITHMIC accesses at data-dependent addresses that no layout of per-request records can avoid: per admission a
+    full 32-byte slot record and the slot's token counter (a 2-byte store into a sector: fill + write), per completion
+    the slot record and the query entry read and the query's plan word written back, per arrival the query entry."""
+    N = spec.n_models
+    SP = int(sum(((int(x) + 7) // 8) * 8 for x in spec.slots))
+    n_chunks = spec.rcap // 32 + N
+    hdr_words = 3 * N + (SP + 31) // 32 + 2 + spec.qcap // 32 + (n_chunks + 3) // 4 + 4 + 2      # im_api.cu: carve()
+    cm_words = (SP // 8 + 3) // 4
+    per_tick = 1.0 / T
+    n_exec, n_arr, n_done, n_fin = (float(counters_sum[i]) * per_tick for i in (11, 0, 6, 2))
+    stream_read = E * (hdr_words + cm_words + N) * 4 / 32.0 + n_exec * 8 / 32.0
+    stream_write = E * (hdr_words * 4 + 12 * N + 10) / 32.0 + (n_exec + n_arr + n_fin) * 16 / 32.0   # + rows / log records
+    rand = dict(read16=2.0 * n_done, write32=n_exec, write16=n_exec + (n_done - n_fin) + n_arr)
+    return dict(stream_read_sectors=stream_read, stream_write_sectors=stream_write, rand_ops=rand, hdr_words=hdr_words)
+
+
+def random_access_report(spec, csum, T, E, cfg, dev, peaks, sim_ms):
+    """roofline['random_access']: measured rates of the device for accesses at data-dependent addresses, and two lower
+    bounds of one k_sim launch built from them: `t_alg_ms` from the algorithmic access counts of `sim_access_model`,
+    `t_traffic_ms` from the DRAM sectors ncu counted for that launch (profiles/ncu_sim_dram.csv, used only while the
+    kernel sources still hash to the capture's)."""
+    from paper_2606_11440_b200.probe import random_access_rates
+    rates = random_access_rates(device=str(dev), gib=16)
+    m = sim_access_model(spec, csum, T, E)
+    hbm = peaks["hbm"] * 1e9
+    t_stream = (m["stream_read_sectors"] + m["stream_write_sectors"]) * 32.0 / hbm
+    t_alg = t_stream + sum(m["rand_ops"][k] / (rates[k] * 1e9) for k in m["rand_ops"])
+    out = {"peak_gops": rates, "peak_source": "libimprobe (include/im_probe.h), 1 MiB windows, measured in this run",
+           "alg_ops_per_launch": m["rand_ops"], "stream_sectors_per_launch": m["stream_read_sectors"] + m["stream_write_sectors"],
+           "t_alg_ms": t_alg * 1e3, "frac_alg": t_alg * 1e3 / max(sim_ms, 1e-9), "t_traffic_ms": None, "frac_traffic": None}
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "ncu_sim_dram.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["config"] == f"cfg{cfg}" and E == CONFIGS[cfg]["E"] and row["csrc_sha"] == csrc_sha():
+                    rd, wr = float(row["dram_sectors_read"]), float(row["dram_sectors_write"])
+                    r_rand, w_rand = max(rd - m["stream_read_sectors"], 0.0), max(wr - m["stream_write_sectors"], 0.0)
+                    t_tr = t_stream + r_rand / (rates["read16"] * 1e9) + w_rand / (rates["write32"] * 1e9)
+                    out.update(dram_sectors_per_launch={"read": rd, "write": wr}, t_traffic_ms=t_tr * 1e3, frac_traffic=t_tr * 1e3 / max(sim_ms, 1e-9))
+    except (OSError, ValueError, KeyError):
+        pass
+    return out
+
+
 def baseline_sample(cfg: int, cores: int):
     """(envs, ticks) of the bounded sample the oracle is timed on: the first envs x the first ticks of the config."""
     return max(cores * 4, 32), {1: 200, 2: 500, 3: 300, 4: 200, 5: 512}[cfg]
@@ -195,6 +243,7 @@ def main():
     ap.add_argument("--envs", type=int, default=None, help="override E (debug)")
     ap.add_argument("--ticks", type=int, default=None, help="override T (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probe", action="store_true", help="skip the random-access probe (libimprobe)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -348,6 +397,12 @@ def main():
     roof["step_lb_frac"] = max(roof["step_hbm_frac"], roof["step_tensor_frac"] or 0.0)
     # one im_returns call covers one rollout call (chunk): bytes of that call over the time of that call
     roof["returns_hbm_frac"] = per_s("ret_bytes", "returns") / 1e9 / peaks["hbm"]
+    # ---- k_sim against the ceilings that apply to it: accesses at data-dependent addresses (libimprobe, measured now)
+    if rank == 0 and not args.no_probe:
+        try:
+            roof["random_access"] = random_access_report(spec, csum, T, E, cfg, dev, peaks, per_launch_ms["sim"])
+        except Exception as err:  # the probe is a measurement aid: never fail the bench line over it
+            roof["random_access"] = {"error": str(err)[:200]}
 
     # ---- end to end through the C ABI with HOST buffers: host blob in, ADV / RET / scalars out to pinned host memory
     adv_h = torch.empty((chunk, E), dtype=torch.float32, pin_memory=True)

@@ -9,6 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libinframind.so")
 SOURCES = ["im_api.cu", "im_sim.cu", "im_policy.cu", "im_returns.cu"]
+PROBE_SO = os.path.join(HERE, "libimprobe.so")     # include/im_probe.h: measurement probe used by bench.py, a library of its own
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 
@@ -17,7 +18,11 @@ def _stale() -> bool:
     if not os.path.exists(SO):
         return True
     t = os.path.getmtime(SO)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "inframind.h")]
+    if not os.path.exists(PROBE_SO):
+        return True
+    t = min(t, os.path.getmtime(PROBE_SO))
+    inc = os.path.join(HERE, "..", "include")
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(inc, f) for f in os.listdir(inc)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
@@ -40,6 +45,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
         objs.append(obj)
     cmd = [nvcc, "-shared", "-o", SO, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
     subprocess.check_call(cmd)
+    cmd = [nvcc, *NVCC_FLAGS, "-shared", os.path.join(CSRC, "im_probe.cu"), "-o", PROBE_SO, "-lcudart"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed on im_probe.cu")
     return SO
 
 

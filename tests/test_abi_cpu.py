@@ -31,6 +31,20 @@ def test_exports_every_declared_symbol(lib):
     assert set(EXPORTS) == declared
 
 
+def test_probe_library_exports_its_symbol(lib):
+    """include/im_probe.h (the measurement probe of bench.py) is a library of its own; a bad argument is refused on the host."""
+    from paper_2606_11440_b200.probe import load_probe
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "im_probe.h")).read(), flags=re.S)
+    declared = set(re.findall(r"\b(im_[a-z_]+)\s*\(", hdr))
+    assert declared == {"im_probe_random_access"}
+    p = load_probe()
+    for name in declared:
+        assert hasattr(p, name)
+        assert not hasattr(lib, name)                       # the boundary of the method holds nothing but the method
+    g = C.c_double(0.0)
+    assert p.im_probe_random_access(None, 1 << 30, 1 << 20, 0, 64, 1, None, C.byref(g)) == -1
+
+
 def test_spec_struct_layout_matches_header(lib):
     """The ctypes mirror must have the C struct's size: 26 u32 + 3 u64 + 16 models x 32 B + 4 pointers."""
     from paper_2606_11440_b200.binding import im_pool_spec, im_model_spec

@@ -116,3 +116,13 @@ def test_device_blob_of_another_spec_is_rejected():
     g.reset(); g.rollout(good, 10)
     assert np.array_equal(a, g.rew()) and np.array_equal(c1, g.counters())
     g.close()
+
+
+def test_random_access_probe_orders_the_access_shapes():
+    """libimprobe (bench.py's ceilings for k_sim): a full-sector 256-bit store must beat a half-sector store clearly (the
+    reason the running-slot records are 32 bytes), and every rate is a positive, sane number."""
+    from paper_2606_11440_b200.probe import random_access_rates
+    r = random_access_rates(gib=4, rounds=16)
+    assert set(r) == {"read16", "write16", "write32", "rmw4"}
+    assert all(1.0 < v < 2000.0 for v in r.values()), r
+    assert r["write32"] > 1.3 * r["write16"] and r["read16"] > r["write16"] > r["rmw4"], r
