@@ -601,6 +601,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             bulk::g2s(img + o, W.tc_img + o, Net::kImageBytes - o < kPiece ? Net::kImageBytes - o : kPiece, &wbar);
     }
     if (threadIdx.x < 32) tc::tmem_alloc(&tmem_slot, Net::kTmemCols);
+    griddep_wait();                                       // the weights were packed before the rollout's first kernel; the rows are the predecessor's
     const RowBuf &rb = EXEC ? P.exec : P.plan;
     const uint32_t n_crit = EXEC ? P.E : 0u;
     sched_init(P, sched, rb, parity, 128, n_crit);
@@ -831,8 +832,8 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
     }
     if (W.tc_img) {      // F = 128, H = 256: tcgen05
         const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot);
-        if (exec) k_policy_tc<true><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
-        else k_policy_tc<false><<<n_sm, kTcThreads, smem, st>>>(P, W, parity, t0, trow);
+        if (exec) launch_chained(k_policy_tc<true>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
+        else launch_chained(k_policy_tc<false>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
         return 0;
     }
     if (P.f_in == 64 && P.hidden == 128) {      // too narrow for a 128 x 256 UMMA tile to pay: mma.sync

@@ -76,6 +76,7 @@ __device__ __forceinline__ uint32_t u16_field(const Ph4 &u, uint32_t f)
 __global__ void __launch_bounds__(kServeWarps * 32, 4)
 k_serve(const Params P, int32_t t)
 {
+    griddep_wait();
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t w = blockIdx.x * kServeWarps + (threadIdx.x >> 5);
     if (w >= P.NB * P.N) return;
@@ -140,6 +141,7 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
     if (lane == 0) bulk::mbar_init(&s_bar[wib], 1);
     bulk::fence_mbar_init();
     __syncthreads();
+    griddep_wait();                                                         // everything above reads the spec only
     // blocks in descending order: neutral in general; where load rises with the env index (the utilisation sweep of
     // configs[3]-[4]) the heaviest blocks start first and the last wave is the lightest
     const uint32_t wg = blockIdx.x * kSimWarps + wib;
@@ -825,14 +827,15 @@ int sim_prepare_device()
 void launch_serve(const Params &P, int32_t t, cudaStream_t st)
 {
     const uint32_t warps = P.NB * P.N;
-    k_serve<<<(warps + kServeWarps - 1) / kServeWarps, kServeWarps * 32, 0, st>>>(P, t);
+    launch_chained(k_serve, dim3((warps + kServeWarps - 1) / kServeWarps), dim3(kServeWarps * 32), 0, st, true, P, t);
 }
 
 void launch_sim(const Params &P, int32_t t_post, uint32_t trow_post, int32_t t_pre, uint32_t pre_mode, int32_t t0, cudaStream_t st)
 {
     const SimSmem L = sim_smem(P);
     const uint32_t blocks = (P.NB + kSimWarps - 1) / kSimWarps;
-    k_sim<<<blocks, kSimWarps * 32, (size_t)kSimWarps * L.per_warp, st>>>(P, L, t_post, trow_post, t_pre, pre_mode, t0);
+    // the first launch of a rollout (t_post < 0) follows host copies and other kernels: a plain launch
+    launch_chained(k_sim, dim3(blocks), dim3(kSimWarps * 32), (size_t)kSimWarps * L.per_warp, st, t_post >= 0, P, L, t_post, trow_post, t_pre, pre_mode, t0);
 }
 
 }  // namespace im
