@@ -373,7 +373,7 @@ def main():
         import csv
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
             for row in csv.DictReader(f):
-                if (row["config"] == f"cfg{cfg}" and row["kernel"] == roof["kernel"].split("<")[0] and E == CONFIGS[cfg]["E"]
+                if (row["config"] == f"cfg{cfg}" and row["kernel"] == roof["kernel"] and E == CONFIGS[cfg]["E"]
                         and row["csrc_sha"] == csrc_sha()):
                     roof["traffic"] = float(row["dram_bytes_per_launch"]) / 1e9
                     roof["traffic_source"] = row["source"]

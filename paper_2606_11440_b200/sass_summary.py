@@ -10,7 +10,7 @@ import re
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-WANT = ["UTCHMMA", "LDTM", "STTM", "UTCBAR", "UBLKCP", "SYNCS", "HMMA", "MUFU.TANH", "VIMNMX.U16x2", "ATOMG", "REDG", "RED.", "total"]
+WANT = ["UTCHMMA", "LDTM", "STTM", "UTCBAR", "UBLKCP", "SYNCS", "HMMA", "MUFU.TANH", "VIMNMX.U16x2", "STG.E.ENL2.256", "ACQBULK", "ATOMG", "REDG", "RED.", "total"]
 
 
 def main():
