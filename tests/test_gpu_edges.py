@@ -118,6 +118,27 @@ def test_device_blob_of_another_spec_is_rejected():
     g.close()
 
 
+@pytest.mark.parametrize("sched_mode,kv_preempt", [(1, 0), (0, 0), (1, 1)])
+def test_direct_admission_borderline_cases(sched_mode, kv_preempt):
+    """k_sim admits a call straight from its issue record when it is its model's only issue of the tick and the queue is
+    empty.  Debate with K = 4 issues three calls in ONE tick, forced onto two models with two slots each and a KV capacity
+    that fits one or two requests: same-model issues in one tick (must go through the list, smallest key first, stop at
+    the first misfit), lone issues that do not fit (must wait), lone issues that fit (admitted directly), all interleaved
+    with completions and, with kv_preempt, evictions back into the list.  Compared with the oracle after EVERY tick
+    (state dump included), EDF and FCFS."""
+    from helpers import planner_bias_blob
+    N = 2
+    spec = tiny_spec(n_envs=37, N=N, n_ticks=220, qcap=32, rcap=128, rate_tick=[0.05, 0.25, 0.6], slots=2, rates=[90, 140],
+                     kv_cap=[700, 1100], kv_preempt=kv_preempt, sched_mode=sched_mode, budget=(20, 120), medians=(60, 120, 240),
+                     in_tok=300, prefill=400, f_in=32, hidden=16, seed=21)
+    bias = np.full(3 * N, -40.0)
+    bias[[0, 1, 3, 4, 5]] = 0.0                               # both models, several depths: uniform among them
+    st = _run(spec, seed=6, chunks=[1] * 220, blob=planner_bias_blob(spec, topo=2, count=4, exec_bias=bias))
+    assert st["decisions"] > 3000 and st["finished"] > 50
+    if kv_preempt:
+        assert st["preemptions"] > 0
+
+
 def test_random_access_probe_orders_the_access_shapes():
     """libimprobe (bench.py's ceilings for k_sim): a full-sector 256-bit store must beat a half-sector store clearly (the
     reason the running-slot records are 32 bytes), and every rate is a positive, sane number."""
