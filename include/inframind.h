@@ -200,6 +200,29 @@ uint64_t im_launch_count(const im_ctx *ctx);
 int im_set_profiling(im_ctx *ctx, int enable);
 int im_kernel_times(im_ctx *ctx, double *ms, uint64_t *launches);
 
+/* The returns kernel for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): GAE with the Lagrangian reward r - mu C (Eq. 3; R29, R31), the same arithmetic
+ * as im_returns, on plain DEVICE arrays of the caller, without a ctx and without ANY allocation: the kernel's scratch
+ * memory (one partial cost sum per 256 envs and a ticket) is a static device array of 33 024 bytes inside the library,
+ * held by every GPU that loads the library until the process exits.
+ *   rew, cost   [n_ticks][n_envs] f32 (env fastest)       val  [n_ticks + 1][n_envs] f32 (row n_ticks = bootstrap value, R30)
+ *   done        [n_ticks][n_envs] u8 (R33)                adv, ret  [n_ticks][n_envs] f32, written
+ *   sum_cost    one f64, written: sum of cost over all rows (numerator of C-bar, Eq. 7), added up in a
+ *               fixed order (the same bits in every run); may be NULL
+ *   cuda_stream cudaStream_t (may be NULL); asynchronous: the results are valid after the stream has synchronised
+ *   errbuf      optional host buffer that receives the message of a failing call ("" on success)
+ * All arrays are caller-owned; device pointers of the CURRENT device.  n_envs > IM_GAE_STATIC_MAX_ENVS is refused with
+ * IM_ERR_CAPACITY (split the batch by env ranges, or use im_returns); null arrays or zero sizes IM_ERR_INVALID_ARG; a
+ * CUDA failure IM_ERR_CUDA.  Calls no cudaMalloc / cudaFree or allocating routine; the first call on a device looks the
+ * scratch address up (cudaGetSymbolAddress), so make one call per device before capturing a graph.
+ * EVERY call on a device shares the one scratch array: calls that overlap on the GPU (different streams, or graphs
+ * replayed concurrently) race on it and return a wrong sum_cost; calls ordered on one stream are safe (each call clears
+ * the ticket it needs at zero; the partial sums are rewritten before they are read). */
+#define IM_GAE_STATIC_MAX_ENVS 1048576u
+int im_gae_static(const float *rew, const float *cost, const float *val, const uint8_t *done, float *adv, float *ret,
+                  double *sum_cost, uint32_t n_ticks, uint32_t n_envs, float gamma, float lambda, float lagrange_mu,
+                  void *cuda_stream, char *errbuf, size_t errbuf_bytes);
+
 void im_destroy(im_ctx *ctx);
 
 /* Message of the last failing call on this ctx (string owned by ctx, valid until the next call); "" if none.

@@ -23,7 +23,8 @@ IM_FLAG_LOG_DECISIONS, IM_FLAG_LOG_LOGITS = 1, 2
  IM_TEL_QUEUE_ORDER, IM_TEL_TABLES, IM_TEL_LOGITS_EXEC, IM_TEL_LOGITS_PLAN, IM_TEL_SUMS) = range(1, 21)
 
 EXPORTS = ["im_arena_bytes", "im_create", "im_bind", "im_reset", "im_rollout", "im_returns", "im_returns_finish", "im_read_telemetry",
-           "im_device_ptr", "im_launch_count", "im_set_profiling", "im_kernel_times", "im_destroy", "im_last_error"]
+           "im_device_ptr", "im_launch_count", "im_set_profiling", "im_kernel_times", "im_destroy", "im_last_error", "im_gae_static"]
+IM_GAE_STATIC_MAX_ENVS = 1048576
 
 
 class im_model_spec(C.Structure):
@@ -72,8 +73,28 @@ def load_library():
         L.im_destroy.argtypes = [C.c_void_p]
         L.im_last_error.restype = C.c_char_p
         L.im_last_error.argtypes = [C.c_void_p]
+        L.im_gae_static.argtypes = [C.c_void_p] * 7 + [C.c_uint32, C.c_uint32, C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_char_p, C.c_size_t]
         _lib = L
     return _lib
+
+
+def gae_static(rew, cost, val, done, adv, ret, sum_cost, gamma: float, lam: float, mu: float, stream=None):
+    """im_gae_static: GAE / Lagrangian returns on the caller's CUDA tensors, no ctx and no allocation (static scratch inside
+    the library, <= IM_GAE_STATIC_MAX_ENVS envs).  rew / cost [T, E] f32, val [T + 1, E] f32, done [T, E] u8, adv / ret
+    [T, E] f32 (written), sum_cost: one-element f64 CUDA tensor (written) or None.  Argument marshalling only."""
+    import torch
+    T, E = rew.shape
+    for x, dt, sh in ((rew, torch.float32, (T, E)), (cost, torch.float32, (T, E)), (val, torch.float32, (T + 1, E)),
+                      (done, torch.uint8, (T, E)), (adv, torch.float32, (T, E)), (ret, torch.float32, (T, E))):
+        assert x.is_cuda and x.is_contiguous() and x.dtype == dt and tuple(x.shape) == sh
+    assert sum_cost is None or (sum_cost.is_cuda and sum_cost.dtype == torch.float64 and sum_cost.numel() == 1)
+    err = C.create_string_buffer(512)
+    st = (stream if stream is not None else torch.cuda.current_stream(rew.device)).cuda_stream
+    with torch.cuda.device(rew.device):
+        rc = load_library().im_gae_static(rew.data_ptr(), cost.data_ptr(), val.data_ptr(), done.data_ptr(), adv.data_ptr(), ret.data_ptr(),
+                                          None if sum_cost is None else sum_cost.data_ptr(), T, E, gamma, lam, mu, st, err, 512)
+    if rc != 0:
+        raise IMError(rc, err.value.decode())
 
 
 def marshal_spec(spec, debug_flags: Optional[int] = None):

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libinframind.so")
-SOURCES = ["im_api.cu", "im_sim.cu", "im_policy.cu", "im_returns.cu"]
+SOURCES = ["im_api.cu", "im_sim.cu", "im_policy.cu", "im_returns.cu", "im_noalloc.cu"]
 PROBE_SO = os.path.join(HERE, "libimprobe.so")     # include/im_probe.h: measurement probe used by bench.py, a library of its own
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
