@@ -608,10 +608,11 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     tc::tc_fence_before();
     __syncthreads();
     tc::tc_fence_after();
-    const uint32_t tmem_base = tmem_slot;
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, tmem_slot, 0);          // (the shuffles tell ptxas that these are warp-uniform:
+    const uint32_t warp_u = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);      //  the UMMA operands then live in uniform registers)
     const uint32_t N3 = 3 * P.N;
     const bool vec = (N3 % 8u) == 0;                      // snapshot block = whole 16-byte chunks (N = 8, 16)
-    const uint32_t wg = threadIdx.x >> 7, r = threadIdx.x & 127u;
+    const uint32_t wg = warp_u >> 2, r = threadIdx.x & 127u;
     const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
     const float *bias = reinterpret_cast<const float *>(img + Net::kBias);
     const uint32_t total = sched.total;
@@ -682,7 +683,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             tc::fence_proxy_async_smem();
             tc::bar_sync(4, 128);
             tc::mbar_wait(&wbar, 0);
-            if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
+            if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
             nxt = tc_fetch_row(sched, rb, blockIdx.x + gridDim.x, r, n_crit);
             fetch_snap(nxt, sn);
         }
@@ -701,14 +702,14 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             tc::bar_sync(2, 128);
             // layer 2 overwrites D3 / A3 of the previous tile: wait until warpgroup 0 has its logits in registers
             if (it > 0) tc::bar_sync(3, 256);
-            if (r == 0) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
+            if (warp_u == 4) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
             // the next tile: features (layer 1 of this tile is done with a1), layer 1 behind layer 2 in the tensor pipe
             // (UMMAs of one thread execute in order, so A2 is consumed by then), row loads of the tile after it
             if (tile + gridDim.x < total) {
                 build_a1(nxt, sn, rowbuf + 128 * ((it + 1) & 1u));
                 tc::fence_proxy_async_smem();
                 tc::bar_sync(4, 128);
-                if (r == 0) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
+                if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
                 nxt = tc_fetch_row(sched, rb, tile + 2 * gridDim.x, r, n_crit);
                 fetch_snap(nxt, sn);
             }
@@ -723,7 +724,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         Net::half_epilogue(tlane, Net::kColD2 + 128, Net::kColD2 + 128, bias + kTcH + 128);
         tc::tc_fence_before();
         tc::bar_sync(5, 128);
-        if (threadIdx.x == 0) Net::issue_l3(img, tmem_base, &bars[4]);
+        if (warp_u == 0) Net::issue_l3(img, tmem_base, &bars[4]);
         // ---- warpgroup 0: sampling epilogue of row r, logits in registers
         const TcRowSlot sl = rowbuf[128 * (it & 1u) + r];
         uint32_t islot = ~0u;                              // executor rows: the env's issue-list slot, claimed before the wait

@@ -93,6 +93,21 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
         "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// One lane of a CONVERGED warp (elect.sync).  UMMAs are issued this way - `if (warp-uniform condition) if (elect_one())` -
+// and never under a per-thread condition such as threadIdx.x == 0: there ptxas cannot prove the operands uniform and
+// wraps every UTCHMMA in an elect / broadcast / branch loop of ~15 dependent instructions (measured: 62 cycles per
+// UMMA, 2000 cycles of blocking issue for layer 2).
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P;\n\t"
+        "elect.sync _|P, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t"
+        "}" : "=r"(pred));
+    return pred != 0;
+}
 // all UMMAs issued so far by this thread arrive on `bar` when they complete (implies fence::before_thread_sync)
 __device__ __forceinline__ void umma_commit(uint64_t *bar)
 {
@@ -209,42 +224,51 @@ struct TcMlp {
         tc_wait_st();
     }
 
-    // ---- UMMA issue, ONE thread each.  Layer 1 (SS): A1 in shared memory (canonical [128][K1]) x W1 -> D1, two halves.
+    // ---- UMMA issue: called by ONE CONVERGED WARP, one elected lane issues.  Layer 1 (SS): A1 in shared memory (canonical [128][K1]) x W1 -> D1, two halves.
     static __device__ __forceinline__ void issue_l1(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
     {
         tc_fence_after();
         const uint32_t sa = smem_u32(a1), sb = smem_u32(image + kW1);
+        if (elect_one()) {
 #pragma unroll
-        for (int h = 0; h < 2; h++) {
+            for (int h = 0; h < 2; h++) {
 #pragma unroll
-            for (int k = 0; k < K1 / 16; k++)
-                umma_ss(tmem_base + 128 * h, smem_desc(sa + k * 2 * 128 * 16, 128 * 16, 128),
-                        smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
-            umma_commit(h ? bar_b : bar_a);
+                for (int k = 0; k < K1 / 16; k++)
+                    umma_ss(tmem_base + 128 * h, smem_desc(sa + k * 2 * 128 * 16, 128 * 16, 128),
+                            smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
+                umma_commit(h ? bar_b : bar_a);
+            }
         }
+        __syncwarp();
     }
     // Layer 2 (TS): A2 (TMEM cols [0,128), 8 columns per K-chunk) x W2 -> D2 = [256,512), two N-halves
     static __device__ __forceinline__ void issue_l2(const uint8_t *image, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
     {
         tc_fence_after();
         const uint32_t sb = smem_u32(image + kW2);
+        if (elect_one()) {
 #pragma unroll
-        for (int h = 0; h < 2; h++) {
+            for (int h = 0; h < 2; h++) {
 #pragma unroll
-            for (int k = 0; k < H / 16; k++)
-                umma_ts(tmem_base + kColD2 + 128 * h, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
-            umma_commit(h ? bar_b : bar_a);
+                for (int k = 0; k < H / 16; k++)
+                    umma_ts(tmem_base + kColD2 + 128 * h, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
+                umma_commit(h ? bar_b : bar_a);
+            }
         }
+        __syncwarp();
     }
     // Layer 3 (TS): A3 (K-chunks 0-7 at [256,320), 8-15 at [384,448)) x W3 -> D3 = [448,448+NO)
     static __device__ __forceinline__ void issue_l3(const uint8_t *image, uint32_t tmem_base, uint64_t *bar)
     {
         tc_fence_after();
         const uint32_t sb = smem_u32(image + kW3);
+        if (elect_one()) {
 #pragma unroll
-        for (int k = 0; k < H / 16; k++)
-            umma_ts(tmem_base + kColD3, tmem_base + kColD2 + (k < 8 ? 8 * k : 128 + 8 * (k - 8)), smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
-        umma_commit(bar);
+            for (int k = 0; k < H / 16; k++)
+                umma_ts(tmem_base + kColD3, tmem_base + kColD2 + (k < 8 ? 8 * k : 128 + 8 * (k - 8)), smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
+            umma_commit(bar);
+        }
+        __syncwarp();
     }
     // one output of this thread's row, column `o` chosen at run time (the value head sits at 3N): D3[o] + b3[o]
     static __device__ __forceinline__ float load_output(const uint8_t *image, uint32_t tlane, uint32_t o)
