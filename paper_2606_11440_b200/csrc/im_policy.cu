@@ -620,10 +620,13 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
 
     // snapshot floats of a row's env (R14): up to 12 float4 per thread, issued early, consumed one tile later
     auto fetch_snap = [&](const TcRaw &x, float4 (&sn)[12]) {
-        const uint32_t env = x.critic ? x.env : x.row.x;
+        // Unconditional loads from an address that is always valid (env 0 for a padding row, chunk 0 beyond 3N): a load
+        // under a condition ends in a select, and the select waits for the load - 2000 cycles of DRAM latency per tile that
+        // were meant to pass behind the tanh epilogue.  build_a1 reads only the chunks below 3N, and only of rows that exist.
+        const uint32_t env = (x.ok && vec) ? (x.critic ? x.env : x.row.x) : 0u;
         const float4 *src = reinterpret_cast<const float4 *>(P.snap + (size_t)env * N3);
 #pragma unroll
-        for (int j = 0; j < 12; j++) sn[j] = (x.ok && vec && (uint32_t)(4 * j) < N3) ? ld_early_f4(src + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int j = 0; j < 12; j++) sn[j] = ld_early_f4(src + ((uint32_t)(4 * j) < N3 ? j : 0));
     };
     // features of row `cur` -> A1 (bf16 RNE), canonical layout: chunk c of row r at c * 2048 + r * 16; row -> rowbuf
     auto build_a1 = [&](const TcRaw &cur, const float4 (&sn)[12], TcRowSlot *slot) {
