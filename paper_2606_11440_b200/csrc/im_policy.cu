@@ -692,8 +692,11 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         }
     }
     tc::mbar_wait(&wbar, 0);
-    for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
-        if (wg == 1) {
+    // One loop per warpgroup.  (With one loop and a branch on the warpgroup inside it, the loop's back edge is a merge of
+    // both roles and ptxas waits there for EVERY outstanding scoreboard: warpgroup 1 sat out the 2000 cycles of its
+    // snapshot prefetch at the top of every tile instead of behind the tanh epilogue.)
+    if (wg == 1) {
+        for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
             // ---- warpgroup 1: tanh of layer 1, packed in place (half a while the tensor core computes half b)
             tc::mbar_wait(&bars[0], phase);
             tc::tc_fence_after();
@@ -716,8 +719,9 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
                 nxt = tc_fetch_row(sched, rb, tile + 2 * gridDim.x, r, n_crit);
                 fetch_snap(nxt, sn);
             }
-            continue;
         }
+    } else
+    for (uint32_t tile = blockIdx.x; tile < total; tile += gridDim.x, it++, phase ^= 1u) {
         // ---- warpgroup 0: tanh of layer 2, packed in place (half a while the tensor core computes half b), layer 3
         tc::mbar_wait(&bars[2], phase);
         tc::tc_fence_after();
