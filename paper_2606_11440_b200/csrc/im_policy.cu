@@ -18,6 +18,7 @@ struct TileSched {
     uint32_t pref[kRegions + 1];
     uint32_t base[kRegions];
     uint32_t cnt[kRegions];      // append counters at kernel start (the kernel's own list does not grow while it runs)
+    uint32_t base_mod[kRegions]; // base % regcap: the ring position of the region's first row of this tick
     uint32_t crit_tiles, total;
 };
 
@@ -29,6 +30,7 @@ __device__ __forceinline__ void sched_init(const Params &P, TileSched &S, const 
         if (blockIdx.x == 0 && !P.log_mode && c - b > rb.regcap) atomicOr(P.err_flag, 1u);
         S.base[threadIdx.x] = b;
         S.cnt[threadIdx.x] = c;
+        S.base_mod[threadIdx.x] = b % rb.regcap;
         S.pref[threadIdx.x + 1] = (c - b + rows_per_tile - 1) / rows_per_tile;
         if (blockIdx.x == 0) rb.base[(parity ^ 1u) * kRegions + threadIdx.x] = c;   // next tick starts here
     }
@@ -541,21 +543,27 @@ __device__ __forceinline__ float4 ld_early_f4(const float4 *p)
 __device__ __forceinline__ TcRaw tc_fetch_row(const TileSched &S, const RowBuf &rb, uint32_t tile, uint32_t r, uint32_t n_crit)
 {
     TcRaw x;
-    x.row = make_uint4(0, 0, 0, 0); x.env = 0; x.gidx = 0; x.ok = false; x.critic = false;
-    if (tile >= S.total) return x;
-    if (tile < S.crit_tiles) {
-        const uint32_t env = tile * 128u + r;
-        x.ok = env < n_crit; x.critic = true; x.env = env;
-        return x;
+    x.env = 0; x.gidx = 0; x.ok = false; x.critic = false;
+    if (tile < S.total) {
+        if (tile < S.crit_tiles) {
+            const uint32_t env = tile * 128u + r;
+            x.ok = env < n_crit; x.critic = true; x.env = env;
+        } else {
+            const uint32_t lt = tile - S.crit_tiles;
+            uint32_t lo = 0, hi = kRegions;
+            while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
+            const uint32_t off = (lt - S.pref[lo]) * 128u + r;
+            if (S.base[lo] + off < S.cnt[lo]) {
+                uint32_t pos = S.base_mod[lo] + off;             // off < cnt - base <= regcap (checked by sched_init): one wrap at most
+                if (pos >= rb.regcap) pos -= rb.regcap;
+                x.gidx = lo * rb.regcap + pos;
+                x.ok = true;
+            }
+        }
     }
-    const uint32_t lt = tile - S.crit_tiles;
-    uint32_t lo = 0, hi = kRegions;
-    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (S.pref[mid] <= lt) lo = mid; else hi = mid; }
-    const uint32_t idx = S.base[lo] + (lt - S.pref[lo]) * 128u + r;
-    if (idx >= S.cnt[lo]) return x;
-    x.gidx = row_gid(rb, lo, idx);
+    // ONE unconditional load on the single exit path (row 0 of the list for a row that does not exist or a critic row: never
+    // decoded): a load under a condition is merged by a select, and the select waits for the load
     x.row = ld_early_u4(rb.row + x.gidx);
-    x.ok = true;
     return x;
 }
 
@@ -676,7 +684,10 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         }
     };
     // ---- prologue: warpgroup 1 gathers the first tile and starts its layer 1
-    TcRaw nxt;
+    // Row prefetch runs TWO tiles ahead of the tile whose layer 1 is being read out, the snapshot of its env one tile ahead:
+    // the snapshot address comes out of the row, so a row fetched only one tile ahead put a full DRAM round trip (2000+
+    // cycles under load) into warpgroup 1's serial path on every tile of executor rows.
+    TcRaw nxt, nxt2;
     float4 sn[12];
     if (wg == 1) {
         nxt = tc_fetch_row(sched, rb, blockIdx.x, r, n_crit);
@@ -689,6 +700,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
             nxt = tc_fetch_row(sched, rb, blockIdx.x + gridDim.x, r, n_crit);
             fetch_snap(nxt, sn);
+            nxt2 = tc_fetch_row(sched, rb, blockIdx.x + 2 * gridDim.x, r, n_crit);
         }
     }
     tc::mbar_wait(&wbar, 0);
@@ -716,8 +728,9 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
                 tc::fence_proxy_async_smem();
                 tc::bar_sync(4, 128);
                 if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
-                nxt = tc_fetch_row(sched, rb, tile + 2 * gridDim.x, r, n_crit);
+                nxt = nxt2;                                   // row of tile + 2 grids: its load went out one tile ago
                 fetch_snap(nxt, sn);
+                nxt2 = tc_fetch_row(sched, rb, tile + 3 * gridDim.x, r, n_crit);
             }
         }
     } else
