@@ -623,16 +623,30 @@ k_sim(const Params P, const SimSmem L, int32_t t_post, uint32_t trow_post, int32
                 while (kv > cap) {
                     uint32_t best = 0, bsl = 0;
                     uint4 bcd = make_uint4(0, 0, 0, 0);
+                    // the records of the model's running slots, EIGHT loads in flight at a time (one load per iteration, with
+                    // the running maximum carried through it, is a chain of ~12 DRAM round trips per eviction, and with 32 envs
+                    // per warp some lane evicts in most ticks).  The loads are unconditional - a slot that is not there reads
+                    // the model's first slot and is ignored - so that nothing waits before all eight are out.
 #pragma unroll 1
                     for (uint32_t half = 0; half < 2; half++) {
                         uint32_t ob = half ? ohi : olo;
 #pragma unroll 1
                         while (ob) {
-                            const uint32_t sl = half * 32u + (uint32_t)__ffs(ob) - 1u;
-                            ob &= ob - 1u;
-                            const uint4 cd = cold[2u * (sb + sl)];
-                            const uint32_t key = (((cd.x >> 16) << 12) | cd.z) + 1u;      // (deadline, id) + 1; unique
-                            if (key > best) { best = key; bsl = sl; bcd = cd; }
+                            uint32_t sl[8];
+                            uint4 cd[8];
+                            bool have[8];
+#pragma unroll
+                            for (int j = 0; j < 8; j++) {
+                                have[j] = ob != 0;
+                                sl[j] = have[j] ? half * 32u + (uint32_t)__ffs(ob) - 1u : 0u;
+                                ob &= ob - 1u;                                              // 0 stays 0
+                                cd[j] = cold[2u * (sb + sl[j])];
+                            }
+#pragma unroll
+                            for (int j = 0; j < 8; j++) {
+                                const uint32_t key = have[j] ? (((cd[j].x >> 16) << 12) | cd[j].z) + 1u : 0u;   // (deadline, id) + 1; unique
+                                if (key > best) { best = key; bsl = sl[j]; bcd = cd[j]; }
+                            }
                         }
                     }
                     if (best == 0) break;
