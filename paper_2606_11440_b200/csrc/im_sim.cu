@@ -80,7 +80,7 @@ k_serve(const Params P, int32_t t)
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t w = blockIdx.x * kServeWarps + (threadIdx.x >> 5);
     if (w >= P.NB * P.N) return;
-    const uint32_t blk = P.NB - 1u - w / P.N, k = w % P.N;
+    const uint32_t blk = w / P.N, k = w % P.N;     // ascending: k_sim walks the blocks in descending order, so the blocks it starts with are the ones this kernel wrote last (still in L2)
     const uint32_t g0 = P.slot_base[k] >> 3, ng = (P.slot_base[k + 1] - P.slot_base[k]) >> 3;    // 1 .. 8 groups
     const uint32_t gid = P.env_id_base + blk * 32u + lane;
     uint8_t *blkp = P.env_base + (size_t)blk * P.blk_stride;
