@@ -202,14 +202,26 @@ k_policy_f32(const Params P, const Weights W, uint32_t parity, int32_t t0, uint3
     const uint32_t F = P.f_in, H = P.hidden, NO = W.n_out, NOP = W.n_out_pad;
     float *sW1 = smem_f, *sW2 = sW1 + F * H, *sW3 = sW2 + H * H, *sb1 = sW3 + H * NOP, *sb2 = sb1 + H, *sb3 = sb2 + H;
     float *sx = sb3 + NOP;                               // per warp: [4][F] + [4][H] + [4][H] + [4][64] logits + [4][64] scratch
-    for (uint32_t i = threadIdx.x; i < F * H; i += blockDim.x) sW1[i] = W.W1t[i];
-    for (uint32_t i = threadIdx.x; i < H * H; i += blockDim.x) sW2[i] = W.W2t[i];
-    for (uint32_t i = threadIdx.x; i < H * NOP; i += blockDim.x) sW3[i] = W.W3t[i];
-    for (uint32_t i = threadIdx.x; i < H; i += blockDim.x) { sb1[i] = W.b1[i]; sb2[i] = W.b2[i]; }
-    for (uint32_t i = threadIdx.x; i < NOP; i += blockDim.x) sb3[i] = W.b3[i];
+    // The weights come by bulk async copies (TMA 1-D) that one thread issues and that fly while the CTA builds its tile
+    // schedule.  (Copied by a loop of scalar loads and stores they were 80 % of the kernel's time on the small
+    // configurations: ptxas does not overlap the loads of such a loop, 32 dependent L2 round trips per launch.)
+    __shared__ uint64_t wbar;
+    if (threadIdx.x == 0) {
+        bulk::mbar_init(&wbar, 1);
+        bulk::fence_mbar_init();
+        bulk::mbar_expect_tx(&wbar, 4u * (F * H + H * H + H * NOP + 2u * H + NOP));
+        auto copy = [&](float *dst, const float *src, uint32_t n_floats) {       // sizes and addresses are multiples of 16 bytes
+            constexpr uint32_t kPiece = 32 * 1024;
+            for (uint32_t o = 0; o < 4u * n_floats; o += kPiece)
+                bulk::g2s(reinterpret_cast<uint8_t *>(dst) + o, reinterpret_cast<const uint8_t *>(src) + o, min(kPiece, 4u * n_floats - o), &wbar);
+        };
+        copy(sW1, W.W1t, F * H); copy(sW2, W.W2t, H * H); copy(sW3, W.W3t, H * NOP);
+        copy(sb1, W.b1, H); copy(sb2, W.b2, H); copy(sb3, W.b3, NOP);
+    }
     const RowBuf &rb = EXEC ? P.exec : P.plan;
     const uint32_t n_crit = EXEC ? P.E : 0u;
     sched_init(P, sched, rb, parity, kF32Rows, n_crit);
+    bulk::mbar_wait(&wbar, 0);
 
     const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const uint32_t per_warp = kF32RowsPerWarp * (F + 2 * H + 128);
