@@ -362,7 +362,7 @@ def main():
         achieved = fl / n_l[dominant] / (per_launch_ms[dominant] * 1e-3) / 1e12
         if bf16:
             pk = peaks["bf16_sustained"]
-            kname = ("k_policy_tc" if spec.hidden == 256 else "k_policy_bf16") + f"<{dominant}>"
+            kname = "k_policy_tc" + f"<{dominant}>"
             roof = {"bound": "tensor", "kernel": kname, "achieved": achieved, "peak": pk, "unit": "TFLOP/s", "frac": achieved / pk, "traffic": None, "traffic_unit": tunit}
         else:
             pk = 148 * 128 * 2 * 1.965e9 / 1e12       # fp32 FFMA: 148 SMs x 128 lanes x 2 flop x max clock

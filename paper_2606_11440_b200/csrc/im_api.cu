@@ -25,7 +25,7 @@ int launch_queue_order(const Params &P, int32_t t, uint32_t *out, cudaStream_t s
 size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP);
 bool tc_supported(uint32_t F, uint32_t H);
 size_t tc_image_bytes(bool exec);
-void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t st);
+void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, uint32_t f_in, uint32_t hidden, cudaStream_t st);
 
 // empty pools: per 32-env block, zero the SoA-32 parts (header, counters, slot groups: a free slot holds 0, issue list,
 // ready bitmap), query bitmap all free for the envs that exist (the padding lanes of the last block have no free slot
@@ -507,7 +507,7 @@ static int upload_weights(im_ctx *c, const void *blob)
                                             (float *)w.W1t, (float *)w.W2t, (float *)w.W3t, (__nv_bfloat16 *)w.W1, (__nv_bfloat16 *)w.W2,
                                             (__nv_bfloat16 *)w.W3, (float *)w.b1, (float *)w.b2, (float *)w.b3);
         c->launches++;
-        if (w.tc_img) { launch_pack_tc(w, net == 1, c->spec.n_models, c->stream); c->launches++; }
+        if (w.tc_img) { launch_pack_tc(w, net == 1, c->spec.n_models, (uint32_t)F, (uint32_t)H, c->stream); c->launches++; }
     }
     CUDA_TRY(c, cudaGetLastError());
     return IM_OK;

@@ -124,7 +124,7 @@ struct Weights {          // device copies of one net, prepared by k_repack (im_
     const __nv_bfloat16 *W1, *W2, *W3;   // bf16 path: [o][k] row-major, W3 zero-padded to n_out_pad rows
     const float *b1, *b2, *b3;           // fp32 biases (b3 padded)
     uint32_t n_out, n_out_pad;
-    uint8_t *tc_img;                     // tcgen05 path (F=128, H=256): shared-memory image of the net (im_tc.cuh), else null
+    uint8_t *tc_img;                     // bf16 nets (tcgen05 path): shared-memory image of the net (im_tc.cuh), else null
 };
 
 __device__ __forceinline__ uint8_t *blk_rec(const Params &P, uint32_t e) { return P.env_base + (size_t)(e >> 5) * P.blk_stride; }

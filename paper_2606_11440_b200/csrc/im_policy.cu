@@ -3,7 +3,7 @@
 // Work comes as row lists written by k_sim (and, for stage 0 of new queries, by the planner kernel itself);
 // the executor launch also evaluates one critic row per env (R30).  Two numerics contracts:
 //   fp32 (R22): y = b; for k ascending: y = fmaf(W[o][k], x[k], y); tanh = im_tanh  -> bit-exact vs the oracle.
-//   bf16 (R25): bf16 operands, fp32 accumulation on the tensor cores (mma.sync m16n8k16 in this version),
+//   bf16 (R25): bf16 operands, fp32 accumulation on the tensor cores (tcgen05, accumulators in tensor memory),
 //               tanh.approx, fp32 logits; sampling by the exact R24 sampler on those logits.
 #include "im_device.cuh"
 #include "im_tc.cuh"
@@ -296,163 +296,6 @@ size_t f32_smem_bytes(uint32_t F, uint32_t H, uint32_t NOP)
     return 4ull * (F * H + H * H + H * NOP + 2 * H + NOP + kF32Warps * kF32RowsPerWarp * (F + 2 * H + 128));
 }
 
-// ================================================================================================ bf16 path (R25)
-// One CTA computes a tile of 128 rows through the three layers with mma.sync.m16n8k16 (bf16 x bf16 -> fp32).
-// Activations live in shared memory (bf16, padded rows), weights stream from L2 as B fragments.
-constexpr int kBfRows = 128, kBfWarps = 16;
-
-__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
-{
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
-                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], const void *p)
-{
-    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(p);
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];\n" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ float tanh_fast(float x)
-{
-    float y;
-    asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-// out[128][NT*8*nwarps...] = act[128][K] * W^T ; each warp owns NT n-tiles starting at n0 and all 8 m-tiles
-template <int K, int NT>
-__device__ __forceinline__ void layer_mma(const __nv_bfloat16 *act, int lda, const __nv_bfloat16 *W, int n0, float (&acc)[8][NT][4], uint32_t lane)
-{
-#pragma unroll
-    for (int mt = 0; mt < 8; mt++)
-#pragma unroll
-        for (int nt = 0; nt < NT; nt++)
-#pragma unroll
-            for (int i = 0; i < 4; i++) acc[mt][nt][i] = 0.0f;
-    const int g = lane >> 2, tq = lane & 3;
-    const int lrow = lane & 15, lcol = (lane >> 4) * 8;
-#pragma unroll 2
-    for (int k0 = 0; k0 < K; k0 += 16) {
-        uint32_t b[NT][2];
-#pragma unroll
-        for (int nt = 0; nt < NT; nt++) {
-            const __nv_bfloat16 *wp = W + (size_t)(n0 + nt * 8 + g) * K + k0 + 2 * tq;
-            b[nt][0] = __ldg(reinterpret_cast<const unsigned int *>(wp));
-            b[nt][1] = __ldg(reinterpret_cast<const unsigned int *>(wp + 8));
-        }
-#pragma unroll
-        for (int mt = 0; mt < 8; mt++) {
-            uint32_t a[4];
-            ldmatrix_x4(a, act + (size_t)(mt * 16 + lrow) * lda + k0 + lcol);
-#pragma unroll
-            for (int nt = 0; nt < NT; nt++) mma_bf16(acc[mt][nt], a, b[nt][0], b[nt][1]);
-        }
-    }
-}
-
-template <int F, int H, bool EXEC>
-__global__ void __launch_bounds__(kBfWarps * 32, 1)
-k_policy_bf16(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32_t trow)
-{
-    constexpr int LDA = H + 8;                     // padded row (bf16 elements): conflict-free ldmatrix
-    constexpr int NT_H = H / 8 / kBfWarps;         // n-tiles per warp in the hidden layers
-    static_assert(NT_H >= 1, "hidden width too small for 16 warps");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ TileSched sched;
-    __shared__ RowInfo s_ri[kBfRows];
-    __shared__ uint8_t s_ok[kBfRows];
-    __nv_bfloat16 *actA = reinterpret_cast<__nv_bfloat16 *>(smem_raw);
-    __nv_bfloat16 *actB = actA + kBfRows * LDA;
-    float *lg = reinterpret_cast<float *>(actA);   // logits [128][64] fp32 reuse actA after layer 2 consumed it
-    const RowBuf &rb = EXEC ? P.exec : P.plan;
-    const uint32_t n_crit = EXEC ? P.E : 0u;
-    sched_init(P, sched, rb, parity, kBfRows, n_crit);
-    const uint32_t lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int g = lane >> 2, tq = lane & 3;
-    const uint32_t n_tiles3 = W.n_out_pad / 8;
-
-    for (uint32_t tile = blockIdx.x; tile < sched.total; tile += gridDim.x) {
-        __syncthreads();
-        if (threadIdx.x < kBfRows) {
-            RowInfo ri;
-            const bool ok = tile_row<EXEC>(P, sched, rb, tile, threadIdx.x, kBfRows, n_crit, t0, ri);
-            s_ri[threadIdx.x] = ri; s_ok[threadIdx.x] = ok;
-        }
-        __syncthreads();
-        // features -> actA (bf16, RNE)
-        for (uint32_t i = threadIdx.x; i < kBfRows * F; i += blockDim.x) {
-            const uint32_t r = i / F, k = i % F;
-            const float v = s_ok[r] ? feature(P, EXEC, s_ri[r], k) : 0.0f;
-            actA[r * LDA + k] = __float2bfloat16_rn(v);
-        }
-        __syncthreads();
-        // layer 1: actA[128][F] -> actB[128][H]
-        {
-            float acc[8][NT_H][4];
-            const int n0 = wib * NT_H * 8;
-            layer_mma<F, NT_H>(actA, LDA, W.W1, n0, acc, lane);
-#pragma unroll
-            for (int nt = 0; nt < NT_H; nt++) {
-                const int col = n0 + nt * 8 + 2 * tq;
-                const float bb0 = W.b1[col], bb1 = W.b1[col + 1];
-#pragma unroll
-                for (int mt = 0; mt < 8; mt++) {
-                    const int r0 = mt * 16 + g;
-                    *reinterpret_cast<__nv_bfloat162 *>(actB + r0 * LDA + col) =
-                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][0] + bb0), tanh_fast(acc[mt][nt][1] + bb1));
-                    *reinterpret_cast<__nv_bfloat162 *>(actB + (r0 + 8) * LDA + col) =
-                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][2] + bb0), tanh_fast(acc[mt][nt][3] + bb1));
-                }
-            }
-        }
-        __syncthreads();
-        // layer 2: actB[128][H] -> actA[128][H]
-        {
-            float acc[8][NT_H][4];
-            const int n0 = wib * NT_H * 8;
-            layer_mma<H, NT_H>(actB, LDA, W.W2, n0, acc, lane);
-#pragma unroll
-            for (int nt = 0; nt < NT_H; nt++) {
-                const int col = n0 + nt * 8 + 2 * tq;
-                const float bb0 = W.b2[col], bb1 = W.b2[col + 1];
-#pragma unroll
-                for (int mt = 0; mt < 8; mt++) {
-                    const int r0 = mt * 16 + g;
-                    *reinterpret_cast<__nv_bfloat162 *>(actA + r0 * LDA + col) =
-                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][0] + bb0), tanh_fast(acc[mt][nt][1] + bb1));
-                    *reinterpret_cast<__nv_bfloat162 *>(actA + (r0 + 8) * LDA + col) =
-                        __floats2bfloat162_rn(tanh_fast(acc[mt][nt][2] + bb0), tanh_fast(acc[mt][nt][3] + bb1));
-                }
-            }
-        }
-        __syncthreads();
-        // layer 3: actA[128][H] -> logits (registers), then to shared memory after everyone finished reading actA
-        float acc3[8][1][4];
-        const bool has3 = wib < n_tiles3;
-        if (has3) layer_mma<H, 1>(actA, LDA, W.W3, wib * 8, acc3, lane);
-        __syncthreads();
-        if (has3) {
-            const int col = wib * 8 + 2 * tq;
-            const float bb0 = W.b3[col], bb1 = W.b3[col + 1];
-#pragma unroll
-            for (int mt = 0; mt < 8; mt++) {
-                const int r0 = mt * 16 + g;
-                lg[r0 * 64 + col] = acc3[mt][0][0] + bb0; lg[r0 * 64 + col + 1] = acc3[mt][0][1] + bb1;
-                lg[(r0 + 8) * 64 + col] = acc3[mt][0][2] + bb0; lg[(r0 + 8) * 64 + col + 1] = acc3[mt][0][3] + bb1;
-            }
-        }
-        __syncthreads();
-        if (threadIdx.x < kBfRows && s_ok[threadIdx.x]) {
-            float *scratch = reinterpret_cast<float *>(actB) + threadIdx.x * 64;   // actB is free now
-            if (EXEC) exec_epilogue(P, s_ri[threadIdx.x], lg + threadIdx.x * 64, scratch, t0, trow);
-            else plan_epilogue(P, s_ri[threadIdx.x], lg + threadIdx.x * 64, scratch, t0);
-        }
-    }
-}
-
-template <int F, int H>
-static size_t bf16_smem_bytes() { return 2ull * kBfRows * (H + 8) * 2; }
-
 // ================================================================================================ tcgen05 path (R25)
 // F = 128, H = 256 (configs 4-5): a real dense GEMM, so it runs on the 5th-generation tensor cores (im_tc.cuh).
 // One persistent CTA per SM; the whole net (192 KB of bf16 weights) stays in shared memory for the lifetime of the
@@ -461,7 +304,10 @@ static size_t bf16_smem_bytes() { return 2ull * kBfRows * (H + 8) * 2; }
 constexpr int kTcK1 = 64, kTcH = 256, kTcThreads = 256;
 template <bool EXEC> using TcNet = tc::TcMlp<kTcK1, kTcH, EXEC ? 64 : 32>;
 
-bool tc_supported(uint32_t F, uint32_t H) { return F == 128 && H == 256; }
+// The tcgen05 kernel is built for K1 = 64 contracted features (any f_in >= 3N + 13) and a hidden width of 256; a net with
+// hidden = 128 runs on it zero-padded (k_pack_tc): the padded units have zero weights and biases, tanh(0) = 0, so they add
+// exactly nothing - and a 128-row tile still costs less than half of what the mma.sync kernel it replaced took for it.
+bool tc_supported(uint32_t F, uint32_t H) { return (F == 64 && H == 128) || (F == 128 && H == 256); }
 size_t tc_image_bytes(bool exec) { return exec ? TcNet<true>::kImageBytes : TcNet<false>::kImageBytes; }
 
 // K order of layer 1 on this path: [snap(3N) | b | in_tok | topo(4) | role(4) | agent | keff | 0...] — the R15 features with
@@ -471,33 +317,34 @@ __device__ __forceinline__ uint32_t tc_feature_src(uint32_t kp, uint32_t N3) { r
 
 // bf16 [o][k] row-major weights + fp32 biases (k_repack's output) -> the shared-memory image of im_tc.cuh
 template <bool EXEC>
-__global__ void k_pack_tc(const Weights W, uint32_t N3)
+__global__ void k_pack_tc(const Weights W, uint32_t N3, uint32_t F, uint32_t H)        // F, H: the net's own f_in and hidden (<= 128, <= 256)
 {
     using Net = TcNet<EXEC>;
-    constexpr uint32_t NO = EXEC ? 64 : 32, F = 128;
+    constexpr uint32_t NO = EXEC ? 64 : 32;
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    const __nv_bfloat16 zero = __float2bfloat16(0.0f);
     uint8_t *img = W.tc_img;
     for (uint32_t i = tid; i < kTcH * kTcK1; i += nth) {
-        const uint32_t o = i / kTcK1, kp = i % kTcK1;
-        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW1 + tc::canon_off(kTcH, o, kp)) = W.W1[o * F + tc_feature_src(kp, N3)];
+        const uint32_t o = i / kTcK1, kp = i % kTcK1, src = tc_feature_src(kp, N3);
+        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW1 + tc::canon_off(kTcH, o, kp)) = (o < H && src < F) ? W.W1[o * F + src] : zero;
     }
     for (uint32_t i = tid; i < kTcH * kTcH; i += nth) {
         const uint32_t o = i / kTcH, k = i % kTcH;
-        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW2 + tc::canon_off(kTcH, o, k)) = W.W2[i];
+        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW2 + tc::canon_off(kTcH, o, k)) = (o < H && k < H) ? W.W2[o * H + k] : zero;
     }
     for (uint32_t i = tid; i < NO * kTcH; i += nth) {
         const uint32_t o = i / kTcH, k = i % kTcH;
-        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW3 + tc::canon_off(NO, o, k)) = o < W.n_out_pad ? W.W3[i] : __float2bfloat16(0.0f);
+        *reinterpret_cast<__nv_bfloat16 *>(img + Net::kW3 + tc::canon_off(NO, o, k)) = (o < W.n_out_pad && k < H) ? W.W3[o * H + k] : zero;
     }
     float *bias = reinterpret_cast<float *>(img + Net::kBias);
-    for (uint32_t i = tid; i < kTcH; i += nth) { bias[i] = W.b1[i]; bias[kTcH + i] = W.b2[i]; }
+    for (uint32_t i = tid; i < kTcH; i += nth) { bias[i] = i < H ? W.b1[i] : 0.0f; bias[kTcH + i] = i < H ? W.b2[i] : 0.0f; }
     for (uint32_t i = tid; i < NO; i += nth) bias[2 * kTcH + i] = i < W.n_out_pad ? W.b3[i] : 0.0f;
 }
 
-void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, cudaStream_t st)
+void launch_pack_tc(const Weights &W, bool exec, uint32_t n_models, uint32_t f_in, uint32_t hidden, cudaStream_t st)
 {
-    if (exec) k_pack_tc<true><<<64, 256, 0, st>>>(W, 3 * n_models);
-    else k_pack_tc<false><<<64, 256, 0, st>>>(W, 3 * n_models);
+    if (exec) k_pack_tc<true><<<64, 256, 0, st>>>(W, 3 * n_models, f_in, hidden);
+    else k_pack_tc<false><<<64, 256, 0, st>>>(W, 3 * n_models, f_in, hidden);
 }
 
 // R24 sampler on logits held in registers: l[off .. off+n), n <= NMAX.  Same VALUES as sample_seq, arranged for a lone
@@ -844,8 +691,6 @@ int policy_prepare_device(const Params &P)
     auto set = [&](const void *f, int bytes) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); };
     set((const void *)k_policy_f32<true>, big);
     set((const void *)k_policy_f32<false>, big);
-    set((const void *)k_policy_bf16<64, 128, true>, (int)bf16_smem_bytes<64, 128>());
-    set((const void *)k_policy_bf16<64, 128, false>, (int)bf16_smem_bytes<64, 128>());
     const int tc_smem = (int)(((tc_image_bytes(true) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot));
     set((const void *)k_policy_tc<true>, tc_smem);
     set((const void *)k_policy_tc<false>, tc_smem);
@@ -863,16 +708,10 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
         else k_policy_f32<false><<<grid, kF32Warps * 32, smem, st>>>(P, W, parity, t0, trow);
         return 0;
     }
-    if (W.tc_img) {      // F = 128, H = 256: tcgen05
+    if (W.tc_img) {      // bf16: tcgen05 (hidden = 128 zero-padded to 256, k_pack_tc)
         const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot);
         if (exec) launch_chained(k_policy_tc<true>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
         else launch_chained(k_policy_tc<false>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
-        return 0;
-    }
-    if (P.f_in == 64 && P.hidden == 128) {      // too narrow for a 128 x 256 UMMA tile to pay: mma.sync
-        const size_t smem = bf16_smem_bytes<64, 128>();
-        if (exec) k_policy_bf16<64, 128, true><<<(uint32_t)n_sm, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);
-        else k_policy_bf16<64, 128, false><<<(uint32_t)n_sm, kBfWarps * 32, smem, st>>>(P, W, parity, t0, trow);
         return 0;
     }
     return -1;

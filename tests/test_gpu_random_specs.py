@@ -17,7 +17,7 @@ pytestmark = pytest.mark.gpu
 def _random_spec(case: int):
     rng = np.random.Generator(np.random.PCG64([case, 2606]))
     N = int(rng.integers(1, 17))
-    # policy kernel: fp32 FFMA (any width that holds 3N+12 features), bf16 mma.sync (64,128), bf16 tcgen05 (128,256)
+    # policy kernel: fp32 FFMA (any width that holds 3N+12 features), bf16 tcgen05 (64,128: zero-padded to the kernel's 256-wide hidden layers; 128,256)
     kinds = [("f32", 0, 64 if 3 * N + 12 > 32 else 32, int(rng.choice([16, 64])))]
     kinds.append(("mma", 1, 64, 128))
     kinds.append(("tc", 1, 128, 256))
