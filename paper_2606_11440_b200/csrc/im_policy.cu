@@ -306,7 +306,8 @@ template <bool EXEC> using TcNet = tc::TcMlp<kTcK1, kTcH, EXEC ? 64 : 32>;
 
 // The tcgen05 kernel is built for K1 = 64 contracted features (any f_in >= 3N + 13) and a hidden width of 256; a net with
 // hidden = 128 runs on it zero-padded (k_pack_tc): the padded units have zero weights and biases, tanh(0) = 0, so they add
-// exactly nothing - and a 128-row tile still costs less than half of what the mma.sync kernel it replaced took for it.
+// exactly nothing - and the kernel skips them: only the first N-half of the hidden layers and half of the K-steps of layers 2
+// and 3 are issued, only the first half of the tanh epilogues runs (`narrow`).
 bool tc_supported(uint32_t F, uint32_t H) { return (F == 64 && H == 128) || (F == 128 && H == 256); }
 size_t tc_image_bytes(bool exec) { return exec ? TcNet<true>::kImageBytes : TcNet<false>::kImageBytes; }
 
@@ -443,7 +444,7 @@ __device__ __forceinline__ RowInfo tc_decode_row(const Params &P, const TcRaw &x
 // Row handed from the gathering warpgroup to the sampling warpgroup through shared memory
 struct TcRowSlot { uint4 row; uint32_t env, gidx, flags, pad; };           // flags: bit 0 ok, bit 1 critic
 
-template <bool EXEC>
+template <bool EXEC, bool NARROW>
 __global__ void __launch_bounds__(kTcThreads, 1)
 k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32_t trow)
 {
@@ -479,6 +480,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
     const uint32_t warp_u = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);      //  the UMMA operands then live in uniform registers)
     const uint32_t N3 = 3 * P.N;
     const bool vec = (N3 % 8u) == 0;                      // snapshot block = whole 16-byte chunks (N = 8, 16)
+    constexpr bool narrow = NARROW;                       // a 128-wide net on the 256-wide kernel: half a of the hidden layers only
     const uint32_t wg = warp_u >> 2, r = threadIdx.x & 127u;
     const uint32_t tlane = tmem_base + (((threadIdx.x >> 5) & 3u) * 32u << 16);
     const float *bias = reinterpret_cast<const float *>(img + Net::kBias);
@@ -556,7 +558,7 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             tc::fence_proxy_async_smem();
             tc::bar_sync(4, 128);
             tc::mbar_wait(&wbar, 0);
-            if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
+            if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1], narrow);
             nxt = tc_fetch_row(sched, rb, blockIdx.x + gridDim.x, r, n_crit);
             fetch_snap(nxt, sn);
             nxt2 = tc_fetch_row(sched, rb, blockIdx.x + 2 * gridDim.x, r, n_crit);
@@ -572,21 +574,23 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
             tc::mbar_wait(&bars[0], phase);
             tc::tc_fence_after();
             Net::half_epilogue(tlane, 0, 0, bias);
-            tc::mbar_wait(&bars[1], phase);
-            tc::tc_fence_after();
-            Net::half_epilogue(tlane, 128, 64, bias + 128);
+            if (!narrow) {
+                tc::mbar_wait(&bars[1], phase);
+                tc::tc_fence_after();
+                Net::half_epilogue(tlane, 128, 64, bias + 128);
+            }
             tc::tc_fence_before();
             tc::bar_sync(2, 128);
             // layer 2 overwrites D3 / A3 of the previous tile: wait until warpgroup 0 has its logits in registers
             if (it > 0) tc::bar_sync(3, 256);
-            if (warp_u == 4) Net::issue_l2(img, tmem_base, &bars[2], &bars[3]);
+            if (warp_u == 4) Net::issue_l2(img, tmem_base, &bars[2], &bars[3], narrow);
             // the next tile: features (layer 1 of this tile is done with a1), layer 1 behind layer 2 in the tensor pipe
             // (UMMAs of one thread execute in order, so A2 is consumed by then), row loads of the tile after it
             if (tile + gridDim.x < total) {
                 build_a1(nxt, sn, rowbuf + 128 * ((it + 1) & 1u));
                 tc::fence_proxy_async_smem();
                 tc::bar_sync(4, 128);
-                if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1]);
+                if (warp_u == 4) Net::issue_l1(img, a1, tmem_base, &bars[0], &bars[1], narrow);
                 nxt = nxt2;                                   // row of tile + 2 grids: its load went out one tile ago
                 fetch_snap(nxt, sn);
                 nxt2 = tc_fetch_row(sched, rb, tile + 3 * gridDim.x, r, n_crit);
@@ -598,12 +602,14 @@ k_policy_tc(const Params P, const Weights W, uint32_t parity, int32_t t0, uint32
         tc::mbar_wait(&bars[2], phase);
         tc::tc_fence_after();
         Net::half_epilogue(tlane, Net::kColD2, Net::kColD2, bias + kTcH);
-        tc::mbar_wait(&bars[3], phase);
-        tc::tc_fence_after();
-        Net::half_epilogue(tlane, Net::kColD2 + 128, Net::kColD2 + 128, bias + kTcH + 128);
+        if (!narrow) {
+            tc::mbar_wait(&bars[3], phase);
+            tc::tc_fence_after();
+            Net::half_epilogue(tlane, Net::kColD2 + 128, Net::kColD2 + 128, bias + kTcH + 128);
+        }
         tc::tc_fence_before();
         tc::bar_sync(5, 128);
-        if (warp_u == 0) Net::issue_l3(img, tmem_base, &bars[4]);
+        if (warp_u == 0) Net::issue_l3(img, tmem_base, &bars[4], narrow);
         // ---- warpgroup 0: sampling epilogue of row r, logits in registers
         const TcRowSlot sl = rowbuf[128 * (it & 1u) + r];
         uint32_t islot = ~0u;                              // executor rows: the env's issue-list slot, claimed before the wait
@@ -692,8 +698,10 @@ int policy_prepare_device(const Params &P)
     set((const void *)k_policy_f32<true>, big);
     set((const void *)k_policy_f32<false>, big);
     const int tc_smem = (int)(((tc_image_bytes(true) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot));
-    set((const void *)k_policy_tc<true>, tc_smem);
-    set((const void *)k_policy_tc<false>, tc_smem);
+    set((const void *)k_policy_tc<true, false>, tc_smem);
+    set((const void *)k_policy_tc<false, false>, tc_smem);
+    set((const void *)k_policy_tc<true, true>, tc_smem);
+    set((const void *)k_policy_tc<false, true>, tc_smem);
     (void)P;
     return e == cudaSuccess ? 0 : -1;
 }
@@ -710,8 +718,14 @@ int launch_policy(const Params &P, const Weights &W, bool exec, uint32_t parity,
     }
     if (W.tc_img) {      // bf16: tcgen05 (hidden = 128 zero-padded to 256, k_pack_tc)
         const size_t smem = ((tc_image_bytes(exec) + 1023u) & ~(size_t)1023u) + TcNet<true>::kA1Bytes + 2 * 128 * sizeof(TcRowSlot);
-        if (exec) launch_chained(k_policy_tc<true>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
-        else launch_chained(k_policy_tc<false>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
+        const bool narrow = P.hidden <= 128;             // template parameter: the wide kernel compiles without a trace of it
+        if (exec) {
+            if (narrow) launch_chained(k_policy_tc<true, true>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
+            else launch_chained(k_policy_tc<true, false>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
+        } else {
+            if (narrow) launch_chained(k_policy_tc<false, true>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
+            else launch_chained(k_policy_tc<false, false>, dim3(n_sm), dim3(kTcThreads), smem, st, true, P, W, parity, t0, trow);
+        }
         return 0;
     }
     return -1;

@@ -225,13 +225,17 @@ struct TcMlp {
     }
 
     // ---- UMMA issue: called by ONE CONVERGED WARP, one elected lane issues.  Layer 1 (SS): A1 in shared memory (canonical [128][K1]) x W1 -> D1, two halves.
-    static __device__ __forceinline__ void issue_l1(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
+    // `narrow` (a net with 128 hidden units on this 256-wide kernel): the units are the first N-half of every layer and the
+    // first half of the next layer's K, so only half a of layers 1 and 2 and 8 of the 16 K-steps of layers 2 and 3 are issued
+    // (the other halves of the padded image are zeros and would add exactly nothing).
+    static __device__ __forceinline__ void issue_l1(const uint8_t *image, const uint8_t *a1, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b, bool narrow)
     {
         tc_fence_after();
         const uint32_t sa = smem_u32(a1), sb = smem_u32(image + kW1);
         if (elect_one()) {
 #pragma unroll
             for (int h = 0; h < 2; h++) {
+                if (h == 1 && narrow) break;
 #pragma unroll
                 for (int k = 0; k < K1 / 16; k++)
                     umma_ss(tmem_base + 128 * h, smem_desc(sa + k * 2 * 128 * 16, 128 * 16, 128),
@@ -242,30 +246,31 @@ struct TcMlp {
         __syncwarp();
     }
     // Layer 2 (TS): A2 (TMEM cols [0,128), 8 columns per K-chunk) x W2 -> D2 = [256,512), two N-halves
-    static __device__ __forceinline__ void issue_l2(const uint8_t *image, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b)
+    static __device__ __forceinline__ void issue_l2(const uint8_t *image, uint32_t tmem_base, uint64_t *bar_a, uint64_t *bar_b, bool narrow)
     {
         tc_fence_after();
         const uint32_t sb = smem_u32(image + kW2);
         if (elect_one()) {
 #pragma unroll
             for (int h = 0; h < 2; h++) {
+                if (h == 1 && narrow) break;
 #pragma unroll
                 for (int k = 0; k < H / 16; k++)
-                    umma_ts(tmem_base + kColD2 + 128 * h, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
+                    if (!(narrow && k >= H / 32)) umma_ts(tmem_base + kColD2 + 128 * h, tmem_base + 8 * k, smem_desc(sb + k * 2 * H * 16 + h * 128 * 16, H * 16, 128), kIdescHalf, k > 0);
                 umma_commit(h ? bar_b : bar_a);
             }
         }
         __syncwarp();
     }
     // Layer 3 (TS): A3 (K-chunks 0-7 at [256,320), 8-15 at [384,448)) x W3 -> D3 = [448,448+NO)
-    static __device__ __forceinline__ void issue_l3(const uint8_t *image, uint32_t tmem_base, uint64_t *bar)
+    static __device__ __forceinline__ void issue_l3(const uint8_t *image, uint32_t tmem_base, uint64_t *bar, bool narrow)
     {
         tc_fence_after();
         const uint32_t sb = smem_u32(image + kW3);
         if (elect_one()) {
 #pragma unroll
             for (int k = 0; k < H / 16; k++)
-                umma_ts(tmem_base + kColD3, tmem_base + kColD2 + (k < 8 ? 8 * k : 128 + 8 * (k - 8)), smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
+                if (!(narrow && k >= H / 32)) umma_ts(tmem_base + kColD3, tmem_base + kColD2 + (k < 8 ? 8 * k : 128 + 8 * (k - 8)), smem_desc(sb + k * 2 * NO * 16, NO * 16, 128), kIdescOut, k > 0);
             umma_commit(bar);
         }
         __syncwarp();
